@@ -1,0 +1,16 @@
+"""fp64 CPU oracle of the RCA Stage-1 projection beamformer -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package (see oracle/ulm_oracle.h).  It imports nothing
+from ``paper_2511_21647_b200`` and the CUDA path imports nothing from here.
+"""
+from .oracle import (  # noqa: F401
+    OracleParams,
+    beamform,
+    build,
+    das_points,
+    demod_channel,
+    fir_taps,
+    threads,
+    volume,
+)
