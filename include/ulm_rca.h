@@ -1,0 +1,156 @@
+/*
+ * ulm_rca.h -- C-ABI boundary of the B200 (sm_100a) RCA projection beamformer.
+ *
+ * The library computes the Stage-1 "2D beamforming step" of the projection-based 3-D ULM pipeline of
+ * arxiv 2511.21647 (Section II.A.1; acquisition geometry PAPER.md:113-117): row-column
+ * array (RCA) delay-and-sum beamforming of multi-angle plane-wave channel data straight into per-frame
+ * 2-D images -- the x-z image from the row-transmit events (received on the columns) and the y-z image
+ * from the column-transmit events (received on the rows), "x-z plane for RC and y-z plane for CR"
+ * (Fig. 1d) -- coherently compounded over the steering angles, with no 3-D volume written
+ * to memory.  The paper prints no formula for this step; the exact definition implemented here is
+ * DESIGN.md "Definition" (= SURVEY.md section 8(c)):
+ *
+ *   step 0 (RF input)  x[n] = rf[n] exp(-j 2 pi fc t_n), t_n = t_start + n/fs;
+ *                      iq[n] = 2 sum_{m=-L..L} h[m] x[n-m]  (x = 0 outside the record),
+ *                      h[m] ~ sinc(2 fc m/fs) (0.54 + 0.46 cos(pi m/L)), sum h = 1, L = (demod_taps-1)/2
+ *   step 1 (x-z image) for pixel (x, z), row-tx angle th_k, column j at x_j:
+ *                      tau = t0_k + (z cos th_k + y_ref sin th_k)/c + sqrt((x - x_j)^2 + z^2)/c
+ *                      u = (tau - t_start) fs, n = floor(u), a = u - n   (term = 0 unless 0 <= n <= Ns-2)
+ *                      P_xz(x, z) = sum_k sum_j w_j(x, z) ((1-a) iq_kj[n] + a iq_kj[n+1]) exp(+j 2 pi fc tau)
+ *                      w_j = elem_window[j] * [f_number == 0 or |x - x_j| <= z / (2 f_number)]
+ *   step 2 (y-z image) the same with x <-> y, columns <-> rows, x_ref for y_ref, grid_yz
+ *   step 3             compound == 0: the k-sum is not taken (the paper's per-transmission slices S_k)
+ *   step 4 (volume)    the same DAS at every voxel (x, y, z) for all events, V = V_RC + V_CR
+ *                      (the "conventional 3D processing" the paper compares against)
+ *
+ * All pointers named d_* are DEVICE pointers owned by the caller; all other pointers are HOST pointers
+ * that are only read during the call (the caller may free them at once).  No call throws, exits or
+ * prints; failures are a status code plus ulm_rca_last_error().  There is no CPU fallback: without a
+ * CUDA device every call that needs one fails with ULM_RCA_ECUDA.
+ */
+#ifndef ULM_RCA_H
+#define ULM_RCA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ulm_rca_plan ulm_rca_plan; /* opaque, owned by the library */
+
+typedef enum {
+    ULM_RCA_OK = 0,
+    ULM_RCA_EINVAL = 1,       /* NULL / non-finite / non-positive argument, inconsistent sizes        */
+    ULM_RCA_ENOMEM = 2,       /* host or device allocation failed                                      */
+    ULM_RCA_ECUDA = 3,        /* CUDA runtime error (text in ulm_rca_last_error)                       */
+    ULM_RCA_EUNSUPPORTED = 4  /* valid request outside what the kernels cover                          */
+} ulm_rca_status;
+
+/* Array geometry (128 + 128 elements, pitch 0.214 mm).  Rows are long in x and indexed
+ * along y, columns are long in y and indexed along x; element e of n sits at (e - (n-1)/2) * pitch. */
+typedef struct {
+    int32_t n_rows, n_cols;
+    float pitch_m;
+} ulm_rca_geometry;
+
+/* One image grid: pixel (il, iz) is at lateral lat0_m + il*dlat_m (x for the x-z image, y for the y-z
+ * image; dlat_m may be negative) and depth z0_m + iz*dz_m (z >= 0, dz_m > 0).  ref_m is the coordinate
+ * of the reference slice along the transmit direction (y_ref for x-z, x_ref for y-z): the "central
+ * slices along the transmit directions" of PAPER.md:31 (Fig. 1b) are ref_m = 0. */
+typedef struct {
+    int32_t n_lat;
+    float lat0_m, dlat_m;
+    int32_t n_ax;
+    float z0_m, dz_m;
+    float ref_m;
+} ulm_rca_grid;
+
+typedef struct {
+    int32_t input_kind;         /* 0 = RF int16 real, 1 = IQ int16 interleaved (re, im)                */
+    int32_t channels_per_event; /* n_rows + n_cols (rows first; only the aperture orthogonal to the
+                                   transmitting one is read), or, when n_rows == n_cols, n_rows
+                                   (orthogonal aperture only); 0 = n_rows + n_cols                     */
+    int32_t n_samples;          /* samples per channel record (Ns >= 2)                                */
+    float t_start_s;            /* time of sample 0                                                    */
+    const float *t0_s;          /* HOST [n_row_tx + n_col_tx] per-event time offset, NULL = 0          */
+    float f_number;             /* 0 = full aperture                                                   */
+    const float *elem_window;   /* HOST [n_cols] weights of the column aperture (x-z image) followed by
+                                   [n_rows] of the row aperture (y-z image); NULL = all ones           */
+    int32_t demod_taps;         /* odd FIR length 2L+1; 0 = default 4*round(fs/fc)+1                   */
+    int32_t compound;           /* 1 = sum over angles; 0 = one slice per event                        */
+    int32_t max_frames;         /* largest n_frames a call will pass (sizes the plan's IQ scratch);
+                                   0 = 32.  Larger calls are processed in batches of this size.        */
+    int32_t build_volume;       /* 1 = also prepare ulm_rca_beamform_volume (needs equal axial grids)  */
+    int32_t kernel;             /* 0 = auto; 1 = generic gather kernel; 2 = shared-memory ring kernel  */
+    int32_t reserved[5];        /* must be 0                                                           */
+} ulm_rca_options;
+
+/*
+ * Build a plan: validates the arguments, derives the touched sample range, builds the per-angle
+ * transmit-delay tables (fp64 on the host, split into integer + fraction), the demodulation filter and
+ * mixer, tile windows and launch geometry, uploads them and allocates the IQ scratch.
+ * Angles are in radians: row_tx_angles steer in the y-z plane, col_tx_angles in the x-z plane.
+ * Event order in the channel data is row-tx angles (as given) then column-tx angles.
+ * Either angle list may be empty (its image is then all zeros) but not both.
+ * On success *out receives the plan; on failure *out is NULL.
+ */
+ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geometry,
+                                   const float *row_tx_angles_rad, int32_t n_row_tx,
+                                   const float *col_tx_angles_rad, int32_t n_col_tx,
+                                   float c_mps, float fs_hz, float fc_hz,
+                                   const ulm_rca_grid *grid_xz, const ulm_rca_grid *grid_yz,
+                                   const ulm_rca_options *options, ulm_rca_plan **out);
+
+/*
+ * Beamform n_frames frames (steps 0-3).  Enqueues on cuda_stream (a cudaStream_t passed as void*, NULL =
+ * the legacy default stream) and returns without synchronising; results are valid once the caller has
+ * synchronised that stream.  Never allocates.
+ *   d_channel : int16 [frame][event][channel][sample] (x2 interleaved for IQ input), device memory
+ *   d_out     : complex fp32 (re, im), device memory,
+ *               compound == 1: [frame][ x-z: n_lat*n_ax | y-z: n_lat*n_ax ], axial index fastest
+ *               compound == 0: [frame][event][lat][ax]
+ * One call in flight per plan (the plan owns the IQ scratch).  n_frames == 0 is a no-op.
+ */
+ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel, int32_t n_frames,
+                                void *d_out, void *cuda_stream);
+
+/*
+ * Conventional full 3-D DAS (step 4) on the grid x = grid_xz lateral, y = grid_yz lateral, z = the
+ * (shared) axial grid: d_out_volume is complex fp32 [frame][x][y][z], z fastest.  Same stream and
+ * ownership rules as ulm_rca_beamform.  Needs options.build_volume = 1.
+ */
+ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_channel,
+                                       int32_t n_frames, void *d_out_volume, void *cuda_stream);
+
+/* Host convenience (this is the end-to-end call bench.py times as "e2e"): copies n_frames of HOST
+ * channel data to an internal device buffer, beamforms, copies the images back to HOST memory and
+ * synchronises.  Allocates device staging on first use (freed by plan_destroy). */
+ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, int32_t n_frames,
+                                     void *h_out);
+
+/* Byte sizes per frame of the three buffers above (any pointer may be NULL). */
+ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_bytes_per_frame,
+                                  size_t *out_bytes_per_frame, size_t *volume_bytes_per_frame);
+
+/* Plan facts for benchmarks and tests: fills up to n values of
+ *   [0] first touched sample  [1] touched samples per record  [2] IQ scratch bytes
+ *   [3] kernel in use (1/2)   [4] frames per thread (F)       [5] pixels per tile
+ *   [6] window entries per stage (W)  [7] ring stages  [8] tiles per projection (x-z)
+ *   [9] dynamic shared memory bytes   [10] kernels launched by the last beamform call
+ *   [11] tiles per projection (y-z) */
+ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
+
+/* FP32 FMA throughput probe used for the roofline denominator: runs a register-only FFMA loop on every
+ * SM on cuda_stream, synchronises, and returns the measured TFLOP/s (2 flop per FMA) in *tflops. */
+ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream);
+
+void ulm_rca_plan_destroy(ulm_rca_plan *plan); /* NULL-safe */
+
+const char *ulm_rca_last_error(void); /* thread-local, valid until the next failing call */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

