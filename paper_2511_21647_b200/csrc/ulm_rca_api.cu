@@ -449,6 +449,12 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
         launch_demod(P, in, nb, st);
+        for (int a = 0; a < 2; ++a) {     // an aperture without transmit events: its image is all zeros
+            const Aperture &A = P.ap[a];
+            if (A.n_tx == 0 && P.compound)
+                CUDA_TRY(cudaMemset2DAsync(outp + A.out_base, (size_t)P.out_per_frame * sizeof(float2), 0,
+                                           (size_t)A.g.n_lat * A.g.n_ax * sizeof(float2), nb, st));
+        }
         if (P.kernel == 2) {
             ulm::RingLaunch L{};
             L.iq = P.iq.as<float4>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.n_events;
