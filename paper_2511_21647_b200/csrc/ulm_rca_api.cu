@@ -14,7 +14,7 @@
 #include <vector>
 
 #include "ulm_rca_device.cuh"
-#include "ulm_rca_ring.cuh"
+#include "ulm_rca_ring_host.cuh"
 
 namespace {
 

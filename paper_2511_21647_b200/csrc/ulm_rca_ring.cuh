@@ -113,17 +113,6 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
     return v;
 }
 
-// shared-memory carve-up (bytes, from the dynamic base)
-template <int F, int WS>
-struct RingSmem {
-    static constexpr int kStageBytes = F * WS * 16;
-    static constexpr int kMisc = kRingMaxBt * 4 + 3 * kRingMaxRx * 4 + kRingMaxStages * 16 + 2 * kRingMaxStages * 8 + 64;
-    static constexpr int stages(int limit) {
-        int n = (limit - kMisc) / kStageBytes;
-        return n > kRingMaxStages ? kRingMaxStages : n;
-    }
-};
-
 template <int F, int WS, bool APOD>
 __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const RingLaunch P) {
     extern __shared__ __align__(128) unsigned char smem[];
