@@ -142,6 +142,12 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [11] tiles per projection (y-z) */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
+/* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this
+ * plan, from CUDA events the library records on the caller's stream around its launches (first 4 batches
+ * of each call): the demodulation/staging pre-pass and the DAS kernel(s).  Waits for those events; the
+ * beamform calls themselves never synchronise. */
+ulm_rca_status ulm_rca_plan_timing(const ulm_rca_plan *plan, int32_t n_calls, double *demod_ms, double *das_ms);
+
 /* FP32 FMA throughput probe used for the roofline denominator: runs a register-only FFMA loop on every
  * SM on cuda_stream, synchronises, and returns the measured TFLOP/s (2 flop per FMA) in *tflops. */
 ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream);

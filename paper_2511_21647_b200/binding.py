@@ -20,7 +20,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
 _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
-           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_fp32_peak", "ulm_rca_plan_destroy",
+           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
 
@@ -75,6 +75,8 @@ def load() -> C.CDLL:
     lib.ulm_rca_plan_sizes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
     lib.ulm_rca_plan_info.restype = C.c_int
     lib.ulm_rca_plan_info.argtypes = [vp, C.POINTER(C.c_int64), i32]
+    lib.ulm_rca_plan_timing.restype = C.c_int
+    lib.ulm_rca_plan_timing.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_plan_destroy.restype = None
@@ -162,6 +164,12 @@ class Plan:
         v = (C.c_int64 * len(INFO_KEYS))()
         _check(load().ulm_rca_plan_info(self._h, v, len(INFO_KEYS)))
         return dict(zip(INFO_KEYS, [int(x) for x in v]))
+
+    def timing(self, n_calls: int = 1) -> tuple:
+        """(demod_ms, das_ms): mean device time per call of the kernels of the last n_calls beamform() calls."""
+        d, g = C.c_double(), C.c_double()
+        _check(load().ulm_rca_plan_timing(self._h, int(n_calls), C.byref(d), C.byref(g)))
+        return d.value, g.value
 
     @property
     def out_complex_per_frame(self) -> int:

@@ -98,6 +98,15 @@ struct ulm_rca_plan {
     // host-convenience staging
     DeviceBuf h_stage_in, h_stage_out;
     size_t h_stage_frames = 0;
+    // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
+    // after DAS; the first kTimedBatches batches of a call)
+    static constexpr int kTimedCalls = 64, kTimedBatches = 4;
+    cudaEvent_t ev[kTimedCalls][kTimedBatches][3] = {};
+    mutable int timed_batches[kTimedCalls] = {};
+    mutable long long n_calls = 0;
+    ~ulm_rca_plan() {
+        for (auto &c : ev) for (auto &b : c) for (auto &e : b) if (e) cudaEventDestroy(e);
+    }
 };
 
 namespace {
@@ -408,6 +417,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     } else if (opt->kernel == 2) {
         return fail(ULM_RCA_EUNSUPPORTED, "the ring kernel covers compound = 1 only");
     }
+    for (auto &c : P.ev) for (auto &b : c) for (auto &e : b) CUDA_TRY(cudaEventCreate(&e));
     CUDA_TRY(cudaDeviceSynchronize());
     guard.p = nullptr;
     *out = Pp;
@@ -444,11 +454,17 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
     size_t ch_bytes = 0;
     ulm_rca_plan_sizes(plan, &ch_bytes, nullptr, nullptr);
     P.last_launches = 0;
+    const int slot = (int)(P.n_calls % ulm_rca_plan::kTimedCalls);
+    ++P.n_calls;
+    P.timed_batches[slot] = 0;
     for (int f0 = 0; f0 < n_frames; f0 += P.max_frames) {
         const int nb = std::min(P.max_frames, n_frames - f0);
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
+        const int tb = P.timed_batches[slot] < ulm_rca_plan::kTimedBatches ? P.timed_batches[slot] : -1;
+        if (tb >= 0) cudaEventRecord(P.ev[slot][tb][0], st);
         launch_demod(P, in, nb, st);
+        if (tb >= 0) cudaEventRecord(P.ev[slot][tb][1], st);
         for (int a = 0; a < 2; ++a) {     // an aperture without transmit events: its image is all zeros
             const Aperture &A = P.ap[a];
             if (A.n_tx == 0 && P.compound)
@@ -480,8 +496,29 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
                 launch_generic(P, D, nb, st);
             }
         }
+        if (tb >= 0) { cudaEventRecord(P.ev[slot][tb][2], st); P.timed_batches[slot] = tb + 1; }
     }
     CUDA_TRY(cudaGetLastError());
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_plan_timing(const ulm_rca_plan *plan, int32_t n_calls, double *demod_ms, double *das_ms) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (n_calls < 1 || n_calls > ulm_rca_plan::kTimedCalls || n_calls > plan->n_calls)
+        return fail(ULM_RCA_EINVAL, "n_calls must be 1..min(64, calls made)");
+    double d = 0, g = 0;
+    for (int c = 1; c <= n_calls; ++c) {
+        const int slot = (int)((plan->n_calls - c) % ulm_rca_plan::kTimedCalls);
+        for (int b = 0; b < plan->timed_batches[slot]; ++b) {
+            float a = 0, e = 0;
+            CUDA_TRY(cudaEventSynchronize(plan->ev[slot][b][2]));
+            CUDA_TRY(cudaEventElapsedTime(&a, plan->ev[slot][b][0], plan->ev[slot][b][1]));
+            CUDA_TRY(cudaEventElapsedTime(&e, plan->ev[slot][b][1], plan->ev[slot][b][2]));
+            d += a; g += e;
+        }
+    }
+    if (demod_ms) *demod_ms = d / n_calls;
+    if (das_ms) *das_ms = g / n_calls;
     return ULM_RCA_OK;
 }
 
