@@ -84,7 +84,12 @@ typedef struct {
                                    0 = 32.  Larger calls are processed in batches of this size.        */
     int32_t build_volume;       /* 1 = also prepare ulm_rca_beamform_volume (needs equal axial grids)  */
     int32_t kernel;             /* 0 = auto; 1 = generic gather kernel; 2 = shared-memory ring kernel  */
-    int32_t reserved[5];        /* must be 0                                                           */
+    int32_t precision;          /* storage of the interpolation difference term iq[n+1] - iq[n] in the
+                                   staged IQ scratch: 1 = compact (fp16; error <= ~2^-13 |difference|
+                                   per term: meant for band-limited data), 2 = full (fp32), 0 = auto:
+                                   compact for RF input (the library's own low-pass band-limits it),
+                                   full for IQ input (spectrum unknown)                                 */
+    int32_t reserved[4];        /* must be 0                                                           */
 } ulm_rca_options;
 
 /*
@@ -139,7 +144,8 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [3] kernel in use (1/2)   [4] frames per thread (F)       [5] pixels per tile
  *   [6] window entries per stage (W)  [7] ring stages  [8] tiles per projection (x-z)
  *   [9] dynamic shared memory bytes   [10] kernels launched by the last beamform call
- *   [11] tiles per projection (y-z) */
+ *   [11] tiles per projection (y-z)   [12] precision in use (1 compact / 2 full)
+ *   [13] scratch bytes per (sample, frame) */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this

@@ -44,7 +44,7 @@ class Options(C.Structure):
                 ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
                 ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
                 ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
-                ("reserved", C.c_int32 * 5)]
+                ("precision", C.c_int32), ("reserved", C.c_int32 * 4)]
 
 
 def library_path() -> str:
@@ -100,7 +100,7 @@ def _farr(v):
 
 
 INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
-             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz"]
+             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample"]
 
 
 class Plan:
@@ -114,7 +114,7 @@ class Plan:
                  n_samples: int, input_kind: int = 0, channels_per_event: Optional[int] = None,
                  t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
                  elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
-                 max_frames: int = 0, build_volume: bool = False, kernel: int = 0):
+                 max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0):
         lib = load()
         self._h = C.c_void_p()
         geo = Geometry(n_rows, n_cols, pitch)
@@ -128,7 +128,7 @@ class Plan:
             raise ValueError("elem_window must have n_cols + n_rows entries")
         opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
                       float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
-                      1 if build_volume else 0, int(kernel))
+                      1 if build_volume else 0, int(kernel), int(precision))
         gx, gy = Grid(*grid_xz), Grid(*grid_yz)
         _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
                                        float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),

@@ -62,7 +62,7 @@ struct Grid {
 // transmit-side tables of one aperture for a list of reference coordinates ("planes")
 struct TxTables {
     int n_planes = 0;
-    DeviceBuf n0, f0m, ph0;
+    DeviceBuf n0, f0m, ph0, tph;
 };
 
 struct Aperture {
@@ -92,6 +92,7 @@ struct ulm_rca_plan {
     size_t iq_bytes = 0;
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
+    bool d32 = false;             // full (fp32) difference term in the scratch
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
     mutable long long last_launches = 0;
@@ -144,6 +145,7 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
     const size_t n = refs.size() * (size_t)A.n_tx * A.g.n_ax;
     std::vector<int> n0(n);
     std::vector<float> f0m(n), ph0(n);
+    std::vector<float2> tph(n);
     size_t i = 0;
     for (double ref : refs)
         for (int k = 0; k < A.n_tx; ++k)
@@ -155,21 +157,24 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
                 // phase of the full delay in cycles: (fc/fs) u + fc t_start, u = n0_abs + 0.5 + (f0m + H)
                 const double cyc = (P.fc / P.fs) * (fl + 0.5) + P.fc * P.t_start;
                 ph0[i] = (float)(cyc - std::floor(cyc));
+                // transmit phasor of the ring kernel: exp(j 2 pi (fc/fs U0 + fc t_start))
+                double cu = (P.fc / P.fs) * u0 + P.fc * P.t_start;
+                cu -= std::floor(cu);
+                tph[i] = make_float2((float)std::cos(2 * M_PI * cu), (float)std::sin(2 * M_PI * cu));
             }
     T.n_planes = (int)refs.size();
     cudaError_t e;
     if ((e = T.n0.upload(n0)) != cudaSuccess) return e;
     if ((e = T.f0m.upload(f0m)) != cudaSuccess) return e;
+    if ((e = T.tph.upload(tph)) != cudaSuccess) return e;
     return T.ph0.upload(ph0);
 }
 
 ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
     ulm::DemodConst &D = P.demod;
     if (P.input_kind == 1) {
-        P.half_len = 0;
-        D.n_taps = 1;
-        D.off[0] = 0;
-        D.g[0] = 1.f;
+        P.half_len = D.half_len = 0;
+        D.gd[0] = 1.f;
         return ULM_RCA_OK;
     }
     const int L = demod_taps > 0 ? (demod_taps - 1) / 2 : 2 * (int)std::lround(P.fs / P.fc);
@@ -183,15 +188,11 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
         h[m + L] = sinc * win;
         sum += h[m + L];
     }
-    D.n_taps = 0;
-    for (int m = -L; m <= L; ++m) {
-        const double g = 2.0 * h[m + L] / sum;
-        if (std::fabs(g) < 1e-13) continue;        // exact zeros of the sinc (every 2nd tap at fs = 4 fc)
-        D.off[D.n_taps] = m;
-        D.g[D.n_taps] = (float)g;
-        ++D.n_taps;
+    for (int t = 0; t <= 2 * L; ++t) {
+        const double g = 2.0 * h[t] / sum;
+        D.gd[t] = std::fabs(g) < 1e-13 ? 0.f : (float)g;     // exact zeros of the sinc (every 2nd tap at fs = 4 fc)
     }
-    P.half_len = L;
+    P.half_len = D.half_len = L;
     return ULM_RCA_OK;
 }
 
@@ -227,7 +228,7 @@ ulm_rca_status upload_aperture(ulm_rca_plan &P, Aperture &A, const float *window
 
 ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTables &T) {
     ulm::DasParams D{};
-    D.iq = P.iq.as<float4>();
+    D.iq = P.iq.as<unsigned char>();
     D.l_row = P.l_row; D.n_rx_max = P.n_rx_max; D.n_events = P.n_events;
     D.e0 = A.e0; D.n_tx = A.n_tx; D.n_rx = A.n_rx; D.n_lat = A.g.n_lat; D.n_ax = A.g.n_ax;
     D.xs = A.xs.as<float>(); D.zs = A.zs.as<float>(); D.ejs = A.ejs.as<float>();
@@ -240,37 +241,63 @@ ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTabl
     return D;
 }
 
+// frames per scratch group for a batch of n_frames
+int group_frames(int n_frames) { return n_frames <= 4 ? 4 : 12; }
+
 template <int F>
 void launch_generic_f(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames, cudaStream_t st) {
     const int npix = D.n_lat * D.n_ax;
     dim3 grid((npix + 127) / 128, (n_frames + F - 1) / F, D.n_planes * (D.per_angle ? D.n_tx : 1));
-    if (P.apod) ulm::das_generic_kernel<F, true><<<grid, 128, 0, st>>>(D);
-    else ulm::das_generic_kernel<F, false><<<grid, 128, 0, st>>>(D);
+    if (P.d32) {
+        if (P.apod) ulm::das_generic_kernel<F, true, true><<<grid, 128, 0, st>>>(D);
+        else ulm::das_generic_kernel<F, true, false><<<grid, 128, 0, st>>>(D);
+    } else {
+        if (P.apod) ulm::das_generic_kernel<F, false, true><<<grid, 128, 0, st>>>(D);
+        else ulm::das_generic_kernel<F, false, false><<<grid, 128, 0, st>>>(D);
+    }
     ++P.last_launches;
 }
 
 void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames, cudaStream_t st) {
     if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
-    if (n_frames >= 8) launch_generic_f<8>(P, D, n_frames, st);
-    else if (n_frames >= 4) launch_generic_f<4>(P, D, n_frames, st);
-    else if (n_frames >= 2) launch_generic_f<2>(P, D, n_frames, st);
-    else launch_generic_f<1>(P, D, n_frames, st);
+    if (group_frames(n_frames) == 12) launch_generic_f<12>(P, D, n_frames, st);
+    else launch_generic_f<4>(P, D, n_frames, st);
 }
 
-void launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, cudaStream_t st) {
+template <int NT, bool IQ, int F, bool D32>
+cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, unsigned blocks, cudaStream_t st) {
+    const size_t smem = (size_t)F * ((ulm::kDemodChunk + 1 + 2 * L + 1) + (ulm::kDemodChunk + 2)) * sizeof(float2);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    ulm::demod_kernel<NT, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
+    return cudaSuccess;
+}
+
+template <int F, bool D32>
+cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, unsigned blocks, cudaStream_t st) {
+    const int L = P.half_len;
+    if (P.input_kind == 1) return launch_demod_t<1, true, F, D32>(D, 0, blocks, st);
+    if (L == 8) return launch_demod_t<17, false, F, D32>(D, L, blocks, st);
+    if (L == 16) return launch_demod_t<33, false, F, D32>(D, L, blocks, st);
+    return launch_demod_t<0, false, F, D32>(D, L, blocks, st);
+}
+
+cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, cudaStream_t st) {
     ulm::DemodParams D{};
-    D.rf = d_channel; D.iq = P.iq.as<float4>(); D.mixer = P.mixer.as<float2>(); D.mix_n0 = P.mix_n0;
-    D.n_events = P.n_events; D.channels_per_event = P.cpe; D.n_samples = P.n_samples;
+    D.rf = d_channel; D.iq = P.iq.as<unsigned char>(); D.mixer = P.mixer.as<float2>(); D.mix_n0 = P.mix_n0;
+    D.n_frames = n_frames; D.n_events = P.n_events; D.channels_per_event = P.cpe; D.n_samples = P.n_samples;
     D.n_row_tx = P.ap[0].n_tx; D.n_rows = P.n_rows; D.n_cols = P.n_cols; D.n_rx_max = P.n_rx_max;
     D.full_channels = P.cpe == P.n_rows + P.n_cols;
-    D.n_lo = P.n_lo; D.l_row = P.l_row; D.half_len = P.half_len;
-    D.chunks_per_row = (P.l_row + 254) / 255;
-    const long long rows = (long long)n_frames * P.n_events * P.n_rx_max;
-    const size_t smem = (256 + 2 * P.half_len) * sizeof(float2);
+    D.n_lo = P.n_lo; D.l_row = P.l_row;
+    D.chunks_per_row = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
+    const int F = group_frames(n_frames);
+    const long long rows = (long long)((n_frames + F - 1) / F) * P.n_events * P.n_rx_max;
     const unsigned blocks = (unsigned)(rows * D.chunks_per_row);
-    if (P.input_kind == 1) ulm::demod_kernel<true><<<blocks, 256, smem, st>>>(D);
-    else ulm::demod_kernel<false><<<blocks, 256, smem, st>>>(D);
     ++P.last_launches;
+    if (P.d32) return F == 12 ? launch_demod_f<12, true>(P, D, blocks, st) : launch_demod_f<4, true>(P, D, blocks, st);
+    return F == 12 ? launch_demod_f<12, false>(P, D, blocks, st) : launch_demod_f<4, false>(P, D, blocks, st);
 }
 
 }  // namespace
@@ -296,7 +323,8 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
     if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
-    for (int i = 0; i < 5; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    for (int i = 0; i < 4; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->precision < 0 || opt->precision > 2) return fail(ULM_RCA_EINVAL, "precision must be 0, 1 or 2");
     if (opt->input_kind != 0 && opt->input_kind != 1) return fail(ULM_RCA_EINVAL, "input_kind must be 0 or 1");
     if (opt->n_samples < 2) return fail(ULM_RCA_EINVAL, "n_samples must be >= 2");
     if (!std::isfinite(opt->t_start_s) || !std::isfinite(opt->f_number) || opt->f_number < 0)
@@ -334,6 +362,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     P.n_events = n_row_tx + n_col_tx;
     P.n_rx_max = std::max(P.n_rows, P.n_cols);
     P.apod = opt->f_number > 0 || opt->elem_window != nullptr;
+    P.d32 = opt->precision == 2 || (opt->precision == 0 && opt->input_kind == 1);
 
     for (int a = 0; a < 2; ++a) {
         Aperture &A = P.ap[a];
@@ -394,14 +423,13 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         if (P.build_volume) CUDA_TRY(build_tx_tables(P, A, vol_refs[a], A.vol));
     }
 
-    P.iq_bytes = (size_t)P.max_frames * P.n_events * P.n_rx_max * P.l_row * sizeof(float4);
+    P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * P.n_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
     CUDA_TRY(cudaMalloc(&P.iq.p, P.iq_bytes));
 
     // kernel choice: the shared-memory ring kernel covers compounded projections; everything else
     // (per-angle slices, the volume, shapes whose window does not fit) takes the generic kernel.
     P.kernel = 1;
     if (P.compound && opt->kernel != 1) {
-        std::vector<const ulm::RingApertureDesc *> none;
         ulm::RingApertureDesc desc[2];
         for (int a = 0; a < 2; ++a) {
             const Aperture &A = P.ap[a];
@@ -409,8 +437,8 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
                                             A.g.ref, A.angles.data(), A.t0.data()};
         }
         const char *why = nullptr;
-        const bool ok = ulm::ring_plan(desc, P.pitch, P.c, P.fs, P.t_start, P.n_lo, P.l_row, P.apod, P.ring,
-                                       P.ap[0].ring, P.ap[1].ring, &why);
+        const bool ok = ulm::ring_plan(desc, P.pitch, P.c, P.fs, P.t_start, P.l_row, P.ring, P.ap[0].ring,
+                                       P.ap[1].ring, &why);
         if (ok) P.kernel = 2;
         else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
         if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
@@ -434,12 +462,13 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *ch, size_t *
 
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n) {
     if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
-    const int64_t vals[12] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel,
-                              plan->kernel == 2 ? plan->ring.frames : 8, plan->kernel == 2 ? plan->ring.tile_pixels : 128,
-                              plan->kernel == 2 ? plan->ring.window : 0, plan->kernel == 2 ? plan->ring.stages : 0,
-                              plan->kernel == 2 ? plan->ap[0].ring.n_tiles : 0, plan->kernel == 2 ? plan->ring.smem_bytes : 0,
-                              plan->last_launches, plan->kernel == 2 ? plan->ap[1].ring.n_tiles : 0};
-    for (int i = 0; i < n && i < 12; ++i) v[i] = vals[i];
+    const bool ring = plan->kernel == 2, d32 = plan->d32;
+    const int64_t vals[14] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
+                              ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
+                              ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
+                              ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
+                              ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : 1, ulm::entry_bytes(12, d32) / 12};
+    for (int i = 0; i < n && i < 14; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
 }
 
@@ -463,7 +492,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
         const int tb = P.timed_batches[slot] < ulm_rca_plan::kTimedBatches ? P.timed_batches[slot] : -1;
         if (tb >= 0) cudaEventRecord(P.ev[slot][tb][0], st);
-        launch_demod(P, in, nb, st);
+        CUDA_TRY(launch_demod(P, in, nb, st));
         if (tb >= 0) cudaEventRecord(P.ev[slot][tb][1], st);
         for (int a = 0; a < 2; ++a) {     // an aperture without transmit events: its image is all zeros
             const Aperture &A = P.ap[a];
@@ -473,19 +502,19 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         }
         if (P.kernel == 2) {
             ulm::RingLaunch L{};
-            L.iq = P.iq.as<float4>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.n_events;
+            L.iq = P.iq.as<unsigned char>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.n_events;
             L.out = outp; L.out_frame_stride = P.out_per_frame; L.n_frames = nb;
-            L.fcfs = P.fc / P.fs; L.fct = P.fc * P.t_start; L.n_lo = P.n_lo; L.two_f = (float)(2.0 * P.f_number);
+            L.fcfs = (float)(P.fc / P.fs); L.two_f = (float)(2.0 * P.f_number);
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];
                 ulm::RingApertureArgs &R = L.ap[a];
                 R.e0 = A.e0; R.n_tx = A.n_tx; R.n_rx = A.n_rx; R.n_lat = A.g.n_lat; R.n_ax = A.g.n_ax;
                 R.xs = A.xs.as<float>(); R.zs = A.zs.as<float>(); R.ejs = A.ejs.as<float>();
                 R.xm = A.xm.as<float>(); R.zm = A.zm.as<float>(); R.ejm = A.ejm.as<float>(); R.win = A.win.as<float>();
-                R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
+                R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>(); R.tph = A.proj.tph.as<float2>();
                 R.out_base = A.out_base;
             }
-            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, P.apod, st);
+            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, group_frames(nb), P.d32, P.apod, st);
         } else {
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];
@@ -539,7 +568,7 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
         const int nb = std::min(P.max_frames, n_frames - f0);
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out_volume) + (long long)f0 * P.vol_per_frame;
-        launch_demod(P, in, nb, st);
+        CUDA_TRY(launch_demod(P, in, nb, st));
         // V_RC: lateral = x, planes = y; then V_CR accumulated on top: lateral = y, planes = x
         for (int a = 0; a < 2; ++a) {
             const Aperture &A = P.ap[a];

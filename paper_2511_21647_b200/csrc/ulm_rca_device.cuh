@@ -1,4 +1,5 @@
-// ulm_rca_device.cuh -- device-side data layout and kernels of the RCA projection beamformer (sm_100a).
+// ulm_rca_device.cuh -- device-side data layout, the demodulation/staging pre-pass and the generic
+// gather kernel of the RCA projection beamformer (sm_100a).
 //
 // Numerics shared by every DAS kernel:
 //   u = (tau - t_start) fs is split as  u = U0[k][iz] + H(p, j)  with
@@ -6,12 +7,18 @@
 //          integer n0 (relative to the scratch origin) + fraction f0m = frac - 0.5 (fp32)
 //     H  = (sqrt(dx^2 + z^2) - z) fs/c = dx_s^2 / (sqrt(dx_s^2 + z_s^2) + z_s)   -- device, fp32, <= ~400
 //   so no fp32 quantity ever carries the full ~1300-sample delay.  floor(u) is taken with the
-//   add-magic-constant trick on (u - 0.5); the IQ scratch stores {mid = (iq[n]+iq[n+1])/2, d = iq[n+1]-iq[n]}
-//   so that the interpolated sample is mid + a' d with a' in [-0.5, 0.5].
-//   The phase 2 pi fc tau = 2 pi ((fc/fs) u + fc t_start) is ph0[k][iz] + (fc/fs)(f0m + H) cycles with
-//   ph0 = frac((fc/fs)(n0_abs + 0.5) + fc t_start) from the host in fp64.
+//   add-magic-constant trick on (u - 0.5).
+//
+// IQ scratch ("entries"): frames are processed in groups of F (4 or 12).  For frame group g, event e,
+// receive element j and sample n the scratch holds ONE entry of 12 F bytes
+//     [ mid_f = (iq_f[n] + iq_f[n+1]) / 2   as float2, f = 0..F-1 |  d_f = (iq_f[n+1] - iq_f[n]) / 16  as half2, f = 0..F-1 ]
+// so that the interpolated sample is mid + a' d with a' = a - 0.5 in [-0.5, 0.5]: the value carries fp32
+// precision, only the small difference term is fp16 (with a' also rounded to fp16: one FHFMA
+// `fma.rn.f32.f16` per component, no conversion instruction).  Entry sizes 48 B / 144 B are odd multiples
+// of 16 B, which makes the LDS.128 gathers of neighbouring entries bank-conflict free.
 #pragma once
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -21,30 +28,192 @@ constexpr float kMagic = 12582912.0f;        // 1.5 * 2^23: (x + kMagic) - kMagi
 constexpr int kMagicBits = 0x4B400000;
 constexpr int kMaxTaps = 129;
 constexpr float kTwoPi = 6.283185307179586f;
+constexpr float kDScale = 0.0625f;           // d is stored / 16 (|d| can exceed the fp16 range) ...
+constexpr float kAlScale = 16.0f;            // ... and a' is multiplied by 16 before rounding to fp16
+constexpr int kDemodChunk = 127;             // entries per demodulation CTA (128 iq values)
+
+// D32 = false: compact entries (fp16 difference term, 12 F bytes); true: full entries (fp32 difference
+// term, 16 F bytes + 16 bytes of padding that keep the entry an odd multiple of 16 B)
+__host__ __device__ constexpr int entry_bytes(int F, bool D32) { return D32 ? 16 * F + 16 : 12 * F; }
 
 // Demodulation constants (per plan), in constant memory.
 struct DemodConst {
-    int n_taps;              // number of non-zero taps
-    int off[kMaxTaps];       // tap offset m (iq[n] += g * x[n - m])
-    float g[kMaxTaps];       // 2 h[m]  (1 for IQ input)
+    int half_len;            // L
+    float gd[kMaxTaps];      // dense taps: gd[t] = 2 h[t - L], t = 0..2L   ({1} for IQ input)
 };
 
 struct DemodParams {
     const int16_t *rf;       // [frame][event][channel][sample] (x2 for IQ input)
-    float4 *iq;              // [frame][event][rx elem (n_rx_max)][l_row] entries {mid.re, mid.im, d.re, d.im}
+    unsigned char *iq;       // entries: [group][event][rx elem (n_rx_max)][l_row][12 F bytes]
     const float2 *mixer;     // exp(-j 2 pi fc t_n) for n = mix_n0 .. (RF input only)
     int mix_n0;
-    int n_events, channels_per_event, n_samples;
+    int n_frames, n_events, channels_per_event, n_samples;
     int n_row_tx, n_rows, n_cols, n_rx_max;
     int full_channels;       // 1: channels_per_event = n_rows + n_cols
     int n_lo, l_row;         // scratch origin (absolute sample of entry 0) and entries per row
-    int half_len;            // L
     int chunks_per_row;
 };
 
-// One aperture (image) of the DAS kernels.
+__device__ __forceinline__ void sincos_cycles(float cyc, float &s, float &c) {
+    // cyc in cycles, |cyc| < 2^22.  Reduce to [-0.5, 0.5] exactly, then the MUFU approximations
+    // (abs error ~4e-7 on the reduced argument).
+    float r = cyc - ((cyc + kMagic) - kMagic);
+    __sincosf(kTwoPi * r, &s, &c);
+}
+
+// d(f32) = a(f16) * b(f16) + c(f32), one FHFMA on sm_100a
+__device__ __forceinline__ float fhfma(unsigned short a, unsigned short b, float c) {
+    float r;
+    asm("fma.rn.f32.f16 %0, %1, %2, %3;" : "=f"(r) : "h"(a), "h"(b), "f"(c));
+    return r;
+}
+__device__ __forceinline__ void split_h2(uint32_t v, unsigned short &lo, unsigned short &hi) {
+    asm("mov.b32 {%0, %1}, %2;" : "=h"(lo), "=h"(hi) : "r"(v));
+}
+__device__ __forceinline__ unsigned short f2h_bits(float v) {
+    unsigned short r;
+    asm("cvt.rn.f16.f32 %0, %1;" : "=h"(r) : "f"(v));
+    return r;
+}
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Demodulation / staging pre-pass: int16 RF (or IQ) -> scratch entries over the touched
+// sample range only.  One CTA = one chunk of 127 entries of one (frame group, event, rx element) row, all F
+// frames of the group: (1) the mixed samples x = rf * exp(-j 2 pi fc t) go to shared memory, (2) each
+// thread runs the FIR for 8 consecutive outputs of one frame with the inputs sliding through registers
+// (dense taps straight from constant memory), (3) the entries are assembled and stored as fully
+// coalesced 16-byte chunks.  NT = dense tap count 2L+1 (0: run-time L).
+// ---------------------------------------------------------------------------------------------------
+__constant__ DemodConst c_demod[1];
+
+template <int NT, bool IQ_INPUT, int F, bool D32>
+__global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
+    extern __shared__ float2 s_dyn[];
+    constexpr int NIQ = kDemodChunk + 1;       // iq values per chunk
+    constexpr int IQS = NIQ + 1;               // row stride of s_iq (float2)
+    const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
+    const int XW = NIQ + 2 * L;                // mixed samples per frame
+    const int XS = XW + 1;                     // row stride of s_x (float2), odd
+    float2 *s_x = s_dyn;                       // [F][XS]
+    float2 *s_iq = s_dyn + F * XS;             // [F][IQS]
+
+    const int chunk = blockIdx.x % P.chunks_per_row;
+    const long long row = blockIdx.x / P.chunks_per_row;    // (group * n_events + e) * n_rx_max + j
+    const int j = (int)(row % P.n_rx_max);
+    const long long ge = row / P.n_rx_max;
+    const int e = (int)(ge % P.n_events);
+    const int g = (int)(ge / P.n_events);
+    const int row_tx = e < P.n_row_tx;
+    const int n_rx = row_tx ? P.n_cols : P.n_rows;
+    if (j >= n_rx) return;                      // rows of the shorter aperture stay unused
+    const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
+    const int base = P.n_lo + chunk * kDemodChunk;   // absolute sample of this chunk's first iq value
+
+    // (1) mixed samples
+    for (int idx = threadIdx.x; idx < F * XW; idx += 256) {
+        const int f = idx / XW, i = idx - f * XW;
+        const int n = base - L + i;
+        const int fr = g * F + f;
+        float2 v = make_float2(0.f, 0.f);
+        if (fr < P.n_frames && n >= 0 && n < P.n_samples) {
+            const long long rec = (((long long)fr * P.n_events + e) * P.channels_per_event + ch) * (long long)P.n_samples;
+            if (IQ_INPUT) {
+                const short2 q = reinterpret_cast<const short2 *>(P.rf)[rec + n];
+                v = make_float2((float)q.x, (float)q.y);
+            } else {
+                const float r = (float)P.rf[rec + n];
+                const float2 m = __ldg(P.mixer + (n - P.mix_n0));
+                v = make_float2(r * m.x, r * m.y);
+            }
+        }
+        s_x[f * XS + i] = v;
+    }
+    __syncthreads();
+
+    // (2) FIR: iq[base + r] = sum_{i = r .. r + 2L} gd[r + 2L - i] x[i]   (x index relative to base - L)
+    constexpr int R = 8;
+    if (threadIdx.x < F * (NIQ / R)) {
+        const int f = threadIdx.x / (NIQ / R), r0 = (threadIdx.x - f * (NIQ / R)) * R;
+        const float2 *x = s_x + f * XS + r0;
+        float ar[R], ai[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) ar[q] = ai[q] = 0.f;
+        if (NT > 0) {
+#pragma unroll
+            for (int u = 0; u < R + NT - 1; ++u) {
+                const float2 xv = x[u];
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int t = q - u + (NT - 1);
+                    if (t >= 0 && t < NT) {
+                        ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
+                        ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
+                    }
+                }
+            }
+        } else {
+            for (int u = 0; u < R + 2 * L; ++u) {
+                const float2 xv = x[u];
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int t = q - u + 2 * L;
+                    if (t >= 0 && t <= 2 * L) {
+                        ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
+                        ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) s_iq[f * IQS + r0 + q] = make_float2(ar[q], ai[q]);
+    }
+    __syncthreads();
+
+    // (3) entries: chunk c < F/2 of an entry = mid of frames 2c, 2c+1; then the difference terms: d/16 as
+    // half2 of 4 frames per chunk (compact) or d as float2 of 2 frames per chunk + one padding chunk (full)
+    constexpr int EB = entry_bytes(F, D32);
+    constexpr int CPE = EB / 16;                // 16-byte chunks per entry
+    const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
+    uint4 *dst = reinterpret_cast<uint4 *>(P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB);
+    for (int idx = threadIdx.x; idx < n_ent * CPE; idx += 256) {
+        const int ent = idx / CPE, c = idx - ent * CPE;
+        const int n = base + ent;
+        uint4 o = make_uint4(0u, 0u, 0u, 0u);
+        if (n >= 0 && n + 1 <= P.n_samples - 1 && c < (D32 ? F : CPE)) {      // edge rule: both taps inside the record
+            if (c < F / 2 || D32) {
+                const int cc = c < F / 2 ? c : c - F / 2;
+                const float2 a0 = s_iq[(2 * cc) * IQS + ent], b0 = s_iq[(2 * cc) * IQS + ent + 1];
+                const float2 a1 = s_iq[(2 * cc + 1) * IQS + ent], b1 = s_iq[(2 * cc + 1) * IQS + ent + 1];
+                if (c < F / 2) {
+                    o.x = __float_as_uint(0.5f * (a0.x + b0.x)); o.y = __float_as_uint(0.5f * (a0.y + b0.y));
+                    o.z = __float_as_uint(0.5f * (a1.x + b1.x)); o.w = __float_as_uint(0.5f * (a1.y + b1.y));
+                } else {
+                    o.x = __float_as_uint(b0.x - a0.x); o.y = __float_as_uint(b0.y - a0.y);
+                    o.z = __float_as_uint(b1.x - a1.x); o.w = __float_as_uint(b1.y - a1.y);
+                }
+            } else {
+                const int f0 = 4 * (c - F / 2);
+                uint32_t w[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float2 a = s_iq[(f0 + q) * IQS + ent], b = s_iq[(f0 + q) * IQS + ent + 1];
+                    w[q] = pack_h2(kDScale * (b.x - a.x), kDScale * (b.y - a.y));
+                }
+                o = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+        }
+        dst[idx] = o;
+    }
+}
+
+// One aperture (image) of the generic DAS kernel.
 struct DasParams {
-    const float4 *iq;
+    const unsigned char *iq;
     int l_row, n_rx_max, n_events;
     int e0, n_tx, n_rx, n_lat, n_ax;
     const float *xs, *zs, *ejs;      // lateral pixel / depth / element coordinates in samples (coord * fs / c)
@@ -63,88 +232,72 @@ struct DasParams {
     int n_frames;                    // frames in this batch
 };
 
-__device__ __forceinline__ void sincos_cycles(float cyc, float &s, float &c) {
-    // cyc in cycles, |cyc| < 2^22.  Reduce to [-0.5, 0.5] exactly, then the MUFU approximations
-    // (abs error ~4e-7 on the reduced argument).
-    float r = cyc - ((cyc + kMagic) - kMagic);
-    __sincosf(kTwoPi * r, &s, &c);
+// the interpolation weight a' = a - 0.5 of one gather: fp32, and 16 a' split into two fp16 (hi + lo = exact to 2^-24)
+struct Alpha {
+    float al;
+    unsigned short hi, lo;
+};
+__device__ __forceinline__ Alpha make_alpha(float al) {
+    Alpha a;
+    a.al = al;
+    const float a16 = kAlScale * al;
+    a.hi = f2h_bits(a16);
+    float back;
+    asm("cvt.f32.f16 %0, %1;" : "=f"(back) : "h"(a.hi));
+    a.lo = f2h_bits(a16 - back);
+    return a;
 }
 
-// ---------------------------------------------------------------------------------------------------
-// Demodulation / staging pre-pass: int16 RF (or IQ) -> {mid, d} fp32 entries over the
-// touched sample range only.  One CTA = one 255-entry chunk of one (frame, event, rx element) row.
-// ---------------------------------------------------------------------------------------------------
-__constant__ DemodConst c_demod[1];
-
-template <bool IQ_INPUT>
-__global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
-    extern __shared__ float2 s_x[];            // mixed samples x[n] for n = base - L .. base + 255 + L
-    __shared__ float2 s_iq[256];
-    const int chunk = blockIdx.x % P.chunks_per_row;
-    long long row = blockIdx.x / P.chunks_per_row;    // (frame * n_events + e) * n_rx_max + j
-    const int j = (int)(row % P.n_rx_max);
-    const long long fe = row / P.n_rx_max;
-    const int e = (int)(fe % P.n_events);
-    const int row_tx = e < P.n_row_tx;
-    const int n_rx = row_tx ? P.n_cols : P.n_rows;
-    if (j >= n_rx) return;                      // rows of the shorter aperture stay unused
-    const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
-    const long long rec = (fe * P.channels_per_event + ch) * (long long)P.n_samples;
-    const int L = P.half_len;
-    const int base = P.n_lo + chunk * 255;      // absolute sample of this chunk's first iq value
-    const int n_x = 256 + 2 * L;
-    for (int i = threadIdx.x; i < n_x; i += 256) {
-        const int n = base - L + i;
-        float2 v = make_float2(0.f, 0.f);
-        if (n >= 0 && n < P.n_samples) {
-            if (IQ_INPUT) {
-                const short2 q = reinterpret_cast<const short2 *>(P.rf)[rec + n];
-                v = make_float2((float)q.x, (float)q.y);
-            } else {
-                const float r = (float)P.rf[rec + n];
-                const float2 m = P.mixer[n - P.mix_n0];
-                v = make_float2(r * m.x, r * m.y);
+// interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
+// v = mid + a' d  (compact: two FHFMA per component, d in fp16; full: one FFMA),  acc += (c + j s) v
+template <int F, bool D32, class LoadVec>
+__device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, float s, float *accr, float *acci) {
+    if (D32) {
+#pragma unroll
+        for (int q = 0; q < F / 2; ++q) {
+            const uint4 m = ld(q), d = ld(F / 2 + q);
+            const float mv[4] = {__uint_as_float(m.x), __uint_as_float(m.y), __uint_as_float(m.z), __uint_as_float(m.w)};
+            const float dv[4] = {__uint_as_float(d.x), __uint_as_float(d.y), __uint_as_float(d.z), __uint_as_float(d.w)};
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const float vr = fmaf(A.al, dv[2 * i], mv[2 * i]), vi = fmaf(A.al, dv[2 * i + 1], mv[2 * i + 1]);
+                const int f = 2 * q + i;
+                accr[f] = fmaf(c, vr, accr[f]); accr[f] = fmaf(-s, vi, accr[f]);
+                acci[f] = fmaf(s, vr, acci[f]); acci[f] = fmaf(c, vi, acci[f]);
             }
         }
-        s_x[i] = v;
-    }
-    __syncthreads();
-    {
-        // iq[base + t] = sum_m g[m] x[base + t - m]
-        float ar = 0.f, ai = 0.f;
-        const int nt = c_demod[0].n_taps;
-        for (int q = 0; q < nt; ++q) {
-            const float2 x = s_x[threadIdx.x + L - c_demod[0].off[q]];
-            ar = fmaf(c_demod[0].g[q], x.x, ar);
-            ai = fmaf(c_demod[0].g[q], x.y, ai);
+    } else {
+#pragma unroll
+        for (int q = 0; q < F / 4; ++q) {
+            const uint4 m0 = ld(2 * q), m1 = ld(2 * q + 1), dd = ld(F / 2 + q);
+            const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+            const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                unsigned short dr, di;
+                split_h2(ds[i], dr, di);
+                const float vr = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[2 * i])));
+                const float vi = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[2 * i + 1])));
+                const int f = 4 * q + i;
+                accr[f] = fmaf(c, vr, accr[f]); accr[f] = fmaf(-s, vi, accr[f]);
+                acci[f] = fmaf(s, vr, acci[f]); acci[f] = fmaf(c, vi, acci[f]);
+            }
         }
-        s_iq[threadIdx.x] = make_float2(ar, ai);
-    }
-    __syncthreads();
-    const int i_row = chunk * 255 + threadIdx.x;
-    if (threadIdx.x < 255 && i_row < P.l_row) {
-        const int n = base + threadIdx.x;
-        float4 ent = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (n >= 0 && n + 1 <= P.n_samples - 1) {       // edge rule: both taps inside the record
-            const float2 a = s_iq[threadIdx.x], b = s_iq[threadIdx.x + 1];
-            ent = make_float4(0.5f * (a.x + b.x), 0.5f * (a.y + b.y), b.x - a.x, b.y - a.y);
-        }
-        P.iq[row * P.l_row + i_row] = ent;
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Generic gather kernel: one thread = one pixel x F frames, gathers straight from the IQ scratch through
-// L1/L2.  Serves per-angle slices (compound = 0), the 3-D comparator (config 4) and any shape the
-// shared-memory ring kernel does not cover.  grid = (pixel blocks, frame groups, plane * angle groups).
+// Generic gather kernel: one thread = one pixel x the F frames of one group, gathers straight from the
+// IQ scratch through L1/L2.  Serves per-angle slices (compound = 0), the 3-D comparator (config 4) and any
+// shape the shared-memory ring kernel does not cover.  grid = (pixel blocks, frame groups, plane * angle groups).
 // ---------------------------------------------------------------------------------------------------
-template <int F, bool APOD>
+template <int F, bool D32, bool APOD>
 __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
     const int npix = P.n_lat * P.n_ax;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npix) return;
     const int iz = p % P.n_ax, il = p / P.n_ax;
-    const int f_base = blockIdx.y * F;
+    const int g = blockIdx.y;
     const int n_kgroups = P.per_angle ? P.n_tx : 1;
     const int plane = blockIdx.z / n_kgroups;
     const int k_begin = P.per_angle ? (int)(blockIdx.z % n_kgroups) : 0;
@@ -155,13 +308,8 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
     float accr[F], acci[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) accr[f] = acci[f] = 0.f;
-    long long frow[F];                         // row index of (frame, event 0, element 0)
-#pragma unroll
-    for (int f = 0; f < F; ++f) {
-        const int fr = min(f_base + f, P.n_frames - 1);
-        frow[f] = (long long)fr * P.n_events * P.n_rx_max;
-    }
     const int tab0 = (plane * P.n_tx) * P.n_ax + iz;
+    const size_t grow = (size_t)g * P.n_events * P.n_rx_max;
 
     for (int j = 0; j < P.n_rx; ++j) {
         const float dxs = xs - P.ejs[j];
@@ -186,22 +334,18 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             float s, c;
             sincos_cycles(fmaf(P.fcfs, upm, P.ph0[t]), s, c);
             if (APOD) { s *= w; c *= w; }
-            const long long col = (long long)((P.e0 + k) * P.n_rx_max + j) * P.l_row + idx;
-#pragma unroll
-            for (int f = 0; f < F; ++f) {
-                const float4 e = __ldg(P.iq + frow[f] * P.l_row + col);
-                const float vr = fmaf(al, e.z, e.x), vi = fmaf(al, e.w, e.y);
-                accr[f] = fmaf(c, vr, accr[f]); accr[f] = fmaf(-s, vi, accr[f]);
-                acci[f] = fmaf(s, vr, acci[f]); acci[f] = fmaf(c, vi, acci[f]);
-            }
+            const uint4 *ent = reinterpret_cast<const uint4 *>(
+                P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32));
+            entry_mac<F, D32>([&](int i) { return __ldg(ent + i); }, make_alpha(al), c, s, accr, acci);
         }
     }
     const long long o = P.out_base + (long long)il * P.s_lat + (long long)plane * P.s_plane +
                         (long long)k_begin * P.s_k + iz;
 #pragma unroll
     for (int f = 0; f < F; ++f) {
-        if (f_base + f < P.n_frames) {
-            float2 *dst = P.out + (long long)(f_base + f) * P.out_frame_stride + o;
+        const int fr = g * F + f;
+        if (fr < P.n_frames) {
+            float2 *dst = P.out + (long long)fr * P.out_frame_stride + o;
             float2 v = make_float2(accr[f], acci[f]);
             if (P.accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
             *dst = v;

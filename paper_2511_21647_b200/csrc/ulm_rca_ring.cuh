@@ -1,18 +1,22 @@
 // ulm_rca_ring.cuh -- the hot kernel: shared-memory ring DAS for sm_100a.
 //
 // One persistent CTA per SM walks work items (frame group of F frames) x (aperture) x (pixel tile).  For a
-// work item the receive elements j are the outer loop and the transmit angles k the middle loop; for
-// every (j, k) a "stage" = the window of W IQ entries of channel j / event k that the tile can touch,
-// for all F frames, is brought from the IQ scratch into a shared-memory ring by one elected producer
-// thread with cp.async.bulk (TMA, SASS UBLKCP) completing on an mbarrier; 12 consumer warps gather from
-// it.  Everything that does not depend on the frame -- receive delay H(p, j), sample index, interpolation
+// work item the receive elements j are the outer loop and the transmit angles k the inner loop; for
+// every (j, k) a "stage" = the window of W scratch entries of channel j / event k that the tile can touch
+// (all F frames of the group are interleaved inside an entry, so a stage is ONE contiguous block) is
+// brought from the IQ scratch into a shared-memory ring by one elected producer thread with one
+// cp.async.bulk (TMA, SASS UBLKCP) completing on an mbarrier; 12 consumer warps gather from it.
+// Everything that does not depend on the frame -- receive delay H(p, j), sample index, interpolation
 // weight, phase rotation, apodisation -- is computed once per (pixel, j, k) and reused for the F frames,
 // whose accumulators stay in registers; the angle sum is taken in the same registers (the transmit phase
-// is folded into the per-(j, k) phasor), so one float2 per pixel and frame is written at the end and no
-// per-angle image or volume ever reaches HBM.
+// T_k(z) comes from a per-tile table, the receive phasor R(p, j) is computed once per (pixel, j)), so one
+// float2 per pixel and frame is written at the end and no per-angle image or volume ever reaches HBM.
 //
-// Lanes of a warp are consecutive lateral pixels at one depth: their sample indices form a slowly varying
-// monotone run, so the 16-byte LDS.128 gathers hit distinct or identical (broadcast) bank groups.
+// Pixel mapping: the image is cut into horizontal strips of PX rows; a consumer thread owns the PX
+// vertically adjacent pixels of one (strip, column) position and a tile is 384 consecutive positions, so the
+// lanes of a warp are lateral neighbours at the same depths: their sample indices form a slowly varying
+// monotone run and the LDS.128 gathers of a half-warp mostly fall into <= 8 distinct entries (one
+// shared-memory wavefront; entry size 12 F bytes = odd multiple of 16 B => no bank conflicts).
 #pragma once
 
 #include <cuda_runtime.h>
@@ -23,57 +27,37 @@
 namespace ulm {
 
 constexpr int kRingConsumerWarps = 12;
-constexpr int kRingConsumers = kRingConsumerWarps * 32;     // 384 consumer threads
-constexpr int kRingThreads = kRingConsumers + 32;           // + 1 producer warp
-constexpr int kRingPx = 4;                                  // pixels per consumer thread
-constexpr int kRingTilePixels = kRingConsumers * kRingPx;   // 1536
+constexpr int kRingConsumers = kRingConsumerWarps * 32;     // 384 consumer threads = positions per tile
+constexpr int kRingThreads = kRingConsumers + 128;          // + 1 producer warp group (1 working warp)
+constexpr int kRingConsumerRegs = 160;                      // setmaxnreg targets: 3 x 160 + 32 = 512 per SM sub-partition
+constexpr int kRingProducerRegs = 32;
 constexpr int kRingMaxStages = 8;
 constexpr int kRingMaxRx = 256;                             // receive elements per aperture
-constexpr int kRingMaxTz = 96;                              // tile rows
-constexpr int kRingMaxBt = 2048;                            // n_tx * tile rows
-
-struct RingConfig {
-    int frames = 0, tile_pixels = 0, window = 0, stages = 0, smem_bytes = 0;
-    int ws = 0;          // compile-time frame stride (entries) of a stage, >= window
-    int n_sms = 0;
-};
-
-struct RingTables {
-    int n_tiles = 0;
-    int tx = 0, tz = 0, tiles_x = 0, tiles_z = 0;
-    int *d_s0 = nullptr;     // [tile][j][k] window start, relative to the scratch origin
-    ~RingTables() { if (d_s0) cudaFree(d_s0); }
-};
-
-struct RingApertureDesc {
-    int n_tx, n_rx, n_lat, n_ax;
-    double lat0, dlat, z0, dz, ref;
-    const double *angles, *t0;
-};
+constexpr int kRingMaxTab = 1024;                           // n_tx * tile rows
 
 struct RingApertureArgs {
     int e0, n_tx, n_rx, n_lat, n_ax;
     const float *xs, *zs, *ejs, *xm, *zm, *ejm, *win;
-    const int *n0;
-    const float *f0m;
+    const int *n0;           // [k][iz] floor(U0) - n_lo
+    const float *f0m;        // [k][iz] U0 - floor(U0) - 0.5
+    const float2 *tph;       // [k][iz] exp(j 2 pi (fc/fs U0 + fc t_start))
     long long out_base;
     // filled by ring_launch from RingTables:
-    const int *s0;
-    int n_tiles, tx, tz, tiles_x;
+    const int *dj;           // [tile][j] floor(min H over the tile) - 2
+    int n_tiles;
 };
 
 struct RingLaunch {
-    const float4 *iq;
+    const unsigned char *iq;
     int l_row, n_rx_max, n_events;
     float2 *out;
     long long out_frame_stride;
     int n_frames;
-    double fcfs, fct;
-    int n_lo;
+    float fcfs;
     float two_f;
     RingApertureArgs ap[2];
     // filled by ring_launch:
-    int window, n_stages, n_groups, n_work;
+    int window, stage_stride, n_stages, n_groups, n_work;
 };
 
 // ---- PTX helpers (mbarrier + bulk async copy) --------------------------------------------------------
@@ -107,23 +91,28 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 __device__ __forceinline__ void consumer_bar() {
     asm volatile("bar.sync 1, %0;" ::"n"(kRingConsumers) : "memory");
 }
-__device__ __forceinline__ float4 lds128(uint32_t addr) {
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
 
-template <int F, int WS, bool APOD>
-__global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const RingLaunch P) {
+// the fields of ap[a] for a run-time a, selected field by field (indexing the kernel parameter with a
+// run-time index would copy the whole struct to local memory)
+#define ULM_AP(field) (a ? P.ap[1].field : P.ap[0].field)
+
+template <int F, int PX, bool D32, bool APOD>
+__global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_constant__ RingLaunch P) {
     extern __shared__ __align__(128) unsigned char smem[];
-    constexpr int kStageBytes = F * WS * 16;
+    constexpr int EB = entry_bytes(F, D32);
     const int NS = P.n_stages;
-    unsigned char *p_misc = smem + (size_t)NS * kStageBytes;
-    float *s_bt = reinterpret_cast<float *>(p_misc);                       // [k][tz]
-    float *s_ejs = s_bt + kRingMaxBt;                                      // [n_rx]
+    unsigned char *p_misc = smem + (size_t)NS * P.stage_stride;
+    float4 *s_tab = reinterpret_cast<float4 *>(p_misc);                    // [k][row] {bt, T.re, T.im, -}
+    float *s_ejs = reinterpret_cast<float *>(s_tab + kRingMaxTab);         // [n_rx]
     float *s_win = s_ejs + kRingMaxRx;
     float *s_ejm = s_win + kRingMaxRx;
-    float4 *s_hdr = reinterpret_cast<float4 *>(s_ejm + kRingMaxRx);        // [NS] {off, phi, -, -}
+    float *s_dj = s_ejm + kRingMaxRx;                                      // [n_rx] (float)(dj)
+    int *s_hdr = reinterpret_cast<int *>(s_dj + kRingMaxRx);               // [NS] entry shift of the stage
     uint64_t *s_full = reinterpret_cast<uint64_t *>(s_hdr + kRingMaxStages);
     uint64_t *s_empty = s_full + kRingMaxStages;
 
@@ -140,48 +129,41 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const RingLau
     const int tiles_all = P.ap[0].n_tiles + P.ap[1].n_tiles;
     uint32_t stage_ctr = 0;     // global stage counter (identical sequence in producer and consumers)
 
-    if (warp == kRingConsumerWarps) {
-        // =================================== PRODUCER WARP ===================================
+    if (warp >= kRingConsumerWarps) {
+        // ============ PRODUCER WARP GROUP: gives its registers to the consumers; one warp works ============
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRingProducerRegs));
+        if (warp != kRingConsumerWarps) return;
         for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
             const int g = w / tiles_all;
             int tt = w - g * tiles_all;
             const int a = tt >= P.ap[0].n_tiles ? 1 : 0;
             if (a) tt -= P.ap[0].n_tiles;
-            const RingApertureArgs &A = P.ap[a];
-            const int iz0 = (tt / A.tiles_x) * A.tz;
-            const int n_st = A.n_rx * A.n_tx;
-            const int *s0_tab = A.s0 + (size_t)tt * n_st;
-            const int f_first = g * F;
+            const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+            const int e0 = ULM_AP(e0);
+            const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx;
+            const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
+            const int n_st = n_rx * n_tx;
+            const unsigned char *grp = P.iq + (size_t)g * P.n_events * P.n_rx_max * P.l_row * EB;
             for (int sb = 0; sb < n_st; sb += 32) {
-                // each lane fetches the window start and the tile's reference n0 of one stage
+                // each lane fetches the (unclamped) window start of one stage
                 const int my = sb + lane;
-                int my_s0 = 0, my_nref = 0;
-                if (my < n_st) {
-                    my_s0 = __ldg(s0_tab + my);
-                    my_nref = __ldg(A.n0 + (my % A.n_tx) * A.n_ax + iz0);
-                }
+                int my_s0 = 0;
+                if (my < n_st) my_s0 = __ldg(n0 + (my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
                 const int cnt = min(32, n_st - sb);
                 for (int i = 0; i < cnt; ++i) {
-                    const int s0 = __shfl_sync(0xffffffffu, my_s0, i);
-                    const int nref = __shfl_sync(0xffffffffu, my_nref, i);
+                    const int s0_raw = __shfl_sync(0xffffffffu, my_s0, i);
                     if (lane == 0) {
                         const int st = sb + i;
-                        const int j = st / A.n_tx, k = st - j * A.n_tx;
+                        const int j = st / n_tx, k = st - j * n_tx;
                         const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
+                        const int s0 = max(0, min(s0_raw, P.l_row - P.window));
                         mbar_wait(smem_u32(&s_empty[slot]), phase ^ 1);
-                        double cyc = P.fcfs * ((double)(P.n_lo + s0) + 0.5) + P.fct;
-                        cyc -= floor(cyc);
-                        s_hdr[slot] = make_float4((float)(nref - s0), (float)cyc, 0.f, 0.f);
+                        s_hdr[slot] = s0_raw - s0;
                         const uint32_t bar = smem_u32(&s_full[slot]);
-                        const uint32_t bytes = (uint32_t)P.window * 16u;
-                        mbar_expect_tx(bar, bytes * F);
-                        const uint32_t dst = smem_u32(smem) + slot * kStageBytes;
-#pragma unroll
-                        for (int f = 0; f < F; ++f) {
-                            const int fr = min(f_first + f, P.n_frames - 1);
-                            const float4 *src = P.iq + ((long long)(fr * P.n_events + A.e0 + k) * P.n_rx_max + j) * P.l_row + s0;
-                            bulk_g2s(dst + f * (WS * 16), src, bytes, bar);
-                        }
+                        const uint32_t bytes = (uint32_t)P.window * EB;
+                        mbar_expect_tx(bar, bytes);
+                        const unsigned char *src = grp + (((size_t)(e0 + k) * P.n_rx_max + j) * P.l_row + s0) * EB;
+                        bulk_g2s(smem_u32(smem) + slot * P.stage_stride, src, bytes, bar);
                     }
                     ++stage_ctr;
                 }
@@ -191,97 +173,110 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const RingLau
     }
 
     // ===================================== CONSUMER WARPS =====================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRingConsumerRegs));
     const int t = threadIdx.x;
+    const float fcfs = P.fcfs;
     for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
         const int g = w / tiles_all;
         int tt = w - g * tiles_all;
         const int a = tt >= P.ap[0].n_tiles ? 1 : 0;
         if (a) tt -= P.ap[0].n_tiles;
-        const RingApertureArgs &A = P.ap[a];
-        const int tile_z = tt / A.tiles_x, tile_x = tt - tile_z * A.tiles_x;
-        const int ix0 = tile_x * A.tx, iz0 = tile_z * A.tz;
-        const int tx = min(A.tx, A.n_lat - ix0), tz = min(A.tz, A.n_ax - iz0);
-        const int npx = tx * tz;
+        const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+        const int pos0 = tt * kRingConsumers;
+        const int iz0 = (pos0 / n_lat) * PX;                                // first row of the tile
+        const int n_pos = n_lat * ((n_ax + PX - 1) / PX);
+        const int last_pos = min(pos0 + kRingConsumers, n_pos) - 1;
+        const int rows = min(n_ax, (last_pos / n_lat + 1) * PX) - iz0;      // rows the tile touches
+        const int rows_cap = kRingMaxTab / n_tx;                             // table row stride (>= rows, host-checked)
 
         consumer_bar();     // everybody has left the previous work item: the tables may be rewritten
-        for (int i = t; i < A.n_tx * tz; i += kRingConsumers) {
-            const int k = i / tz, izl = i - k * tz;
-            const int base = k * A.n_ax + iz0;
-            s_bt[k * A.tz + izl] = (float)(A.n0[base + izl] - A.n0[base]) + A.f0m[base + izl];
-        }
-        for (int i = t; i < A.n_rx; i += kRingConsumers) {
-            s_ejs[i] = A.ejs[i];
-            if (APOD) { s_win[i] = A.win[i]; s_ejm[i] = A.ejm[i]; }
+        {
+            const int *n0 = ULM_AP(n0);
+            const float *f0m = ULM_AP(f0m);
+            const float2 *tph = ULM_AP(tph);
+            for (int i = t; i < n_tx * rows; i += kRingConsumers) {
+                const int k = i / rows, r = i - k * rows;
+                const int base = k * n_ax + iz0;
+                const float2 T = tph[base + r];
+                s_tab[k * rows_cap + r] = make_float4((float)(n0[base + r] - n0[base]) + f0m[base + r], T.x, T.y, 0.f);
+            }
+            const float *ejs = ULM_AP(ejs), *win = ULM_AP(win), *ejm = ULM_AP(ejm);
+            const int *dj = ULM_AP(dj) + (size_t)tt * n_rx;
+            for (int i = t; i < n_rx; i += kRingConsumers) {
+                s_ejs[i] = ejs[i];
+                s_dj[i] = (float)dj[i];
+                if (APOD) { s_win[i] = win[i]; s_ejm[i] = ejm[i]; }
+            }
         }
         consumer_bar();
 
-        // this thread's pixels
-        float xs[kRingPx], zs[kRingPx], xm[kRingPx], zm[kRingPx];
-        int bt_off[kRingPx], pix[kRingPx];
+        // this thread's PX vertically adjacent pixels
+        int pos = pos0 + t;
+        const bool active = pos <= last_pos;
+        if (!active) pos = last_pos;
+        const int strip = pos / n_lat, ix = pos - strip * n_lat;
+        const int r0 = strip * PX - iz0;                                     // tile-relative first row
+        const float xs = ULM_AP(xs)[ix];
+        float zs[PX], xm = 0.f, zm[PX];
+        if (APOD) xm = ULM_AP(xm)[ix];
 #pragma unroll
-        for (int m = 0; m < kRingPx; ++m) {
-            int q = t + m * kRingConsumers;
-            const bool ok = q < npx;
-            if (!ok) q = npx - 1;
-            const int izl = q / tx, ixl = q - izl * tx;
-            xs[m] = A.xs[ix0 + ixl];
-            zs[m] = A.zs[iz0 + izl];
-            if (APOD) { xm[m] = A.xm[ix0 + ixl]; zm[m] = A.zm[iz0 + izl]; }
-            bt_off[m] = izl;
-            pix[m] = ok ? (ix0 + ixl) * A.n_ax + iz0 + izl : -1;
+        for (int m = 0; m < PX; ++m) {
+            const int iz = min(strip * PX + m, n_ax - 1);
+            zs[m] = ULM_AP(zs)[iz];
+            if (APOD) zm[m] = ULM_AP(zm)[iz];
         }
-        float accr[kRingPx][F], acci[kRingPx][F];
+        const uint32_t tab_addr = smem_u32(s_tab + min(r0, rows - 1));
+        // rows past the image bottom re-read the last table row (their results are never stored)
+        uint32_t tab_off[PX];
 #pragma unroll
-        for (int m = 0; m < kRingPx; ++m)
+        for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 16u;
+
+        float accr[PX][F], acci[PX][F];
+#pragma unroll
+        for (int m = 0; m < PX; ++m)
 #pragma unroll
             for (int f = 0; f < F; ++f) accr[m][f] = acci[m][f] = 0.f;
 
-        const float fcfs = (float)P.fcfs;
-        for (int j = 0; j < A.n_rx; ++j) {
-            float H[kRingPx], wgt[kRingPx];
-            const float ej = s_ejs[j];
-#pragma unroll
-            for (int m = 0; m < kRingPx; ++m) {
-                const float dxs = xs[m] - ej;
+        for (int j = 0; j < n_rx; ++j) {
+            float Hs[PX], Rr[PX], Ri[PX];
+            {
+                const float dxs = xs - s_ejs[j];
                 const float dx2 = dxs * dxs;
-                const float den = sqrtf(fmaf(zs[m], zs[m], dx2)) + zs[m];
-                H[m] = den > 0.f ? __fdividef(dx2, den) : 0.f;
-                if (APOD) {
-                    float wv = s_win[j];
-                    if (P.two_f > 0.f) {
-                        const float lhs = __fmul_rn(fabsf(__fsub_rn(xm[m], s_ejm[j])), P.two_f);
-                        if (!(lhs <= zm[m])) wv = 0.f;
+                const float djf = s_dj[j];
+#pragma unroll
+                for (int m = 0; m < PX; ++m) {
+                    const float den = sqrtf(fmaf(zs[m], zs[m], dx2)) + zs[m];
+                    const float H = den > 0.f ? __fdividef(dx2, den) : 0.f;
+                    Hs[m] = H - djf;
+                    sincos_cycles(fcfs * H, Ri[m], Rr[m]);
+                    if (APOD) {
+                        float wv = s_win[j];
+                        if (P.two_f > 0.f) {
+                            const float lhs = __fmul_rn(fabsf(__fsub_rn(xm, s_ejm[j])), P.two_f);
+                            if (!(lhs <= zm[m])) wv = 0.f;
+                        }
+                        Rr[m] *= wv; Ri[m] *= wv;
                     }
-                    wgt[m] = wv;
                 }
             }
-            for (int k = 0; k < A.n_tx; ++k) {
+            for (int k = 0; k < n_tx; ++k) {
                 const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
                 mbar_wait(smem_u32(&s_full[slot]), phase);
-                const float4 hdr = s_hdr[slot];
-                // entry address = stage base + 16 * rint(upm); the magic-constant bits are folded into cbase
-                const uint32_t cbase = smem_u32(smem) + slot * kStageBytes - ((uint32_t)kMagicBits << 4);
-                const float *bt = s_bt + k * A.tz;
+                // entry address = stage base + EB * (rint(upm) + shift); the magic-constant bits are folded in
+                const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride + (uint32_t)(s_hdr[slot] - kMagicBits) * EB;
+                const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
 #pragma unroll
-                for (int m = 0; m < kRingPx; ++m) {
-                    const float upm = (bt[bt_off[m]] + hdr.x) + H[m];
+                for (int m = 0; m < PX; ++m) {
+                    const uint4 tb = lds128(tk + tab_off[m]);
+                    const float upm = __uint_as_float(tb.x) + Hs[m];
                     const float tt_ = upm + kMagic;
                     const float al = upm - (tt_ - kMagic);
-                    const uint32_t addr = ((uint32_t)__float_as_int(tt_) << 4) + cbase;
-                    float s, c;
-                    sincos_cycles(fmaf(fcfs, upm, hdr.y), s, c);
-                    if (APOD) { s *= wgt[m]; c *= wgt[m]; }
-                    float4 e[F];
-#pragma unroll
-                    for (int f = 0; f < F; ++f) e[f] = lds128(addr + f * (WS * 16));
-#pragma unroll
-                    for (int f = 0; f < F; ++f) {
-                        const float vr = fmaf(al, e[f].z, e[f].x), vi = fmaf(al, e[f].w, e[f].y);
-                        accr[m][f] = fmaf(c, vr, accr[m][f]);
-                        accr[m][f] = fmaf(-s, vi, accr[m][f]);
-                        acci[m][f] = fmaf(s, vr, acci[m][f]);
-                        acci[m][f] = fmaf(c, vi, acci[m][f]);
-                    }
+                    const uint32_t addr = (uint32_t)__float_as_int(tt_) * EB + cbase;
+                    const float Tr = __uint_as_float(tb.y), Ti = __uint_as_float(tb.z);
+                    const float c = fmaf(Tr, Rr[m], -Ti * Ri[m]);
+                    const float s = fmaf(Tr, Ri[m], Ti * Rr[m]);
+                    entry_mac<F, D32>([&](int i) { return lds128(addr + 16u * i); }, make_alpha(al), c, s,
+                                      accr[m], acci[m]);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&s_empty[slot]));
@@ -289,17 +284,24 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const RingLau
             }
         }
         // projection write: one float2 per pixel and frame
+        if (active) {
+            const long long out_base = ULM_AP(out_base);
 #pragma unroll
-        for (int m = 0; m < kRingPx; ++m) {
-            if (pix[m] < 0) continue;
+            for (int m = 0; m < PX; ++m) {
+                const int iz = strip * PX + m;
+                if (iz >= n_ax) continue;
 #pragma unroll
-            for (int f = 0; f < F; ++f) {
-                const int fr = g * F + f;
-                if (fr < P.n_frames)
-                    P.out[(long long)fr * P.out_frame_stride + A.out_base + pix[m]] = make_float2(accr[m][f], acci[m][f]);
+                for (int f = 0; f < F; ++f) {
+                    const int fr = g * F + f;
+                    if (fr < P.n_frames)
+                        P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] =
+                            make_float2(accr[m][f], acci[m][f]);
+                }
             }
         }
     }
 }
+
+#undef ULM_AP
 
 }  // namespace ulm

@@ -1,5 +1,5 @@
-// ulm_rca_ring_host.cuh -- host side of the shared-memory ring kernel: tile shape and window planning
-// (fp64), the per-(tile, element, angle) window-start table, and the templated launch.
+// ulm_rca_ring_host.cuh -- host side of the shared-memory ring kernel: tile and window planning (fp64),
+// the per-(tile, element) window-offset table, and the templated launch.
 #pragma once
 
 #include <algorithm>
@@ -11,6 +11,25 @@
 namespace ulm {
 
 constexpr int kSmemLimit = 232448;   // 227 KB opt-in dynamic shared memory per CTA on sm_100
+constexpr int kRingPx = 4;           // rows per strip = pixels per consumer thread
+constexpr int kRingMisc = kRingMaxTab * 16 + 4 * kRingMaxRx * 4 + kRingMaxStages * 4 + 2 * kRingMaxStages * 8 + 64;
+
+struct RingConfig {
+    int window = 0;      // entries per stage
+    int n_sms = 0;
+};
+
+struct RingTables {
+    int n_tiles = 0;
+    int *d_dj = nullptr;     // [tile][j] floor(min H over the tile) - 2
+    ~RingTables() { if (d_dj) cudaFree(d_dj); }
+};
+
+struct RingApertureDesc {
+    int n_tx, n_rx, n_lat, n_ax;
+    double lat0, dlat, z0, dz, ref;
+    const double *angles, *t0;
+};
 
 namespace ringhost {
 
@@ -24,173 +43,148 @@ struct Geo {
         return (d->t0[k] + (z * std::cos(d->angles[k]) + d->ref * std::sin(d->angles[k])) / c + z / c - t_start) * fs;
     }
     double h(double dx, double z) const { return (std::sqrt(dx * dx + z * z) - z) * fs / c; }
-    // delay range [u_lo, u_hi] (samples) of tile x [ix0, ix1] x z [iz0, iz1] for angle k, element j:
-    // U0 grows with z, H grows with |dx| and shrinks with z
-    void range(int ix0, int ix1, int iz0, int iz1, int k, int j, double &u_lo, double &u_hi) const {
-        const double la = lat(ix0), lb = lat(ix1), e = elem(j);
-        const double lo = std::min(la, lb), hi = std::max(la, lb);
-        const double dmin = (e >= lo && e <= hi) ? 0.0 : std::min(std::fabs(la - e), std::fabs(lb - e));
-        const double dmax = std::max(std::fabs(la - e), std::fabs(lb - e));
-        u_lo = u0(k, z(iz0)) + h(dmin, z(iz1));
-        u_hi = u0(k, z(iz1)) + h(dmax, z(iz0));
+};
+
+// one strip segment of a tile: columns [c0, c1], rows [r0, r1] (image rows)
+struct Seg { int c0, c1, r0, r1; };
+
+inline std::vector<Seg> tile_segments(const RingApertureDesc &D, int tile) {
+    const int n_pos = D.n_lat * ((D.n_ax + kRingPx - 1) / kRingPx);
+    const int p0 = tile * kRingConsumers, p1 = std::min(p0 + kRingConsumers, n_pos) - 1;
+    std::vector<Seg> v;
+    for (int s = p0 / D.n_lat; s <= p1 / D.n_lat; ++s) {
+        Seg g;
+        g.c0 = s == p0 / D.n_lat ? p0 % D.n_lat : 0;
+        g.c1 = s == p1 / D.n_lat ? p1 % D.n_lat : D.n_lat - 1;
+        g.r0 = s * kRingPx;
+        g.r1 = std::min(s * kRingPx + kRingPx - 1, D.n_ax - 1);
+        v.push_back(g);
     }
-};
-
-struct Tiling {
-    int tx = 0, tz = 0, tiles_x = 0, tiles_z = 0, window = 0;
-    int n_tiles() const { return tiles_x * tiles_z; }
-};
-
-inline int window_of(const Geo &G, const Tiling &T) {
-    int w = 0;
-    const RingApertureDesc &D = *G.d;
-    for (int tzi = 0; tzi < T.tiles_z; ++tzi)
-        for (int txi = 0; txi < T.tiles_x; ++txi) {
-            const int ix0 = txi * T.tx, ix1 = std::min(D.n_lat, ix0 + T.tx) - 1;
-            const int iz0 = tzi * T.tz, iz1 = std::min(D.n_ax, iz0 + T.tz) - 1;
-            for (int k = 0; k < D.n_tx; ++k)
-                for (int j = 0; j < D.n_rx; ++j) {
-                    double lo, hi;
-                    G.range(ix0, ix1, iz0, iz1, k, j, lo, hi);
-                    w = std::max(w, (int)std::floor(hi) - (int)std::floor(lo) + 6);
-                }
-        }
-    return w;
+    return v;
 }
 
-// pick the tile shape that minimises  tiles * (pixel capacity + window)  ~ shared-memory traffic
-inline bool choose_tiling(const Geo &G, int max_window, Tiling &best) {
-    const RingApertureDesc &D = *G.d;
-    double best_cost = 1e300;
-    bool found = false;
-    for (int tiles_x = 1; tiles_x <= std::max(1, D.n_lat / 8); ++tiles_x) {
-        Tiling T;
-        T.tiles_x = tiles_x;
-        T.tx = (D.n_lat + tiles_x - 1) / tiles_x;
-        T.tiles_x = (D.n_lat + T.tx - 1) / T.tx;
-        int tz = std::min({D.n_ax, kRingTilePixels / T.tx, kRingMaxTz, kRingMaxBt / std::max(1, D.n_tx)});
-        if (tz < 1) continue;
-        T.tiles_z = (D.n_ax + tz - 1) / tz;
-        T.tz = (D.n_ax + T.tiles_z - 1) / T.tiles_z;
-        T.window = (window_of(G, T) + 7) / 8 * 8;
-        if (T.window > max_window) continue;
-        const double cost = (double)T.n_tiles() * (kRingTilePixels + T.window);
-        if (cost < best_cost) { best_cost = cost; best = T; found = true; }
-    }
-    return found;
+// receive-excess range [h_lo, h_hi] of element j over a segment: H grows with |dx| and shrinks with z
+inline void h_range(const Geo &G, const Seg &s, int j, double &h_lo, double &h_hi) {
+    const double la = G.lat(s.c0), lb = G.lat(s.c1), e = G.elem(j);
+    const double lo = std::min(la, lb), hi = std::max(la, lb);
+    const double dmin = (e >= lo && e <= hi) ? 0.0 : std::min(std::fabs(la - e), std::fabs(lb - e));
+    const double dmax = std::max(std::fabs(la - e), std::fabs(lb - e));
+    h_lo = G.h(dmin, G.z(s.r1));
+    h_hi = G.h(dmax, G.z(s.r0));
 }
 
 }  // namespace ringhost
 
-// Plans both apertures.  Returns false (with *why) when the ring kernel does not cover the shape.
-inline bool ring_plan(const RingApertureDesc *desc, double pitch, double c, double fs, double t_start, int n_lo,
-                      int l_row, bool /*apod*/, RingConfig &cfg, RingTables &tab0, RingTables &tab1, const char **why) {
+// Plans one aperture: fills dj (host) and returns the window (entries) it needs, or -1 with *why.
+inline int ring_plan_aperture(const RingApertureDesc &D, double pitch, double c, double fs, double t_start,
+                              std::vector<int> &dj, int &n_tiles, const char **why) {
     using namespace ringhost;
+    n_tiles = 0;
+    dj.clear();
+    if (D.n_tx == 0) return 0;
+    if (D.n_rx > kRingMaxRx) { *why = "more than 256 receive elements"; return -1; }
+    Geo G{&D, pitch, c, fs, t_start};
+    const int n_pos = D.n_lat * ((D.n_ax + kRingPx - 1) / kRingPx);
+    n_tiles = (n_pos + kRingConsumers - 1) / kRingConsumers;
+    dj.assign((size_t)n_tiles * D.n_rx, 0);
+    int window = 8;
+    for (int t = 0; t < n_tiles; ++t) {
+        const std::vector<Seg> segs = tile_segments(D, t);
+        const int iz0 = segs.front().r0, rows = segs.back().r1 - iz0 + 1;
+        if ((long long)rows * D.n_tx > kRingMaxTab) { *why = "tile rows x angles exceed the transmit table"; return -1; }
+        for (int j = 0; j < D.n_rx; ++j) {
+            double h_min = 1e300;
+            for (const Seg &s : segs) {
+                double lo, hi;
+                h_range(G, s, j, lo, hi);
+                h_min = std::min(h_min, lo);
+            }
+            const int d = (int)std::floor(h_min) - 2;
+            dj[(size_t)t * D.n_rx + j] = d;
+            for (const Seg &s : segs) {
+                double lo, hi;
+                h_range(G, s, j, lo, hi);
+                for (int k = 0; k < D.n_tx; ++k) {
+                    // upm = U0_k(z_r) - floor(U0_k(z_iz0)) - 0.5 + H - dj; the entry index is rint(upm)
+                    const double top = G.u0(k, G.z(s.r1)) - std::floor(G.u0(k, G.z(iz0))) - 0.5 + hi - d;
+                    window = std::max(window, (int)std::floor(top + 0.5) + 4);
+                }
+            }
+        }
+    }
+    return window;
+}
+
+inline int ring_stage_stride(int window, int F, bool d32) { return (window * entry_bytes(F, d32) + 127) / 128 * 128; }
+inline int ring_stages(int window, int F, bool d32) {
+    return std::min(kRingMaxStages, (kSmemLimit - kRingMisc) / ring_stage_stride(window, F, d32));
+}
+inline int ring_smem_bytes(int window, int F, bool d32) {
+    return ring_stages(window, F, d32) * ring_stage_stride(window, F, d32) + kRingMisc;
+}
+
+// Plans both apertures.  Returns false (with *why) when the ring kernel does not cover the shape.
+inline bool ring_plan(const RingApertureDesc *desc, double pitch, double c, double fs, double t_start,
+                      int l_row, RingConfig &cfg, RingTables &tab0, RingTables &tab1, const char **why) {
     RingTables *tabs[2] = {&tab0, &tab1};
-    Tiling til[2];
     int window = 8;
     for (int a = 0; a < 2; ++a) {
-        const RingApertureDesc &D = desc[a];
-        if (D.n_tx == 0) continue;
-        if (D.n_rx > kRingMaxRx) { *why = "more than 256 receive elements"; return false; }
-        if (D.n_tx > kRingMaxBt) { *why = "too many angles"; return false; }
-        Geo G{&D, pitch, c, fs, t_start};
-        if (!choose_tiling(G, 512, til[a])) { *why = "no tile shape whose window fits 512 entries"; return false; }
-        window = std::max(window, til[a].window);
-    }
-    if (window > l_row) { *why = "window exceeds the scratch row"; return false; }
-    const int ws_opts[5] = {128, 192, 256, 384, 512};
-    int ws = 0;
-    for (int o : ws_opts) if (o >= window) { ws = o; break; }
-    if (!ws) { *why = "window too large"; return false; }
-
-    for (int a = 0; a < 2; ++a) {
-        const RingApertureDesc &D = desc[a];
-        RingTables &T = *tabs[a];
-        if (D.n_tx == 0) { T.n_tiles = 0; continue; }
-        Geo G{&D, pitch, c, fs, t_start};
-        const Tiling &L = til[a];
-        T.n_tiles = L.n_tiles(); T.tx = L.tx; T.tz = L.tz; T.tiles_x = L.tiles_x; T.tiles_z = L.tiles_z;
-        std::vector<int> s0((size_t)T.n_tiles * D.n_rx * D.n_tx);
-        size_t i = 0;
-        for (int tzi = 0; tzi < L.tiles_z; ++tzi)
-            for (int txi = 0; txi < L.tiles_x; ++txi) {
-                const int ix0 = txi * L.tx, ix1 = std::min(D.n_lat, ix0 + L.tx) - 1;
-                const int iz0 = tzi * L.tz, iz1 = std::min(D.n_ax, iz0 + L.tz) - 1;
-                for (int j = 0; j < D.n_rx; ++j)
-                    for (int k = 0; k < D.n_tx; ++k, ++i) {
-                        double lo, hi;
-                        G.range(ix0, ix1, iz0, iz1, k, j, lo, hi);
-                        int rel = (int)std::floor(lo) - 2 - n_lo;
-                        rel = std::max(0, std::min(rel, l_row - window));
-                        s0[i] = rel;
-                    }
-            }
-        if (cudaMalloc(&T.d_s0, s0.size() * sizeof(int)) != cudaSuccess) { *why = "table allocation failed"; return false; }
-        if (cudaMemcpy(T.d_s0, s0.data(), s0.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+        std::vector<int> dj;
+        const int w = ring_plan_aperture(desc[a], pitch, c, fs, t_start, dj, tabs[a]->n_tiles, why);
+        if (w < 0) return false;
+        window = std::max(window, w);
+        if (dj.empty()) continue;
+        if (cudaMalloc(&tabs[a]->d_dj, dj.size() * sizeof(int)) != cudaSuccess) { *why = "table allocation failed"; return false; }
+        if (cudaMemcpy(tabs[a]->d_dj, dj.data(), dj.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
             *why = "table upload failed";
             return false;
         }
     }
+    window = (window + 7) / 8 * 8;
+    if (window > l_row) { *why = "window exceeds the scratch row"; return false; }
+    if (ring_stages(window, 12, true) < 2) { *why = "fewer than two ring stages fit in shared memory"; return false; }
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cfg.frames = 8;
-    cfg.tile_pixels = kRingTilePixels;
     cfg.window = window;
-    cfg.ws = ws;
     cfg.n_sms = sms;
-    const int misc = kRingMaxBt * 4 + 3 * kRingMaxRx * 4 + kRingMaxStages * 16 + 2 * kRingMaxStages * 8 + 64;
-    cfg.stages = std::min(kRingMaxStages, (kSmemLimit - misc) / (8 * ws * 16));
-    cfg.smem_bytes = cfg.stages * 8 * ws * 16 + misc;
-    if (cfg.stages < 2) { *why = "fewer than two ring stages fit in shared memory"; return false; }
     return true;
 }
 
-template <int F, int WS, bool APOD>
+template <int F, bool D32, bool APOD>
 inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) {
-    const int misc = kRingMaxBt * 4 + 3 * kRingMaxRx * 4 + kRingMaxStages * 16 + 2 * kRingMaxStages * 8 + 64;
-    const int stages = std::min(kRingMaxStages, (kSmemLimit - misc) / (F * WS * 16));
-    const int smem = stages * F * WS * 16 + misc;
-    L.n_stages = stages;
+    L.stage_stride = ring_stage_stride(cfg.window, F, D32);
+    L.n_stages = ring_stages(cfg.window, F, D32);
     L.n_groups = (L.n_frames + F - 1) / F;
     L.n_work = L.n_groups * (L.ap[0].n_tiles + L.ap[1].n_tiles);
     if (L.n_work == 0) return 0;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(das_ring_kernel<F, WS, APOD>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+        cudaFuncSetAttribute(das_ring_kernel<F, kRingPx, D32, APOD>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
         attr_set = true;
     }
     const int grid = std::min(L.n_work, cfg.n_sms);
-    das_ring_kernel<F, WS, APOD><<<grid, kRingThreads, smem, st>>>(L);
+    das_ring_kernel<F, kRingPx, D32, APOD><<<grid, kRingThreads, ring_smem_bytes(cfg.window, F, D32), st>>>(L);
     return 1;
 }
 
-template <int F, bool APOD>
-inline int ring_launch_ws(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) {
-    switch (cfg.ws) {
-        case 128: return ring_launch_t<F, 128, APOD>(cfg, L, st);
-        case 192: return ring_launch_t<F, 192, APOD>(cfg, L, st);
-        case 256: return ring_launch_t<F, 256, APOD>(cfg, L, st);
-        case 384: return ring_launch_t<F, 384, APOD>(cfg, L, st);
-        default: return ring_launch_t<F, 512, APOD>(cfg, L, st);
-    }
+template <int F, bool D32>
+inline int ring_launch_a(const RingConfig &cfg, RingLaunch &L, bool apod, cudaStream_t st) {
+    return apod ? ring_launch_t<F, D32, true>(cfg, L, st) : ring_launch_t<F, D32, false>(cfg, L, st);
 }
 
-// returns the number of kernels launched
+// returns the number of kernels launched; F = frames per group of the scratch (4 or 12), d32 = full entries
 inline int ring_launch(const RingConfig &cfg, const RingTables &tab0, const RingTables &tab1, const RingLaunch &Lin,
-                       bool apod, cudaStream_t st) {
+                       int F, bool d32, bool apod, cudaStream_t st) {
     RingLaunch L = Lin;
     const RingTables *tabs[2] = {&tab0, &tab1};
     for (int a = 0; a < 2; ++a) {
-        L.ap[a].s0 = tabs[a]->d_s0;
+        L.ap[a].dj = tabs[a]->d_dj;
         L.ap[a].n_tiles = L.ap[a].n_tx > 0 ? tabs[a]->n_tiles : 0;
-        L.ap[a].tx = tabs[a]->tx; L.ap[a].tz = tabs[a]->tz; L.ap[a].tiles_x = std::max(1, tabs[a]->tiles_x);
     }
     L.window = cfg.window;
-    if (L.n_frames > 2)
-        return apod ? ring_launch_ws<8, true>(cfg, L, st) : ring_launch_ws<8, false>(cfg, L, st);
-    return apod ? ring_launch_ws<2, true>(cfg, L, st) : ring_launch_ws<2, false>(cfg, L, st);
+    if (F == 12) return d32 ? ring_launch_a<12, true>(cfg, L, apod, st) : ring_launch_a<12, false>(cfg, L, apod, st);
+    return d32 ? ring_launch_a<4, true>(cfg, L, apod, st) : ring_launch_a<4, false>(cfg, L, apod, st);
 }
 
 }  // namespace ulm
