@@ -266,7 +266,8 @@ void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames
 
 template <int NT, bool IQ, int F, bool D32>
 cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, unsigned blocks, cudaStream_t st) {
-    const size_t smem = (size_t)F * ((ulm::kDemodChunk + 1 + 2 * L + 1) + (ulm::kDemodChunk + 2)) * sizeof(float2);
+    const int xw = ulm::kDemodChunk + 1 + 2 * L;
+    const size_t smem = (size_t)F * ((xw + xw / 8 + 2) + (ulm::kDemodChunk + 2)) * sizeof(float2);
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;

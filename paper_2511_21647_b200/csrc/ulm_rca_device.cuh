@@ -98,7 +98,8 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     constexpr int IQS = NIQ + 1;               // row stride of s_iq (float2)
     const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
     const int XW = NIQ + 2 * L;                // mixed samples per frame
-    const int XS = XW + 1;                     // row stride of s_x (float2), odd
+    const int XS = XW + XW / 8 + 2;            // row stride of s_x (float2): one pad slot after every 8 samples, so
+                                               // that the FIR threads (8 samples apart) hit distinct banks
     float2 *s_x = s_dyn;                       // [F][XS]
     float2 *s_iq = s_dyn + F * XS;             // [F][IQS]
 
@@ -131,7 +132,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
                 v = make_float2(r * m.x, r * m.y);
             }
         }
-        s_x[f * XS + i] = v;
+        s_x[f * XS + i + (i >> 3)] = v;
     }
     __syncthreads();
 
@@ -139,14 +140,14 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     constexpr int R = 8;
     if (threadIdx.x < F * (NIQ / R)) {
         const int f = threadIdx.x / (NIQ / R), r0 = (threadIdx.x - f * (NIQ / R)) * R;
-        const float2 *x = s_x + f * XS + r0;
+        const float2 *x = s_x + f * XS + r0 + (r0 >> 3);     // r0 is a multiple of 8: x[u + u/8] = sample r0 + u
         float ar[R], ai[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) ar[q] = ai[q] = 0.f;
         if (NT > 0) {
 #pragma unroll
             for (int u = 0; u < R + NT - 1; ++u) {
-                const float2 xv = x[u];
+                const float2 xv = x[u + (u >> 3)];
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
                     const int t = q - u + (NT - 1);
@@ -158,7 +159,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             }
         } else {
             for (int u = 0; u < R + 2 * L; ++u) {
-                const float2 xv = x[u];
+                const float2 xv = x[u + (u >> 3)];
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
                     const int t = q - u + 2 * L;

@@ -158,7 +158,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                         const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
                         const int s0 = max(0, min(s0_raw, P.l_row - P.window));
                         mbar_wait(smem_u32(&s_empty[slot]), phase ^ 1);
-                        s_hdr[slot] = s0_raw - s0;
+                        s_hdr[slot] = s0_raw - s0 - kMagicBits;     // entry shift, with the magic-constant bits folded in
                         const uint32_t bar = smem_u32(&s_full[slot]);
                         const uint32_t bytes = (uint32_t)P.window * EB;
                         mbar_expect_tx(bar, bytes);
@@ -262,8 +262,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             for (int k = 0; k < n_tx; ++k) {
                 const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
                 mbar_wait(smem_u32(&s_full[slot]), phase);
-                // entry address = stage base + EB * (rint(upm) + shift); the magic-constant bits are folded in
-                const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride + (uint32_t)(s_hdr[slot] - kMagicBits) * EB;
+                // entry address = stage base + EB * (rint(upm) + shift); hdr = shift - magic-constant bits
+                const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride;
+                const int hdr = s_hdr[slot];
                 const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
 #pragma unroll
                 for (int m = 0; m < PX; ++m) {
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     const float upm = __uint_as_float(tb.x) + Hs[m];
                     const float tt_ = upm + kMagic;
                     const float al = upm - (tt_ - kMagic);
-                    const uint32_t addr = (uint32_t)__float_as_int(tt_) * EB + cbase;
+                    const uint32_t addr = (uint32_t)(__float_as_int(tt_) + hdr) * EB + cbase;
                     const float Tr = __uint_as_float(tb.y), Ti = __uint_as_float(tb.z);
                     const float c = fmaf(Tr, Rr[m], -Ti * Ri[m]);
                     const float s = fmaf(Tr, Ri[m], Ti * Rr[m]);
