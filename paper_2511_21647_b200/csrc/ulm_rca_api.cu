@@ -93,6 +93,7 @@ struct ulm_rca_plan {
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
     bool d32 = false;             // full (fp32) difference term in the scratch
+    bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
     mutable long long last_launches = 0;
@@ -193,6 +194,9 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
         D.gd[t] = std::fabs(g) < 1e-13 ? 0.f : (float)g;     // exact zeros of the sinc (every 2nd tap at fs = 4 fc)
     }
     P.half_len = D.half_len = L;
+    P.half_band = true;
+    for (int t = 0; t <= 2 * L; ++t)
+        if (t != L && ((t - L) & 1) == 0 && D.gd[t] != 0.f) P.half_band = false;
     return ULM_RCA_OK;
 }
 
@@ -264,25 +268,25 @@ void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames
     else launch_generic_f<4>(P, D, n_frames, st);
 }
 
-template <int NT, bool IQ, int F, bool D32>
+template <int NT, bool HB, bool IQ, int F, bool D32>
 cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, unsigned blocks, cudaStream_t st) {
-    const int xw = ulm::kDemodChunk + 1 + 2 * L;
-    const size_t smem = (size_t)F * ((xw + xw / 8 + 2) + (ulm::kDemodChunk + 2)) * sizeof(float2);
+    const size_t smem = (size_t)ulm::demod_smem_bytes(F, D32, L);
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, HB, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    ulm::demod_kernel<NT, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
+    ulm::demod_kernel<NT, HB, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
     return cudaSuccess;
 }
 
 template <int F, bool D32>
 cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, unsigned blocks, cudaStream_t st) {
     const int L = P.half_len;
-    if (P.input_kind == 1) return launch_demod_t<1, true, F, D32>(D, 0, blocks, st);
-    if (L == 8) return launch_demod_t<17, false, F, D32>(D, L, blocks, st);
-    if (L == 16) return launch_demod_t<33, false, F, D32>(D, L, blocks, st);
-    return launch_demod_t<0, false, F, D32>(D, L, blocks, st);
+    if (P.input_kind == 1) return launch_demod_t<1, false, true, F, D32>(D, 0, blocks, st);
+    if (L == 8) return P.half_band ? launch_demod_t<17, true, false, F, D32>(D, L, blocks, st)
+                                   : launch_demod_t<17, false, false, F, D32>(D, L, blocks, st);
+    if (L == 16) return launch_demod_t<33, false, false, F, D32>(D, L, blocks, st);
+    return launch_demod_t<0, false, false, F, D32>(D, L, blocks, st);
 }
 
 cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, cudaStream_t st) {

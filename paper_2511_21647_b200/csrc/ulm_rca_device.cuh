@@ -84,24 +84,36 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
 // ---------------------------------------------------------------------------------------------------
 // Demodulation / staging pre-pass: int16 RF (or IQ) -> scratch entries over the touched
 // sample range only.  One CTA = one chunk of 127 entries of one (frame group, event, rx element) row, all F
-// frames of the group: (1) the mixed samples x = rf * exp(-j 2 pi fc t) go to shared memory, (2) each
-// thread runs the FIR for 8 consecutive outputs of one frame with the inputs sliding through registers
-// (dense taps straight from constant memory), (3) the entries are assembled and stored as fully
-// coalesced 16-byte chunks.  NT = dense tap count 2L+1 (0: run-time L).
+// frames of the group:
+//   (1) the mixed samples x = rf * exp(-j 2 pi fc t) of the F frames go to shared memory;
+//   (2) thread (frame f, group of 8 entries) runs the FIR for 9 consecutive outputs with the inputs sliding
+//       through registers (dense taps straight from constant memory; HB = half-band filter, fs = 4 fc: the
+//       even taps other than the centre are exactly zero and are skipped at compile time), forms
+//       mid = (a + b)/2 and d = b - a and writes them into an image of the output block in shared memory;
+//   (3) one elected thread stores the block (127 x 12 F contiguous bytes) with one cp.async.bulk (TMA).
+// NT = dense tap count 2L+1 (0: run-time L).  Lanes of a half-warp are the frames of one group, so every
+// shared-memory access of step (2) is conflict free (row stride of x = 1 mod 16 float2).
 // ---------------------------------------------------------------------------------------------------
 __constant__ DemodConst c_demod[1];
 
-template <int NT, bool IQ_INPUT, int F, bool D32>
+__host__ __device__ constexpr int demod_threads_per_group(int F) { return F == 12 ? 16 : F; }
+__host__ __device__ inline int demod_xs(int L) { return ((kDemodChunk + 2 + 2 * L) + 14) / 16 * 16 + 1; }
+__host__ __device__ inline int demod_smem_bytes(int F, bool D32, int L) {
+    return (kDemodChunk * entry_bytes(F, D32) + 127) / 128 * 128 + F * demod_xs(L) * 8;
+}
+
+template <int NT, bool HB, bool IQ_INPUT, int F, bool D32>
 __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
-    extern __shared__ float2 s_dyn[];
-    constexpr int NIQ = kDemodChunk + 1;       // iq values per chunk
-    constexpr int IQS = NIQ + 1;               // row stride of s_iq (float2)
+    extern __shared__ __align__(128) unsigned char s_raw[];
+    constexpr int EB = entry_bytes(F, D32);
+    constexpr int OUT_BYTES = (kDemodChunk * EB + 127) / 128 * 128;
+    constexpr int R = 8;                       // entries per thread
+    constexpr int TPG = demod_threads_per_group(F);
     const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
-    const int XW = NIQ + 2 * L;                // mixed samples per frame
-    const int XS = XW + XW / 8 + 2;            // row stride of s_x (float2): one pad slot after every 8 samples, so
-                                               // that the FIR threads (8 samples apart) hit distinct banks
-    float2 *s_x = s_dyn;                       // [F][XS]
-    float2 *s_iq = s_dyn + F * XS;             // [F][IQS]
+    const int XW = kDemodChunk + 2 + 2 * L;    // mixed samples per frame: iq[0..128] needs x[0 .. 128 + 2L]
+    const int XS = demod_xs(L);                // row stride of s_x (float2)
+    unsigned char *s_out = s_raw;              // [127][EB] image of the output block
+    float2 *s_x = reinterpret_cast<float2 *>(s_raw + OUT_BYTES);   // [F][XS]
 
     const int chunk = blockIdx.x % P.chunks_per_row;
     const long long row = blockIdx.x / P.chunks_per_row;    // (group * n_events + e) * n_rx_max + j
@@ -132,36 +144,37 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
                 v = make_float2(r * m.x, r * m.y);
             }
         }
-        s_x[f * XS + i + (i >> 3)] = v;
+        s_x[f * XS + i] = v;
     }
     __syncthreads();
 
     // (2) FIR: iq[base + r] = sum_{i = r .. r + 2L} gd[r + 2L - i] x[i]   (x index relative to base - L)
-    constexpr int R = 8;
-    if (threadIdx.x < F * (NIQ / R)) {
-        const int f = threadIdx.x / (NIQ / R), r0 = (threadIdx.x - f * (NIQ / R)) * R;
-        const float2 *x = s_x + f * XS + r0 + (r0 >> 3);     // r0 is a multiple of 8: x[u + u/8] = sample r0 + u
-        float ar[R], ai[R];
+    const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
+    const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
+    if (f < F && grp * R < n_ent) {
+        const int r0 = grp * R;
+        const float2 *x = s_x + f * XS + r0;
+        float ar[R + 1], ai[R + 1];
 #pragma unroll
-        for (int q = 0; q < R; ++q) ar[q] = ai[q] = 0.f;
+        for (int q = 0; q <= R; ++q) ar[q] = ai[q] = 0.f;
         if (NT > 0) {
 #pragma unroll
-            for (int u = 0; u < R + NT - 1; ++u) {
-                const float2 xv = x[u + (u >> 3)];
+            for (int u = 0; u < R + NT; ++u) {
+                const float2 xv = x[u];
 #pragma unroll
-                for (int q = 0; q < R; ++q) {
+                for (int q = 0; q <= R; ++q) {
                     const int t = q - u + (NT - 1);
-                    if (t >= 0 && t < NT) {
+                    if (t >= 0 && t < NT && !(HB && t != NT / 2 && ((t - NT / 2) & 1) == 0)) {
                         ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
                         ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
                     }
                 }
             }
         } else {
-            for (int u = 0; u < R + 2 * L; ++u) {
-                const float2 xv = x[u + (u >> 3)];
+            for (int u = 0; u <= R + 2 * L; ++u) {
+                const float2 xv = x[u];
 #pragma unroll
-                for (int q = 0; q < R; ++q) {
+                for (int q = 0; q <= R; ++q) {
                     const int t = q - u + 2 * L;
                     if (t >= 0 && t <= 2 * L) {
                         ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
@@ -171,44 +184,33 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             }
         }
 #pragma unroll
-        for (int q = 0; q < R; ++q) s_iq[f * IQS + r0 + q] = make_float2(ar[q], ai[q]);
-    }
-    __syncthreads();
-
-    // (3) entries: chunk c < F/2 of an entry = mid of frames 2c, 2c+1; then the difference terms: d/16 as
-    // half2 of 4 frames per chunk (compact) or d as float2 of 2 frames per chunk + one padding chunk (full)
-    constexpr int EB = entry_bytes(F, D32);
-    constexpr int CPE = EB / 16;                // 16-byte chunks per entry
-    const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
-    uint4 *dst = reinterpret_cast<uint4 *>(P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB);
-    for (int idx = threadIdx.x; idx < n_ent * CPE; idx += 256) {
-        const int ent = idx / CPE, c = idx - ent * CPE;
-        const int n = base + ent;
-        uint4 o = make_uint4(0u, 0u, 0u, 0u);
-        if (n >= 0 && n + 1 <= P.n_samples - 1 && c < (D32 ? F : CPE)) {      // edge rule: both taps inside the record
-            if (c < F / 2 || D32) {
-                const int cc = c < F / 2 ? c : c - F / 2;
-                const float2 a0 = s_iq[(2 * cc) * IQS + ent], b0 = s_iq[(2 * cc) * IQS + ent + 1];
-                const float2 a1 = s_iq[(2 * cc + 1) * IQS + ent], b1 = s_iq[(2 * cc + 1) * IQS + ent + 1];
-                if (c < F / 2) {
-                    o.x = __float_as_uint(0.5f * (a0.x + b0.x)); o.y = __float_as_uint(0.5f * (a0.y + b0.y));
-                    o.z = __float_as_uint(0.5f * (a1.x + b1.x)); o.w = __float_as_uint(0.5f * (a1.y + b1.y));
-                } else {
-                    o.x = __float_as_uint(b0.x - a0.x); o.y = __float_as_uint(b0.y - a0.y);
-                    o.z = __float_as_uint(b1.x - a1.x); o.w = __float_as_uint(b1.y - a1.y);
-                }
+        for (int q = 0; q < R; ++q) {
+            const int ent = r0 + q;
+            if (ent >= n_ent) break;
+            const int n = base + ent;
+            const bool ok = n >= 0 && n + 1 <= P.n_samples - 1;      // edge rule: both taps inside the record
+            const float mr = ok ? 0.5f * (ar[q] + ar[q + 1]) : 0.f, mi = ok ? 0.5f * (ai[q] + ai[q + 1]) : 0.f;
+            const float dr = ok ? ar[q + 1] - ar[q] : 0.f, di = ok ? ai[q + 1] - ai[q] : 0.f;
+            unsigned char *ep = s_out + ent * EB;
+            reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
+            if (D32) {
+                reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(dr, di);
+                if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
             } else {
-                const int f0 = 4 * (c - F / 2);
-                uint32_t w[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float2 a = s_iq[(f0 + q) * IQS + ent], b = s_iq[(f0 + q) * IQS + ent + 1];
-                    w[q] = pack_h2(kDScale * (b.x - a.x), kDScale * (b.y - a.y));
-                }
-                o = make_uint4(w[0], w[1], w[2], w[3]);
+                reinterpret_cast<uint32_t *>(ep + 8 * F)[f] = pack_h2(kDScale * dr, kDScale * di);
             }
         }
-        dst[idx] = o;
+    }
+    // (3) one bulk store of the block: generic-proxy writes -> async proxy, then TMA shared -> global
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned char *dst = P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB;
+        const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_out);
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"((uint32_t)(n_ent * EB))
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     }
 }
 
