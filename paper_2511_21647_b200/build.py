@@ -41,5 +41,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe() -> str:
+    """Compile the stand-alone shared-memory / pipe-rate micro-benchmark (probes/smem_probe.cu)."""
+    out = os.path.join(HERE, "probes", "smem_probe")
+    src = os.path.join(HERE, "probes", "smem_probe.cu")
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", out, src], check=True, cwd=HERE)
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--probe" in sys.argv:
+        print(build_probe())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

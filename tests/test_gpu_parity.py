@@ -248,3 +248,37 @@ def test_config4_volume_sampled(torch_cuda):
     scale = np.abs(ref).max()
     assert np.abs(got - ref).max() <= TOL * scale
     assert np.abs(vol).max() <= 1.5 * scale * 3       # no garbage anywhere in the volume
+
+
+@pytest.mark.parametrize("index", [2, 3])
+def test_ensemble_full_size_sampled(torch_cuda, index):
+    """Configs 2 and 3 at full size in the launch configuration bench.py times (300 frames, one call,
+    max_frames = 300): a few frames of the moving scene are rendered on the host, tiled over the 300-frame
+    device buffer exactly as bench.py does, and every distinct frame is compared with the oracle at three
+    positions of the ensemble (first group, a middle group, the last frame)."""
+    torch = torch_cuda
+    import bench
+    from paper_2511_21647_b200 import Plan
+    cfg = synth.config(index)
+    dev = torch.device("cuda", 0)
+    channel, host, distinct = bench.make_ensemble(cfg, torch, dev)
+    kw = rounded_kwargs(cfg)
+    p = oracle.OracleParams(**kw)
+    check = [0, 1, 2, 3, 149, 150, 298, 299]
+    with Plan(**kw, max_frames=cfg.n_frames) as plan:
+        out = plan.beamform(channel)
+        torch.cuda.synchronize()
+        info = plan.info()
+        got = out[check].cpu().numpy()
+    assert info["kernel"] == 2 and info["launches_last_call"] == 2
+    del out, channel
+    refs = {}
+    worst = 0.0
+    for row, fr in enumerate(check):
+        d = fr % len(distinct)
+        if d not in refs:
+            refs[d] = oracle.beamform(p, host[d][None])[0]
+        e = rel_err(got[row], refs[d])
+        worst = max(worst, e)
+        assert e <= TOL, "cfg %d frame %d: %.3e" % (index, fr, e)
+    print("PARITY cfg%d full size worst %.3e over frames %s" % (index, worst, check))
