@@ -251,6 +251,22 @@ __device__ __forceinline__ Alpha make_alpha(float al) {
     return a;
 }
 
+// four frames of a compact entry: m0, m1 = mid of frames (0,1), (2,3); dd = d/16 of the four frames as half2
+__device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A, float c,
+                                          float s, float *accr, float *acci) {
+    const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        unsigned short dr, di;
+        split_h2(ds[i], dr, di);
+        const float vr = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[2 * i])));
+        const float vi = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[2 * i + 1])));
+        accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
+        acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
+    }
+}
+
 // interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
 // v = mid + a' d  (compact: two FHFMA per component, d in fp16; full: one FFMA),  acc += (c + j s) v
 template <int F, bool D32, class LoadVec>
@@ -271,21 +287,7 @@ __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, f
         }
     } else {
 #pragma unroll
-        for (int q = 0; q < F / 4; ++q) {
-            const uint4 m0 = ld(2 * q), m1 = ld(2 * q + 1), dd = ld(F / 2 + q);
-            const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
-            const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                unsigned short dr, di;
-                split_h2(ds[i], dr, di);
-                const float vr = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[2 * i])));
-                const float vi = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[2 * i + 1])));
-                const int f = 4 * q + i;
-                accr[f] = fmaf(c, vr, accr[f]); accr[f] = fmaf(-s, vi, accr[f]);
-                acci[f] = fmaf(s, vr, acci[f]); acci[f] = fmaf(c, vi, acci[f]);
-            }
-        }
+        for (int q = 0; q < F / 4; ++q) chunk_mac(ld(2 * q), ld(2 * q + 1), ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q);
     }
 }
 

@@ -44,6 +44,7 @@ struct RingApertureArgs {
     long long out_base;
     // filled by ring_launch from RingTables:
     const int *dj;           // [tile][j] floor(min H over the tile) - 2
+    const int *wj;           // [tile][j] entries of the stages of element j (multiple of 8, <= window)
     int n_tiles;
 };
 
@@ -140,27 +141,31 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             if (a) tt -= P.ap[0].n_tiles;
             const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
             const int e0 = ULM_AP(e0);
-            const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx;
+            const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx, *wj = ULM_AP(wj) + (size_t)tt * n_rx;
             const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
             const int n_st = n_rx * n_tx;
             const unsigned char *grp = P.iq + (size_t)g * P.n_events * P.n_rx_max * P.l_row * EB;
             for (int sb = 0; sb < n_st; sb += 32) {
                 // each lane fetches the (unclamped) window start of one stage
                 const int my = sb + lane;
-                int my_s0 = 0;
-                if (my < n_st) my_s0 = __ldg(n0 + (my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
+                int my_s0 = 0, my_w = 0;
+                if (my < n_st) {
+                    my_s0 = __ldg(n0 + (my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
+                    my_w = __ldg(wj + my / n_tx);
+                }
                 const int cnt = min(32, n_st - sb);
                 for (int i = 0; i < cnt; ++i) {
                     const int s0_raw = __shfl_sync(0xffffffffu, my_s0, i);
+                    const int wlen = __shfl_sync(0xffffffffu, my_w, i);
                     if (lane == 0) {
                         const int st = sb + i;
                         const int j = st / n_tx, k = st - j * n_tx;
                         const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
-                        const int s0 = max(0, min(s0_raw, P.l_row - P.window));
+                        const int s0 = max(0, min(s0_raw, P.l_row - wlen));
                         mbar_wait(smem_u32(&s_empty[slot]), phase ^ 1);
                         s_hdr[slot] = s0_raw - s0 - kMagicBits;     // entry shift, with the magic-constant bits folded in
                         const uint32_t bar = smem_u32(&s_full[slot]);
-                        const uint32_t bytes = (uint32_t)P.window * EB;
+                        const uint32_t bytes = (uint32_t)wlen * EB;
                         mbar_expect_tx(bar, bytes);
                         const unsigned char *src = grp + (((size_t)(e0 + k) * P.n_rx_max + j) * P.l_row + s0) * EB;
                         bulk_g2s(smem_u32(smem) + slot * P.stage_stride, src, bytes, bar);
@@ -266,18 +271,48 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride;
                 const int hdr = s_hdr[slot];
                 const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
-#pragma unroll
-                for (int m = 0; m < PX; ++m) {
+                // per-pixel setup of this stage: entry address, interpolation weight, phasor T_k(z) R(p, j)
+                struct PixCtx { uint32_t addr; Alpha A; float c, s; };
+                auto prep = [&](int m) {
                     const uint4 tb = lds128(tk + tab_off[m]);
                     const float upm = __uint_as_float(tb.x) + Hs[m];
                     const float tt_ = upm + kMagic;
                     const float al = upm - (tt_ - kMagic);
-                    const uint32_t addr = (uint32_t)(__float_as_int(tt_) + hdr) * EB + cbase;
                     const float Tr = __uint_as_float(tb.y), Ti = __uint_as_float(tb.z);
-                    const float c = fmaf(Tr, Rr[m], -Ti * Ri[m]);
-                    const float s = fmaf(Tr, Ri[m], Ti * Rr[m]);
-                    entry_mac<F, D32>([&](int i) { return lds128(addr + 16u * i); }, make_alpha(al), c, s,
-                                      accr[m], acci[m]);
+                    PixCtx x;
+                    x.addr = (uint32_t)(__float_as_int(tt_) + hdr) * EB + cbase;
+                    x.A = make_alpha(al);
+                    x.c = fmaf(Tr, Rr[m], -Ti * Ri[m]);
+                    x.s = fmaf(Tr, Ri[m], Ti * Rr[m]);
+                    return x;
+                };
+                if (D32) {
+#pragma unroll
+                    for (int m = 0; m < PX; ++m) {
+                        const PixCtx x = prep(m);
+                        entry_mac<F, true>([&](int i) { return lds128(x.addr + 16u * i); }, x.A, x.c, x.s, accr[m], acci[m]);
+                    }
+                } else {
+                    // software pipeline over (pixel, 4-frame chunk): the three LDS.128 of step i + 1 are issued
+                    // before the 32 FMAs of step i
+                    constexpr int NQ = F / 4, NSTEP = PX * NQ;
+                    uint4 buf[2][3];
+                    PixCtx cur = prep(0), nxt = cur;
+                    buf[0][0] = lds128(cur.addr); buf[0][1] = lds128(cur.addr + 16u); buf[0][2] = lds128(cur.addr + 8u * F);
+#pragma unroll
+                    for (int st = 0; st < NSTEP; ++st) {
+                        const int m = st / NQ, q = st % NQ;
+                        if (st + 1 < NSTEP) {
+                            const int m1 = (st + 1) / NQ, q1 = (st + 1) % NQ;
+                            if (q1 == 0) nxt = prep(m1);
+                            const uint32_t a1 = q1 == 0 ? nxt.addr : cur.addr;
+                            uint4 *b = buf[(st + 1) & 1];
+                            b[0] = lds128(a1 + 32u * q1); b[1] = lds128(a1 + 32u * q1 + 16u); b[2] = lds128(a1 + 8u * F + 16u * q1);
+                        }
+                        const uint4 *b = buf[st & 1];
+                        chunk_mac(b[0], b[1], b[2], cur.A, cur.c, cur.s, accr[m] + 4 * q, acci[m] + 4 * q);
+                        if (q == NQ - 1) cur = nxt;
+                    }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&s_empty[slot]));

@@ -21,7 +21,7 @@ struct RingConfig {
 
 struct RingTables {
     int n_tiles = 0;
-    int *d_dj = nullptr;     // [tile][j] floor(min H over the tile) - 2
+    int *d_dj = nullptr;     // [tile][j] floor(min H over the tile) - 2, followed by [tile][j] entries the stage needs
     ~RingTables() { if (d_dj) cudaFree(d_dj); }
 };
 
@@ -86,7 +86,7 @@ inline int ring_plan_aperture(const RingApertureDesc &D, double pitch, double c,
     Geo G{&D, pitch, c, fs, t_start};
     const int n_pos = D.n_lat * ((D.n_ax + kRingPx - 1) / kRingPx);
     n_tiles = (n_pos + kRingConsumers - 1) / kRingConsumers;
-    dj.assign((size_t)n_tiles * D.n_rx, 0);
+    dj.assign((size_t)2 * n_tiles * D.n_rx, 0);     // dj, then the per-(tile, element) window lengths
     int window = 8;
     for (int t = 0; t < n_tiles; ++t) {
         const std::vector<Seg> segs = tile_segments(D, t);
@@ -101,15 +101,19 @@ inline int ring_plan_aperture(const RingApertureDesc &D, double pitch, double c,
             }
             const int d = (int)std::floor(h_min) - 2;
             dj[(size_t)t * D.n_rx + j] = d;
+            int need = 8;
             for (const Seg &s : segs) {
                 double lo, hi;
                 h_range(G, s, j, lo, hi);
                 for (int k = 0; k < D.n_tx; ++k) {
                     // upm = U0_k(z_r) - floor(U0_k(z_iz0)) - 0.5 + H - dj; the entry index is rint(upm)
                     const double top = G.u0(k, G.z(s.r1)) - std::floor(G.u0(k, G.z(iz0))) - 0.5 + hi - d;
-                    window = std::max(window, (int)std::floor(top + 0.5) + 4);
+                    need = std::max(need, (int)std::floor(top + 0.5) + 4);
                 }
             }
+            need = (need + 7) / 8 * 8;
+            dj[(size_t)(n_tiles + t) * D.n_rx + j] = need;
+            window = std::max(window, need);
         }
     }
     return window;
@@ -180,6 +184,7 @@ inline int ring_launch(const RingConfig &cfg, const RingTables &tab0, const Ring
     const RingTables *tabs[2] = {&tab0, &tab1};
     for (int a = 0; a < 2; ++a) {
         L.ap[a].dj = tabs[a]->d_dj;
+        L.ap[a].wj = tabs[a]->d_dj ? tabs[a]->d_dj + (size_t)tabs[a]->n_tiles * L.ap[a].n_rx : nullptr;
         L.ap[a].n_tiles = L.ap[a].n_tx > 0 ? tabs[a]->n_tiles : 0;
     }
     L.window = cfg.window;

@@ -84,16 +84,18 @@ int main() {
     printf("pipe ops/clk/SM (@1965MHz): FFMA(acc,a,b imm-like) %.1f | FHFMA acc %.1f | FFMA 3reg %.1f | sincos(2 MUFU+..)/thread-op %.1f | F2F roundtrip %.1f | FHFMA 3-operand %.1f\n",
            run_pipe<0>(sms, sink), run_pipe<1>(sms, sink), run_pipe<2>(sms, sink), run_pipe<3>(sms, sink), run_pipe<4>(sms, sink), run_pipe<5>(sms, sink));
     CK(cudaGetLastError());
-    const double steps[] = {0.0, 0.25, 0.5, 0.6, 0.75, 1.0, 1.5, 2.0};
-    const int strides[] = {4, 8, 12, 16, 48, 112, 144, 80, 128, 64};
+    const double steps[] = {0.0, 0.25, 0.3, 0.4, 0.45, 0.5, 0.6, 0.75, 1.0, 1.5, 2.0};
+    const double offs[] = {0.0, 0.35, 0.7};
+    const int strides[] = {8, 16, 144, 64, 128};
     for (int stride : strides) {
-        for (double s : steps) {
+        for (double s : steps) for (double off : offs) {
+            if (off != 0.0 && (s == 0.0 || s >= 1.0)) continue;
             std::vector<int> pat(32);
-            for (int l = 0; l < 32; ++l) pat[l] = (int)(l * s);
+            for (int l = 0; l < 32; ++l) pat[l] = (int)(l * s + off);
             double c4 = (stride % 4 == 0) ? run_lds<4>(pat, stride, sink, d_pat, d_cyc) : 0;
             double c8 = (stride % 8 == 0) ? run_lds<8>(pat, stride, sink, d_pat, d_cyc) : 0;
             double c16 = (stride % 16 == 0) ? run_lds<16>(pat, stride, sink, d_pat, d_cyc) : 0;
-            printf("stride %3d B step %.2f entries/lane: cycles per warp-LDS  .32: %.2f  .64: %.2f  .128: %.2f\n", stride, s, c4, c8, c16);
+            printf("stride %3d B step %.2f offset %.2f entries/lane: cycles per warp-LDS  .32: %.2f  .64: %.2f  .128: %.2f\n", stride, s, off, c4, c8, c16);
         }
     }
     CK(cudaGetLastError());
