@@ -93,6 +93,7 @@ struct ulm_rca_plan {
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
     bool d32 = false;             // full (fp32) difference term in the scratch
+    bool quad = false;            // fs = 4 fc exactly, default 17 taps, mixer = (-j)^(n + q0): real-arithmetic pre-pass
     bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
@@ -197,6 +198,17 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
     P.half_band = true;
     for (int t = 0; t <= 2 * L; ++t)
         if (t != L && ((t - L) & 1) == 0 && D.gd[t] != 0.f) P.half_band = false;
+    // quadrature sampling: fs = 4 fc exactly and fc t_start a multiple of 1/4 cycle
+    const double q4 = 4.0 * P.fc * P.t_start;
+    P.quad = P.half_band && L == 8 && P.fs == 4.0 * P.fc && std::fabs(q4 - std::round(q4)) < 1e-9 && std::fabs(q4) < 1e9;
+    if (P.quad) {
+        D.q0 = (int)(((long long)std::llround(q4) % 4 + 4) % 4);
+        for (int t = 0; t <= 2 * L; ++t) {
+            const int m = t - L;
+            const int m4 = ((m % 4) + 4) % 4;
+            D.qd[t] = (m == 0) ? (float)(h[t] / sum) : (m4 == 1 ? (float)(h[t] / sum) : m4 == 3 ? (float)(-h[t] / sum) : 0.f);
+        }
+    }
     return ULM_RCA_OK;
 }
 
@@ -283,6 +295,10 @@ template <int F, bool D32>
 cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, unsigned blocks, cudaStream_t st) {
     const int L = P.half_len;
     if (P.input_kind == 1) return launch_demod_t<1, false, true, F, D32>(D, 0, blocks, st);
+    if (P.quad) {
+        ulm::demod_quad_kernel<F, D32><<<blocks, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
+        return cudaSuccess;
+    }
     if (L == 8) return P.half_band ? launch_demod_t<17, true, false, F, D32>(D, L, blocks, st)
                                    : launch_demod_t<17, false, false, F, D32>(D, L, blocks, st);
     if (L == 16) return launch_demod_t<33, false, false, F, D32>(D, L, blocks, st);
@@ -415,7 +431,14 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
             const double n = (double)P.mix_n0 + i;
             double cyc = P.fc * P.t_start + (P.fc / P.fs) * n;     // fc * t_n in cycles
             cyc -= std::floor(cyc);
-            mix[i] = make_float2((float)std::cos(2 * M_PI * cyc), (float)(-std::sin(2 * M_PI * cyc)));
+            const double c4 = 4.0 * cyc;
+            if (std::fabs(c4 - std::round(c4)) < 1e-12) {       // exact quarter cycles: no 6e-17 residue
+                const float tab[4][2] = {{1.f, 0.f}, {0.f, -1.f}, {-1.f, 0.f}, {0.f, 1.f}};
+                const int q = (int)std::llround(c4) & 3;
+                mix[i] = make_float2(tab[q][0], tab[q][1]);
+            } else {
+                mix[i] = make_float2((float)std::cos(2 * M_PI * cyc), (float)(-std::sin(2 * M_PI * cyc)));
+            }
         }
         CUDA_TRY(P.mixer.upload(mix));
     }

@@ -40,6 +40,8 @@ __host__ __device__ constexpr int entry_bytes(int F, bool D32) { return D32 ? 16
 struct DemodConst {
     int half_len;            // L
     float gd[kMaxTaps];      // dense taps: gd[t] = 2 h[t - L], t = 0..2L   ({1} for IQ input)
+    float qd[17];            // quadrature path (fs = 4 fc, L = 8): qd[8] = h[0], qd[t] = h[m] j^(m-1) for odd m = t - 8
+    int q0;                  // quadrature path: mixer[n] = (-j)^(n + q0)
 };
 
 struct DemodParams {
@@ -127,24 +129,38 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
     const int base = P.n_lo + chunk * kDemodChunk;   // absolute sample of this chunk's first iq value
 
-    // (1) mixed samples
-    for (int idx = threadIdx.x; idx < F * XW; idx += 256) {
-        const int f = idx / XW, i = idx - f * XW;
-        const int n = base - L + i;
-        const int fr = g * F + f;
-        float2 v = make_float2(0.f, 0.f);
-        if (fr < P.n_frames && n >= 0 && n < P.n_samples) {
-            const long long rec = (((long long)fr * P.n_events + e) * P.channels_per_event + ch) * (long long)P.n_samples;
-            if (IQ_INPUT) {
-                const short2 q = reinterpret_cast<const short2 *>(P.rf)[rec + n];
-                v = make_float2((float)q.x, (float)q.y);
-            } else {
-                const float r = (float)P.rf[rec + n];
-                const float2 m = __ldg(P.mixer + (n - P.mix_n0));
-                v = make_float2(r * m.x, r * m.y);
+    // (1) mixed samples: half h of the CTA takes frames [h F/2, (h+1) F/2), a thread takes samples i0, i0 + 128, ...;
+    // all global loads of a sample column are issued before the first shared-memory store
+    {
+        constexpr int FH = F / 2;
+        const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
+        const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
+        const int fr0 = g * F + h * FH;
+        const long long rec0 = ((long long)fr0 * P.n_events + e) * P.channels_per_event * (long long)P.n_samples +
+                               (long long)ch * P.n_samples;
+        for (int i = i0; i < XW; i += 128) {
+            const int n = base - L + i;
+            const bool inb = n >= 0 && n < P.n_samples;
+            float2 *dst = s_x + (h * FH) * XS + i;
+            float re[FH], im[FH];
+#pragma unroll
+            for (int f = 0; f < FH; ++f) {
+                re[f] = im[f] = 0.f;
+                if (inb && fr0 + f < P.n_frames) {
+                    if (IQ_INPUT) {
+                        const short2 q = __ldg(reinterpret_cast<const short2 *>(P.rf) + rec0 + f * frame_stride + n);
+                        re[f] = (float)q.x; im[f] = (float)q.y;
+                    } else {
+                        re[f] = (float)__ldg(P.rf + rec0 + f * frame_stride + n);
+                    }
+                }
             }
+            float2 m = make_float2(1.f, 0.f);
+            if (!IQ_INPUT && inb) m = __ldg(P.mixer + (n - P.mix_n0));
+#pragma unroll
+            for (int f = 0; f < FH; ++f)
+                dst[f * XS] = IQ_INPUT ? make_float2(re[f], im[f]) : make_float2(re[f] * m.x, re[f] * m.y);
         }
-        s_x[f * XS + i] = v;
     }
     __syncthreads();
 
@@ -202,6 +218,142 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
         }
     }
     // (3) one bulk store of the block: generic-proxy writes -> async proxy, then TMA shared -> global
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned char *dst = P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB;
+        const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_out);
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"((uint32_t)(n_ent * EB))
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Quadrature-sampled variant of the pre-pass (RF input, fs = 4 fc exactly, default 17-tap filter): the mixer
+// is (-j)^(n + q0), so  iq[n] = (-j)^(n + q0) (A + j B)  with the REAL filters  A = g[0] rf[n],
+// B = sum_{m odd} g[m] j^(m-1) rf[n-m]  (the even taps of the half-band filter are exactly zero): 9 real FMAs
+// per output instead of 34 complex ones, and the rotation is a compile-time swap/negation.  The taps are
+// stored halved (qd = g/2) so that mid = a' + b' and d/16 = (b' - a')/8 need no further scaling.
+// Same CTA decomposition, shared-memory image and TMA store as demod_kernel.
+// ---------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int demod_quad_xs() { return 225; }    // >= 1.5 * 145 + 4, = 1 mod 32 (words)
+__host__ __device__ inline int demod_quad_smem_bytes(int F, bool D32) {
+    return (kDemodChunk * entry_bytes(F, D32) + 127) / 128 * 128 + F * demod_quad_xs() * 4;
+}
+
+// rotation by (-j)^p of A + jB
+__device__ __forceinline__ float2 quad_rot(int p, float A, float B) {
+    switch (p & 3) {
+        case 0: return make_float2(A, B);
+        case 1: return make_float2(B, -A);
+        case 2: return make_float2(-A, -B);
+        default: return make_float2(-B, A);
+    }
+}
+
+template <int PB, int F, bool D32>
+__device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float (&B)[9], int r0, int n_ent, int base,
+                                                int n_samples, int f, unsigned char *s_out) {
+    constexpr int EB = entry_bytes(F, D32);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const int ent = r0 + q;
+        if (ent >= n_ent) break;
+        const int n = base + ent;
+        const bool ok = n >= 0 && n + 1 <= n_samples - 1;      // edge rule: both taps inside the record
+        const float2 a = quad_rot(PB + q, A[q], B[q]), b = quad_rot(PB + q + 1, A[q + 1], B[q + 1]);   // halved iq[n], iq[n+1]
+        const float mr = ok ? a.x + b.x : 0.f, mi = ok ? a.y + b.y : 0.f;
+        const float dr = ok ? b.x - a.x : 0.f, di = ok ? b.y - a.y : 0.f;                              // = (d)/2
+        unsigned char *ep = s_out + ent * EB;
+        reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
+        if (D32) {
+            reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(2.f * dr, 2.f * di);
+            if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
+        } else {
+            reinterpret_cast<uint32_t *>(ep + 8 * F)[f] = pack_h2(2.f * kDScale * dr, 2.f * kDScale * di);
+        }
+    }
+}
+
+template <int F, bool D32>
+__global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
+    extern __shared__ __align__(128) unsigned char s_raw[];
+    constexpr int EB = entry_bytes(F, D32);
+    constexpr int OUT_BYTES = (kDemodChunk * EB + 127) / 128 * 128;
+    constexpr int L = 8, XW = kDemodChunk + 2 + 2 * L, XS = demod_quad_xs();
+    constexpr int TPG = demod_threads_per_group(F), FH = F / 2;
+    unsigned char *s_out = s_raw;
+    float *s_x = reinterpret_cast<float *>(s_raw + OUT_BYTES);      // [F][XS], sample i at i + 4 (i >> 3)
+
+    const int chunk = blockIdx.x % P.chunks_per_row;
+    const long long row = blockIdx.x / P.chunks_per_row;
+    const int j = (int)(row % P.n_rx_max);
+    const long long ge = row / P.n_rx_max;
+    const int e = (int)(ge % P.n_events);
+    const int g = (int)(ge / P.n_events);
+    const int row_tx = e < P.n_row_tx;
+    const int n_rx = row_tx ? P.n_cols : P.n_rows;
+    if (j >= n_rx) return;
+    const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
+    const int base = P.n_lo + chunk * kDemodChunk;
+
+    // (1) raw samples as float: half h of the CTA takes frames [h FH, (h+1) FH), a thread takes samples i0, i0 + 128
+    {
+        const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
+        const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
+        const int fr0 = g * F + h * FH;
+        const int16_t *rec = P.rf + ((long long)fr0 * P.n_events + e) * P.channels_per_event * (long long)P.n_samples +
+                             (long long)ch * P.n_samples;
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            const int i = i0 + rep * 128;
+            if (i < XW) {
+                const int n = base - L + i;
+                const bool inb = n >= 0 && n < P.n_samples;
+                float *dst = s_x + (h * FH) * XS + i + 4 * (i >> 3);
+                // unconditional loads from clamped addresses, all issued before the first use (out-of-range
+                // samples and frames are zeroed afterwards)
+                const int16_t *src = rec + min(max(n, 0), P.n_samples - 1);
+                const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // >= 0: the group has at least one frame
+                int raw[FH];
+#pragma unroll
+                for (int f = 0; f < FH; ++f) raw[f] = __ldg(src + min(f, f_last) * frame_stride);
+#pragma unroll
+                for (int f = 0; f < FH; ++f) dst[f * XS] = (inb && f <= f_last) ? (float)raw[f] : 0.f;
+            }
+        }
+    }
+    __syncthreads();
+
+    // (2) real FIRs A, B for 9 consecutive outputs, rotation, mid / d into the output image
+    const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
+    const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
+    if (f < F && grp * 8 < n_ent) {
+        const int r0 = grp * 8;
+        const float *x = s_x + f * XS + r0 + (r0 >> 1);         // r0 + 4 (r0 >> 3)
+        float A[9], B[9];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) B[q] = 0.f;
+#pragma unroll
+        for (int u = 0; u < 9 + 2 * L; ++u) {
+            const float xv = x[u + 4 * (u >> 3)];
+#pragma unroll
+            for (int q = 0; q < 9; ++q) {
+                const int t = q - u + 2 * L;                    // tap m = t - L
+                if (t == L) A[q] = c_demod[0].qd[L] * xv;
+                else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(c_demod[0].qd[t], xv, B[q]);
+            }
+        }
+        const int pb = (base + r0 + c_demod[0].q0) & 3;          // (-j)^(n + q0) at the first output
+        switch (pb) {
+            case 0: demod_quad_emit<0, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
+            case 1: demod_quad_emit<1, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
+            case 2: demod_quad_emit<2, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
+            default: demod_quad_emit<3, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
+        }
+    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
     if (threadIdx.x == 0) {
