@@ -209,7 +209,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
 # capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {}
+TRAFFIC_BYTES = {2: 13.515100e9 + 0.143943e9}     # profiles/r01_v2_ncu.md
 
 
 def run_reference(args):

@@ -142,18 +142,25 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             const int n = base - L + i;
             const bool inb = n >= 0 && n < P.n_samples;
             float2 *dst = s_x + (h * FH) * XS + i;
+            // unconditional loads from clamped addresses, all issued before the first use
+            const long long src = rec0 + min(max(n, 0), P.n_samples - 1);
+            const int f_last = min(FH - 1, P.n_frames - 1 - fr0);
             float re[FH], im[FH];
+            if (IQ_INPUT) {
+                short2 q[FH];
 #pragma unroll
-            for (int f = 0; f < FH; ++f) {
-                re[f] = im[f] = 0.f;
-                if (inb && fr0 + f < P.n_frames) {
-                    if (IQ_INPUT) {
-                        const short2 q = __ldg(reinterpret_cast<const short2 *>(P.rf) + rec0 + f * frame_stride + n);
-                        re[f] = (float)q.x; im[f] = (float)q.y;
-                    } else {
-                        re[f] = (float)__ldg(P.rf + rec0 + f * frame_stride + n);
-                    }
+                for (int f = 0; f < FH; ++f) q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src + min(f, f_last) * frame_stride);
+#pragma unroll
+                for (int f = 0; f < FH; ++f) {
+                    const bool ok = inb && f <= f_last;
+                    re[f] = ok ? (float)q[f].x : 0.f; im[f] = ok ? (float)q[f].y : 0.f;
                 }
+            } else {
+                int q[FH];
+#pragma unroll
+                for (int f = 0; f < FH; ++f) q[f] = __ldg(P.rf + src + min(f, f_last) * frame_stride);
+#pragma unroll
+                for (int f = 0; f < FH; ++f) { re[f] = (inb && f <= f_last) ? (float)q[f] : 0.f; im[f] = 0.f; }
             }
             float2 m = make_float2(1.f, 0.f);
             if (!IQ_INPUT && inb) m = __ldg(P.mixer + (n - P.mix_n0));
