@@ -131,7 +131,10 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
 
 /* Host convenience (this is the end-to-end call bench.py times as "e2e"): copies n_frames of HOST
  * channel data to an internal device buffer, beamforms, copies the images back to HOST memory and
- * synchronises.  Allocates device staging on first use (freed by plan_destroy). */
+ * synchronises.  The work is cut into up to 8 chunks of whole 12-frame groups and pipelined on two internal
+ * streams (upload of chunk i+1 overlaps the kernels and the download of chunk i); pass pinned host memory
+ * for the overlap to take place.  Allocates device staging and the streams on first use (freed by
+ * plan_destroy).  One call in flight per plan. */
 ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, int32_t n_frames,
                                      void *h_out);
 

@@ -101,6 +101,9 @@ struct ulm_rca_plan {
     // host-convenience staging
     DeviceBuf h_stage_in, h_stage_out;
     size_t h_stage_frames = 0;
+    cudaStream_t h_copy = nullptr, h_compute = nullptr;     // created on the first host call
+    static constexpr int kHostChunks = 8;
+    cudaEvent_t h_in_done[kHostChunks] = {};
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -109,6 +112,9 @@ struct ulm_rca_plan {
     mutable long long n_calls = 0;
     ~ulm_rca_plan() {
         for (auto &c : ev) for (auto &b : c) for (auto &e : b) if (e) cudaEventDestroy(e);
+        for (auto &e : h_in_done) if (e) cudaEventDestroy(e);
+        if (h_copy) cudaStreamDestroy(h_copy);
+        if (h_compute) cudaStreamDestroy(h_compute);
     }
 };
 
@@ -632,11 +638,32 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
         CUDA_TRY(cudaMalloc(&plan->h_stage_out.p, out_bytes * n_frames));
         plan->h_stage_frames = n_frames;
     }
-    cudaStream_t st = nullptr;
-    CUDA_TRY(cudaMemcpyAsync(plan->h_stage_in.p, h_channel, ch_bytes * n_frames, cudaMemcpyHostToDevice, st));
-    if (ulm_rca_status s = ulm_rca_beamform(plan, plan->h_stage_in.p, n_frames, plan->h_stage_out.p, st)) return s;
-    CUDA_TRY(cudaMemcpyAsync(h_out, plan->h_stage_out.p, out_bytes * n_frames, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+    if (!plan->h_copy) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&plan->h_copy, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&plan->h_compute, cudaStreamNonBlocking));
+        for (auto &e : plan->h_in_done) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    // pipeline over chunks of frames (whole frame groups of 12): the upload of chunk i + 1 overlaps the kernels
+    // and the download of chunk i (the host buffers should be pinned for the copies to be asynchronous)
+    int chunk = (n_frames + ulm_rca_plan::kHostChunks - 1) / ulm_rca_plan::kHostChunks;
+    chunk = std::max(12, (chunk + 11) / 12 * 12);
+    const char *h_in = static_cast<const char *>(h_channel);
+    char *h_o = static_cast<char *>(h_out);
+    char *d_in = plan->h_stage_in.as<char>(), *d_o = plan->h_stage_out.as<char>();
+    int i = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += chunk, ++i) {
+        const int nb = std::min(chunk, n_frames - f0);
+        CUDA_TRY(cudaMemcpyAsync(d_in + (size_t)f0 * ch_bytes, h_in + (size_t)f0 * ch_bytes, ch_bytes * nb,
+                                 cudaMemcpyHostToDevice, plan->h_copy));
+        CUDA_TRY(cudaEventRecord(plan->h_in_done[i], plan->h_copy));
+        CUDA_TRY(cudaStreamWaitEvent(plan->h_compute, plan->h_in_done[i], 0));
+        if (ulm_rca_status s = ulm_rca_beamform(plan, d_in + (size_t)f0 * ch_bytes, nb, d_o + (size_t)f0 * out_bytes,
+                                                plan->h_compute))
+            return s;
+        CUDA_TRY(cudaMemcpyAsync(h_o + (size_t)f0 * out_bytes, d_o + (size_t)f0 * out_bytes, out_bytes * nb,
+                                 cudaMemcpyDeviceToHost, plan->h_compute));
+    }
+    CUDA_TRY(cudaStreamSynchronize(plan->h_compute));
     return ULM_RCA_OK;
 }
 
