@@ -212,6 +212,51 @@ def run_ours(args):
 TRAFFIC_BYTES = {2: 13.515100e9 + 0.143943e9}     # profiles/r01_v2_ncu.md
 
 
+def run_volume(args):
+    """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
+    180 x 180 x 164 volume by das_generic_kernel; reported as volumes/s next to the projection path's frames/s."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(4)
+    host = synth.render(cfg)
+    ch = torch.from_numpy(host).cuda()
+    gathers = cfg.gather_samples_per_frame()
+    with Plan(**rounded_kwargs(cfg), build_volume=True, max_frames=1) as plan:
+        out = plan.beamform_volume(ch)
+        for _ in range(max(args.warmup, 3)):
+            plan.beamform_volume(ch, out=out)
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(args.steps):
+            plan.beamform_volume(ch, out=out)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        # the projection path on the same frame, for the speed ratio
+        proj = plan.beamform(ch)
+        torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(args.steps):
+            plan.beamform(ch, out=proj)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms_proj = ev0.elapsed_time(ev1) / args.steps
+    achieved = FLOP_PER_GATHER * gathers / (ms * 1e-3) / 1e12
+    print(json.dumps({
+        "metric": "full-3D DAS volumes/s (config 4, conventional comparator)", "value": 1e3 / ms, "unit": "volumes/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic: config 1 frame rendered by synth/",
+        "config": {"workload": "BASELINE.json configs[4]: 180x180x164 voxels, 11+11 angles, 128+128 RCA, 1 frame"},
+        "gather_samples_per_s": gathers / (ms * 1e-3),
+        "projection_path_ms_same_frame": ms_proj, "volume_over_projection_time": ms / ms_proj,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None, "kernel": "das_generic_kernel<4,0,0>"},
+        "gpu_launches": 3 * args.steps}))
+
+
 def run_reference(args):
     """Reference arm of this tier: the fp64 oracle, as it stands, on the host cores (rank 0 only).
     Each step beamforms `ref_frames` frames of the same workload (a bounded sample of the ensemble)."""
@@ -254,7 +299,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, choices=[2, 3])
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-frames", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -267,6 +312,8 @@ def main():
             sys.stderr.write("bench.py: --gpus %d needs torchrun with --nproc-per-node %d; running 1 GPU\n" % (args.gpus, args.gpus))
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == 4:
+        run_volume(args)
     else:
         run_ours(args)
 
