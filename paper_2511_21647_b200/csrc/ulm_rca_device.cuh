@@ -411,12 +411,14 @@ __device__ __forceinline__ Alpha make_alpha(float al) {
 }
 
 // four frames of a compact entry: m0, m1 = mid of frames (0,1), (2,3); dd = d/16 of the four frames as half2
+// (nv = number of valid frames among the four: a constant 4 in the ring kernel)
 __device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A, float c,
-                                          float s, float *accr, float *acci) {
+                                          float s, float *accr, float *acci, int nv = 4) {
     const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
     const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
+        if (i >= nv) break;
         unsigned short dr, di;
         split_h2(ds[i], dr, di);
         const float vr = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[2 * i])));
@@ -429,10 +431,12 @@ __device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, cons
 // interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
 // v = mid + a' d  (compact: two FHFMA per component, d in fp16; full: one FFMA),  acc += (c + j s) v
 template <int F, bool D32, class LoadVec>
-__device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, float s, float *accr, float *acci) {
+__device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, float s, float *accr, float *acci,
+                                          int nv = F) {
     if (D32) {
 #pragma unroll
         for (int q = 0; q < F / 2; ++q) {
+            if (2 * q >= nv) break;
             const uint4 m = ld(q), d = ld(F / 2 + q);
             const float mv[4] = {__uint_as_float(m.x), __uint_as_float(m.y), __uint_as_float(m.z), __uint_as_float(m.w)};
             const float dv[4] = {__uint_as_float(d.x), __uint_as_float(d.y), __uint_as_float(d.z), __uint_as_float(d.w)};
@@ -446,7 +450,10 @@ __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, f
         }
     } else {
 #pragma unroll
-        for (int q = 0; q < F / 4; ++q) chunk_mac(ld(2 * q), ld(2 * q + 1), ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q);
+        for (int q = 0; q < F / 4; ++q) {
+            if (4 * q >= nv) break;
+            chunk_mac(ld(2 * q), ld(2 * q + 1), ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
+        }
     }
 }
 
@@ -460,7 +467,7 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
     const int npix = P.n_lat * P.n_ax;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npix) return;
-    const int iz = p % P.n_ax, il = p / P.n_ax;
+    const int il = p % P.n_lat, iz = p / P.n_lat;     // lanes = lateral neighbours: their entries are adjacent in the scratch
     const int g = blockIdx.y;
     const int n_kgroups = P.per_angle ? P.n_tx : 1;
     const int plane = blockIdx.z / n_kgroups;
@@ -473,6 +480,7 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
 #pragma unroll
     for (int f = 0; f < F; ++f) accr[f] = acci[f] = 0.f;
     const int tab0 = (plane * P.n_tx) * P.n_ax + iz;
+    const int nv = min(F, P.n_frames - g * F);          // valid frames of this group (block-uniform)
     const size_t grow = (size_t)g * P.n_events * P.n_rx_max;
 
     for (int j = 0; j < P.n_rx; ++j) {
@@ -500,7 +508,7 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             if (APOD) { s *= w; c *= w; }
             const uint4 *ent = reinterpret_cast<const uint4 *>(
                 P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32));
-            entry_mac<F, D32>([&](int i) { return __ldg(ent + i); }, make_alpha(al), c, s, accr, acci);
+            entry_mac<F, D32>([&](int i) { return __ldg(ent + i); }, make_alpha(al), c, s, accr, acci, nv);
         }
     }
     const long long o = P.out_base + (long long)il * P.s_lat + (long long)plane * P.s_plane +
