@@ -12,6 +12,14 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
+def pytest_collection_modifyitems(config, items):
+    # a wedged kernel must not hang the run: GPU tests are killed (thread method: the main thread may be blocked
+    # inside a CUDA call) after 10 minutes each
+    for item in items:
+        if "gpu" in item.keywords:
+            item.add_marker(pytest.mark.timeout(600, method="thread"))
+
+
 @pytest.fixture(scope="session")
 def oracle_mod():
     import oracle
