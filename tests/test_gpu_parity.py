@@ -282,3 +282,30 @@ def test_ensemble_full_size_sampled(torch_cuda, index):
         worst = max(worst, e)
         assert e <= TOL, "cfg %d frame %d: %.3e" % (index, fr, e)
     print("PARITY cfg%d full size worst %.3e over frames %s" % (index, worst, check))
+
+
+def test_fallback_to_generic_kernel_when_the_ring_does_not_cover_the_shape(torch_cuda):
+    """More than 256 receive elements per aperture: kernel = auto must fall back to the generic gather kernel
+    (and kernel = 2 must refuse), results still within tolerance."""
+    from paper_2511_21647_b200 import Plan, UlmRcaError
+    d = synth.LAMBDA_M / 2
+    cfg = small(n_rows=6, n_cols=260, pitch=0.1e-3, n_frames=2, row_tx_angles=tuple(np.radians([-3.0, 2.0])),
+                col_tx_angles=tuple(np.radians([4.0])), t0=(0.1e-6, -0.1e-6, 0.2e-6),
+                grid_xz=centred_grid(21, d, 17, 6e-3, d), grid_yz=centred_grid(9, d, 13, 6e-3, d))
+    ch = synth.random_channel(cfg, 2, seed=3, amplitude=6000)
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch)
+    assert info["kernel"] == 1
+    assert_parity(gpu, ref)
+    with pytest.raises(UlmRcaError) as ei:
+        Plan(**rounded_kwargs(cfg), kernel=2)
+    assert ei.value.status == 4
+
+
+def test_many_frames_cross_group_boundaries(torch_cuda):
+    """25 frames = two full 12-frame groups + 1: every frame, including the lone one of the last group."""
+    cfg = small(n_frames=25)
+    ch = synth.random_channel(cfg, 25, seed=29, amplitude=3000)
+    ch = (ch.astype(np.int32) + synth.random_channel(cfg, 25, seed=30, amplitude=3000)).astype(np.int16)
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=25))
+    assert info["launches_last_call"] == 2
+    assert_parity(gpu, ref)
