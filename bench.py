@@ -198,7 +198,8 @@ def run_ours(args):
                          "whole_step_frac": FLOP_PER_GATHER * gathers / (ms_step * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS},
             "cpu_baseline": cpu, "clocks": clocks,
             "e2e": {"value": world * n_frames / (e2e_ms_step * 1e-3), "unit": "frames/s",
-                    "h2d_bytes_per_step": int(channel.numel() * 2), "d2h_bytes_per_step": int(out.numel() * 8),
+                    "h2d_bytes_per_step": int(info["host_upload_bytes_per_frame"]) * n_frames,
+                    "host_buffer_bytes": int(channel.numel() * 2), "d2h_bytes_per_step": int(out.numel() * 8),
                     "ms_per_step": e2e_ms_step, "steps": e2e_steps},
             "gpu_launches": int(launches),
         }

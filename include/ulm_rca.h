@@ -132,7 +132,8 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
 /* Host convenience (this is the end-to-end call bench.py times as "e2e"): copies n_frames of HOST
  * channel data to an internal device buffer, beamforms, copies the images back to HOST memory and
  * synchronises.  The work is cut into up to 8 chunks of whole 12-frame groups and pipelined on two internal
- * streams (upload of chunk i+1 overlaps the kernels and the download of chunk i); pass pinned host memory
+ * streams (upload of chunk i+1 overlaps the kernels and the download of chunk i); only what the method reads is
+ * uploaded (the receive aperture of every event, the touched sample range); pass pinned host memory
  * for the overlap to take place.  Allocates device staging and the streams on first use (freed by
  * plan_destroy).  One call in flight per plan. */
 ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, int32_t n_frames,
@@ -148,7 +149,7 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [6] window entries per stage (W)  [7] ring stages  [8] tiles per projection (x-z)
  *   [9] dynamic shared memory bytes   [10] kernels launched by the last beamform call
  *   [11] tiles per projection (y-z)   [12] precision in use (1 compact / 2 full)
- *   [13] scratch bytes per (sample, frame) */
+ *   [13] scratch bytes per (sample, frame)   [14] bytes per frame ulm_rca_beamform_host uploads */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this

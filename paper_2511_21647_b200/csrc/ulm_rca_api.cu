@@ -327,6 +327,23 @@ cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_
     return F == 12 ? launch_demod_f<12, false>(P, D, blocks, st) : launch_demod_f<4, false>(P, D, blocks, st);
 }
 
+// sample range [s_lo, s_hi) of a record the pre-pass can read (rounded outwards to 64 samples)
+void host_sample_range(const ulm_rca_plan &P, int &s_lo, int &s_hi) {
+    const int chunks = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
+    s_lo = std::max(0, P.n_lo - P.half_len) / 64 * 64;
+    const long long hi = (long long)P.n_lo + (long long)chunks * ulm::kDemodChunk + P.half_len + 2;
+    s_hi = (int)std::min<long long>(P.n_samples, (std::max<long long>(hi, 0) + 63) / 64 * 64);
+    if (s_hi < s_lo) s_hi = s_lo;
+}
+
+size_t host_upload_bytes_per_frame(const ulm_rca_plan &P) {
+    int s_lo = 0, s_hi = 0;
+    host_sample_range(P, s_lo, s_hi);
+    size_t n = 0;
+    for (int a = 0; a < 2; ++a) n += (size_t)P.ap[a].n_tx * P.ap[a].n_rx;
+    return n * (size_t)(s_hi - s_lo) * (P.input_kind == 1 ? 4 : 2);
+}
+
 }  // namespace
 
 extern "C" {
@@ -497,12 +514,13 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *ch, size_t *
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n) {
     if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
     const bool ring = plan->kernel == 2, d32 = plan->d32;
-    const int64_t vals[14] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
+    const int64_t vals[15] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
                               ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
                               ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
                               ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
-                              ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : 1, ulm::entry_bytes(12, d32) / 12};
-    for (int i = 0; i < n && i < 14; ++i) v[i] = vals[i];
+                              ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : 1, ulm::entry_bytes(12, d32) / 12,
+                              (int64_t)host_upload_bytes_per_frame(*plan)};
+    for (int i = 0; i < n && i < 15; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
 }
 
@@ -650,11 +668,28 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
     const char *h_in = static_cast<const char *>(h_channel);
     char *h_o = static_cast<char *>(h_out);
     char *d_in = plan->h_stage_in.as<char>(), *d_o = plan->h_stage_out.as<char>();
+    const int eb = plan->input_kind == 1 ? 4 : 2;
+    int s_lo = 0, s_hi = 0;
+    host_sample_range(*plan, s_lo, s_hi);
     int i = 0;
     for (int f0 = 0; f0 < n_frames; f0 += chunk, ++i) {
         const int nb = std::min(chunk, n_frames - f0);
-        CUDA_TRY(cudaMemcpyAsync(d_in + (size_t)f0 * ch_bytes, h_in + (size_t)f0 * ch_bytes, ch_bytes * nb,
-                                 cudaMemcpyHostToDevice, plan->h_copy));
+        // upload only what the pre-pass reads: the receive aperture of every event, touched sample range
+        for (int f = f0; f < f0 + nb; ++f)
+            for (int a = 0; a < 2; ++a) {
+                const Aperture &A = plan->ap[a];
+                if (A.n_tx == 0) continue;
+                cudaMemcpy3DParms cp = {};
+                const size_t row_pitch = (size_t)plan->n_samples * eb;
+                cp.srcPtr = make_cudaPitchedPtr(const_cast<char *>(h_in) + (size_t)f * ch_bytes, row_pitch, row_pitch, plan->cpe);
+                cp.dstPtr = make_cudaPitchedPtr(d_in + (size_t)f * ch_bytes, row_pitch, row_pitch, plan->cpe);
+                const size_t c0 = (a == 0 && plan->cpe == plan->n_rows + plan->n_cols) ? plan->n_rows : 0;
+                cp.srcPos = make_cudaPos((size_t)s_lo * eb, c0, A.e0);
+                cp.dstPos = cp.srcPos;
+                cp.extent = make_cudaExtent((size_t)(s_hi - s_lo) * eb, A.n_rx, A.n_tx);
+                cp.kind = cudaMemcpyHostToDevice;
+                CUDA_TRY(cudaMemcpy3DAsync(&cp, plan->h_copy));
+            }
         CUDA_TRY(cudaEventRecord(plan->h_in_done[i], plan->h_copy));
         CUDA_TRY(cudaStreamWaitEvent(plan->h_compute, plan->h_in_done[i], 0));
         if (ulm_rca_status s = ulm_rca_beamform(plan, d_in + (size_t)f0 * ch_bytes, nb, d_o + (size_t)f0 * out_bytes,
