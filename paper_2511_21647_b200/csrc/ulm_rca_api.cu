@@ -287,7 +287,7 @@ void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames
 }
 
 template <int NT, bool HB, bool IQ, int F, bool D32>
-cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, unsigned blocks, cudaStream_t st) {
+cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, dim3 blocks, cudaStream_t st) {
     const size_t smem = (size_t)ulm::demod_smem_bytes(F, D32, L);
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, HB, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -298,7 +298,7 @@ cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, unsigned blocks, cu
 }
 
 template <int F, bool D32>
-cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, unsigned blocks, cudaStream_t st) {
+cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim3 blocks, cudaStream_t st) {
     const int L = P.half_len;
     if (P.input_kind == 1) return launch_demod_t<1, false, true, F, D32>(D, 0, blocks, st);
     if (P.quad) {
@@ -320,8 +320,7 @@ cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_
     D.n_lo = P.n_lo; D.l_row = P.l_row;
     D.chunks_per_row = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
     const int F = group_frames(n_frames);
-    const long long rows = (long long)((n_frames + F - 1) / F) * P.n_events * P.n_rx_max;
-    const unsigned blocks = (unsigned)(rows * D.chunks_per_row);
+    const dim3 blocks((unsigned)D.chunks_per_row, (unsigned)P.n_rx_max, (unsigned)(((n_frames + F - 1) / F) * P.n_events));
     ++P.last_launches;
     if (P.d32) return F == 12 ? launch_demod_f<12, true>(P, D, blocks, st) : launch_demod_f<4, true>(P, D, blocks, st);
     return F == 12 ? launch_demod_f<12, false>(P, D, blocks, st) : launch_demod_f<4, false>(P, D, blocks, st);
@@ -402,6 +401,8 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     P.c = c_mps; P.fs = fs_hz; P.fc = fc_hz; P.t_start = opt->t_start_s; P.f_number = opt->f_number;
     P.input_kind = opt->input_kind; P.cpe = cpe; P.n_samples = opt->n_samples; P.compound = opt->compound;
     P.max_frames = opt->max_frames > 0 ? opt->max_frames : 32;
+    if ((long long)((P.max_frames + 3) / 4) * (n_row_tx + n_col_tx) > 65535)
+        return fail(ULM_RCA_EUNSUPPORTED, "max_frames x events too large for one batch: lower max_frames");
     P.build_volume = opt->build_volume;
     P.n_events = n_row_tx + n_col_tx;
     P.n_rx_max = std::max(P.n_rows, P.n_cols);

@@ -117,12 +117,10 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     unsigned char *s_out = s_raw;              // [127][EB] image of the output block
     float2 *s_x = reinterpret_cast<float2 *>(s_raw + OUT_BYTES);   // [F][XS]
 
-    const int chunk = blockIdx.x % P.chunks_per_row;
-    const long long row = blockIdx.x / P.chunks_per_row;    // (group * n_events + e) * n_rx_max + j
-    const int j = (int)(row % P.n_rx_max);
-    const long long ge = row / P.n_rx_max;
-    const int e = (int)(ge % P.n_events);
-    const int g = (int)(ge / P.n_events);
+    // grid = (chunks per row, n_rx_max, groups * n_events)
+    const int chunk = blockIdx.x, j = blockIdx.y;
+    const int g = blockIdx.z / P.n_events, e = blockIdx.z - g * P.n_events;
+    const long long row = (long long)blockIdx.z * P.n_rx_max + j;     // (group * n_events + e) * n_rx_max + j
     const int row_tx = e < P.n_row_tx;
     const int n_rx = row_tx ? P.n_cols : P.n_rows;
     if (j >= n_rx) return;                      // rows of the shorter aperture stay unused
@@ -294,12 +292,10 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
     unsigned char *s_out = s_raw;
     float *s_x = reinterpret_cast<float *>(s_raw + OUT_BYTES);      // [F][XS], sample i at i + 4 (i >> 3)
 
-    const int chunk = blockIdx.x % P.chunks_per_row;
-    const long long row = blockIdx.x / P.chunks_per_row;
-    const int j = (int)(row % P.n_rx_max);
-    const long long ge = row / P.n_rx_max;
-    const int e = (int)(ge % P.n_events);
-    const int g = (int)(ge / P.n_events);
+    // grid = (chunks per row, n_rx_max, groups * n_events)
+    const int chunk = blockIdx.x, j = blockIdx.y;
+    const int g = blockIdx.z / P.n_events, e = blockIdx.z - g * P.n_events;
+    const long long row = (long long)blockIdx.z * P.n_rx_max + j;     // (group * n_events + e) * n_rx_max + j
     const int row_tx = e < P.n_row_tx;
     const int n_rx = row_tx ? P.n_cols : P.n_rows;
     if (j >= n_rx) return;
