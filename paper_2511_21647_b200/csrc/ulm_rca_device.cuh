@@ -424,6 +424,45 @@ __device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, cons
     }
 }
 
+// packed fp32x2 helpers (sm_100 FFMA2: two fp32 FMAs in one issue slot)
+__device__ __forceinline__ unsigned long long pack_f2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack_f2(unsigned long long v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
+// chunk_mac with the complex multiply-accumulate of two frames at a time in FFMA2: aR / aI hold (frame 2p,
+// frame 2p+1) pairs of the real / imaginary accumulators; CC = (c, c), SS = (s, s), NS = (-s, -s).
+// Bit-identical to chunk_mac (each half is an ordinary round-to-nearest fp32 FMA).
+__device__ __forceinline__ void chunk_mac2(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A,
+                                           unsigned long long CC, unsigned long long SS, unsigned long long NS,
+                                           unsigned long long *aR, unsigned long long *aI) {
+    const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        float vr[2], vi[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            unsigned short dr, di;
+            split_h2(ds[2 * p + i], dr, di);
+            vr[i] = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[4 * p + 2 * i])));
+            vi[i] = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[4 * p + 2 * i + 1])));
+        }
+        const unsigned long long VR = pack_f2(vr[0], vr[1]), VI = pack_f2(vi[0], vi[1]);
+        aR[p] = ffma2(CC, VR, aR[p]); aR[p] = ffma2(NS, VI, aR[p]);
+        aI[p] = ffma2(SS, VR, aI[p]); aI[p] = ffma2(CC, VI, aI[p]);
+    }
+}
+
 // interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
 // v = mid + a' d  (compact: two FHFMA per component, d in fp16; full: one FFMA),  acc += (c + j s) v
 template <int F, bool D32, class LoadVec>

@@ -236,11 +236,20 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
         for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 16u;
 
-        float accr[PX][F], acci[PX][F];
+        // accumulators: full entries as floats, compact entries as (frame 2p, frame 2p+1) pairs for FFMA2
+        float accr[D32 ? PX : 1][D32 ? F : 1], acci[D32 ? PX : 1][D32 ? F : 1];
+        unsigned long long accR2[D32 ? 1 : PX][D32 ? 1 : F / 2], accI2[D32 ? 1 : PX][D32 ? 1 : F / 2];
+        if constexpr (D32) {
 #pragma unroll
-        for (int m = 0; m < PX; ++m)
+            for (int m = 0; m < PX; ++m)
 #pragma unroll
-            for (int f = 0; f < F; ++f) accr[m][f] = acci[m][f] = 0.f;
+                for (int f = 0; f < F; ++f) accr[m][f] = acci[m][f] = 0.f;
+        } else {
+#pragma unroll
+            for (int m = 0; m < PX; ++m)
+#pragma unroll
+                for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
+        }
 
         for (int j = 0; j < n_rx; ++j) {
             float Hs[PX], Rr[PX], Ri[PX];
@@ -286,7 +295,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     x.s = fmaf(Tr, Ri[m], Ti * Rr[m]);
                     return x;
                 };
-                if (D32) {
+                if constexpr (D32) {
 #pragma unroll
                     for (int m = 0; m < PX; ++m) {
                         const PixCtx x = prep(m);
@@ -310,7 +319,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                             b[0] = lds128(a1 + 32u * q1); b[1] = lds128(a1 + 32u * q1 + 16u); b[2] = lds128(a1 + 8u * F + 16u * q1);
                         }
                         const uint4 *b = buf[st & 1];
-                        chunk_mac(b[0], b[1], b[2], cur.A, cur.c, cur.s, accr[m] + 4 * q, acci[m] + 4 * q);
+                        chunk_mac2(b[0], b[1], b[2], cur.A, pack_f2(cur.c, cur.c), pack_f2(cur.s, cur.s),
+                                   pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
                         if (q == NQ - 1) cur = nxt;
                     }
                 }
@@ -329,9 +339,17 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
                 for (int f = 0; f < F; ++f) {
                     const int fr = g * F + f;
+                    float re, im;
+                    if constexpr (D32) {
+                        re = accr[m][f]; im = acci[m][f];
+                    } else {
+                        float r0, r1, i0, i1;
+                        unpack_f2(accR2[m][f / 2], r0, r1);
+                        unpack_f2(accI2[m][f / 2], i0, i1);
+                        re = (f & 1) ? r1 : r0; im = (f & 1) ? i1 : i0;
+                    }
                     if (fr < P.n_frames)
-                        P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] =
-                            make_float2(accr[m][f], acci[m][f]);
+                        P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] = make_float2(re, im);
                 }
             }
         }
