@@ -83,6 +83,20 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
     return r;
 }
 
+// Compact-entry store of one frame's (mid, d/16): frames are paired (2p, 2p+1); the mid section holds
+// [re_2p, re_2p+1, im_2p, im_2p+1] per pair and the d section the half2 words [(dr_2p, dr_2p+1), (di_2p, di_2p+1)],
+// so that the DAS kernels read aligned (frame 2p, frame 2p+1) register pairs for FFMA2.
+template <int F>
+__device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16) {
+    const int p = f >> 1, h = f & 1;
+    float *mid = reinterpret_cast<float *>(ep) + 4 * p + h;
+    mid[0] = mr;
+    mid[2] = mi;
+    unsigned short *d = reinterpret_cast<unsigned short *>(ep + 8 * F) + 4 * p + h;
+    d[0] = f2h_bits(dr16);
+    d[2] = f2h_bits(di16);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Demodulation / staging pre-pass: int16 RF (or IQ) -> scratch entries over the touched
 // sample range only.  One CTA = one chunk of 127 entries of one (frame group, event, rx element) row, all F
@@ -213,12 +227,12 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             const float mr = ok ? 0.5f * (ar[q] + ar[q + 1]) : 0.f, mi = ok ? 0.5f * (ai[q] + ai[q + 1]) : 0.f;
             const float dr = ok ? ar[q + 1] - ar[q] : 0.f, di = ok ? ai[q + 1] - ai[q] : 0.f;
             unsigned char *ep = s_out + ent * EB;
-            reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
             if (D32) {
+                reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
                 reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(dr, di);
                 if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
             } else {
-                reinterpret_cast<uint32_t *>(ep + 8 * F)[f] = pack_h2(kDScale * dr, kDScale * di);
+                store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di);
             }
         }
     }
@@ -272,12 +286,12 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
         const float mr = ok ? a.x + b.x : 0.f, mi = ok ? a.y + b.y : 0.f;
         const float dr = ok ? b.x - a.x : 0.f, di = ok ? b.y - a.y : 0.f;                              // = (d)/2
         unsigned char *ep = s_out + ent * EB;
-        reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
         if (D32) {
+            reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
             reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(2.f * dr, 2.f * di);
             if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
         } else {
-            reinterpret_cast<uint32_t *>(ep + 8 * F)[f] = pack_h2(2.f * kDScale * dr, 2.f * kDScale * di);
+            store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di);
         }
     }
 }
@@ -390,39 +404,19 @@ struct DasParams {
     int n_frames;                    // frames in this batch
 };
 
-// the interpolation weight a' = a - 0.5 of one gather: fp32, and 16 a' split into two fp16 (hi + lo = exact to 2^-24)
+// the interpolation weight a' = a - 0.5 of one gather, fp32: al for full entries, a16 = 16 a' for compact
+// entries (whose difference term is stored / 16)
 struct Alpha {
-    float al;
-    unsigned short hi, lo;
+    float al, a16;
 };
 __device__ __forceinline__ Alpha make_alpha(float al) {
     Alpha a;
     a.al = al;
-    const float a16 = kAlScale * al;
-    a.hi = f2h_bits(a16);
-    float back;
-    asm("cvt.f32.f16 %0, %1;" : "=f"(back) : "h"(a.hi));
-    a.lo = f2h_bits(a16 - back);
+    a.a16 = kAlScale * al;
     return a;
 }
-
-// four frames of a compact entry: m0, m1 = mid of frames (0,1), (2,3); dd = d/16 of the four frames as half2
-// (nv = number of valid frames among the four: a constant 4 in the ring kernel)
-__device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A, float c,
-                                          float s, float *accr, float *acci, int nv = 4) {
-    const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
-    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        if (i >= nv) break;
-        unsigned short dr, di;
-        split_h2(ds[i], dr, di);
-        const float vr = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[2 * i])));
-        const float vi = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[2 * i + 1])));
-        accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
-        acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
-    }
-}
+// fp16 -> fp32 as 1.0h * h + 0 on the FMA pipe (FHFMA runs at the full FP32 rate; HADD2.F32 does not)
+__device__ __forceinline__ float h2f(unsigned short h) { return fhfma((unsigned short)0x3C00, h, 0.f); }
 
 // packed fp32x2 helpers (sm_100 FFMA2: two fp32 FMAs in one issue slot)
 __device__ __forceinline__ unsigned long long pack_f2(float lo, float hi) {
@@ -439,32 +433,51 @@ __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsign
     return d;
 }
 
-// chunk_mac with the complex multiply-accumulate of two frames at a time in FFMA2: aR / aI hold (frame 2p,
-// frame 2p+1) pairs of the real / imaginary accumulators; CC = (c, c), SS = (s, s), NS = (-s, -s).
-// Bit-identical to chunk_mac (each half is an ordinary round-to-nearest fp32 FMA).
-__device__ __forceinline__ void chunk_mac2(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A,
-                                           unsigned long long CC, unsigned long long SS, unsigned long long NS,
-                                           unsigned long long *aR, unsigned long long *aI) {
+// Four frames (two frame pairs) of a compact entry: m0 / m1 = [re_a, re_b, im_a, im_b] of pairs 0 / 1,
+// dd = [(dr, dr), (di, di)] half2 words of pair 0 then pair 1 (difference term / 16).
+// Scalar version (generic kernel): v = mid + a16 * d with d converted to fp32 (the fp16 x fp32 product is exact
+// in the FMA), acc += (c + j s) v.  nv = number of valid frames among the four.
+__device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A, float c,
+                                          float s, float *accr, float *acci, int nv = 4) {
     const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
     const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
 #pragma unroll
-    for (int p = 0; p < 2; ++p) {
-        float vr[2], vi[2];
+    for (int i = 0; i < 4; ++i) {
+        if (i >= nv) break;
+        const int p = i >> 1, h = i & 1;
+        unsigned short r0, r1, i0, i1;
+        split_h2(ds[2 * p], r0, r1);
+        split_h2(ds[2 * p + 1], i0, i1);
+        const float vr = fmaf(A.a16, h2f(h ? r1 : r0), __uint_as_float(mids[4 * p + h]));
+        const float vi = fmaf(A.a16, h2f(h ? i1 : i0), __uint_as_float(mids[4 * p + 2 + h]));
+        accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
+        acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
+    }
+}
+
+// Packed version (ring kernel): the interpolation and the complex multiply-accumulate of a frame pair run as
+// FFMA2 on (frame 2p, frame 2p+1) register pairs; aR / aI are pairs of real / imaginary accumulators;
+// AA = (a16, a16), CC = (c, c), SS = (s, s), NS = (-s, -s).  Each half is an ordinary round-to-nearest fp32 FMA,
+// so the results are bit-identical to chunk_mac.
+__device__ __forceinline__ void chunk_mac2(const uint4 &m0, const uint4 &m1, const uint4 &dd, unsigned long long AA,
+                                           unsigned long long CC, unsigned long long SS, unsigned long long NS,
+                                           unsigned long long *aR, unsigned long long *aI) {
+    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            unsigned short dr, di;
-            split_h2(ds[2 * p + i], dr, di);
-            vr[i] = fhfma(A.lo, dr, fhfma(A.hi, dr, __uint_as_float(mids[4 * p + 2 * i])));
-            vi[i] = fhfma(A.lo, di, fhfma(A.hi, di, __uint_as_float(mids[4 * p + 2 * i + 1])));
-        }
-        const unsigned long long VR = pack_f2(vr[0], vr[1]), VI = pack_f2(vi[0], vi[1]);
+    for (int p = 0; p < 2; ++p) {
+        const uint4 &m = p ? m1 : m0;
+        unsigned short r0, r1, i0, i1;
+        split_h2(ds[2 * p], r0, r1);
+        split_h2(ds[2 * p + 1], i0, i1);
+        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), pack_f2(__uint_as_float(m.x), __uint_as_float(m.y)));
+        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), pack_f2(__uint_as_float(m.z), __uint_as_float(m.w)));
         aR[p] = ffma2(CC, VR, aR[p]); aR[p] = ffma2(NS, VI, aR[p]);
         aI[p] = ffma2(SS, VR, aI[p]); aI[p] = ffma2(CC, VI, aI[p]);
     }
 }
 
 // interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
-// v = mid + a' d  (compact: two FHFMA per component, d in fp16; full: one FFMA),  acc += (c + j s) v
+// v = mid + a' d  (a' in fp32; compact: d converted from fp16),  acc += (c + j s) v
 template <int F, bool D32, class LoadVec>
 __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, float s, float *accr, float *acci,
                                           int nv = F) {

@@ -319,8 +319,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                             b[0] = lds128(a1 + 32u * q1); b[1] = lds128(a1 + 32u * q1 + 16u); b[2] = lds128(a1 + 8u * F + 16u * q1);
                         }
                         const uint4 *b = buf[st & 1];
-                        chunk_mac2(b[0], b[1], b[2], cur.A, pack_f2(cur.c, cur.c), pack_f2(cur.s, cur.s),
-                                   pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
+                        chunk_mac2(b[0], b[1], b[2], pack_f2(cur.A.a16, cur.A.a16), pack_f2(cur.c, cur.c),
+                                   pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
                         if (q == NQ - 1) cur = nxt;
                     }
                 }
