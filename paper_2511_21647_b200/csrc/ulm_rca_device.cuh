@@ -9,13 +9,15 @@
 //   so no fp32 quantity ever carries the full ~1300-sample delay.  floor(u) is taken with the
 //   add-magic-constant trick on (u - 0.5).
 //
-// IQ scratch ("entries"): frames are processed in groups of F (4 or 12).  For frame group g, event e,
-// receive element j and sample n the scratch holds ONE entry of 12 F bytes
-//     [ mid_f = (iq_f[n] + iq_f[n+1]) / 2   as float2, f = 0..F-1 |  d_f = (iq_f[n+1] - iq_f[n]) / 16  as half2, f = 0..F-1 ]
+// IQ scratch ("entries"): frames are processed in groups of F (4 or 12) and paired (2p, 2p+1).  For frame group g,
+// event e, receive element j and sample n the scratch holds ONE compact entry of 12 F bytes:
+//     mid section, 16 B per frame pair:  [re_2p, re_2p+1, im_2p, im_2p+1]  of  mid = (iq[n] + iq[n+1]) / 2   (fp32)
+//     d section,    8 B per frame pair:  half2 (dr_2p, dr_2p+1), half2 (di_2p, di_2p+1)  of  d/16 = (iq[n+1] - iq[n]) / 16
 // so that the interpolated sample is mid + a' d with a' = a - 0.5 in [-0.5, 0.5]: the value carries fp32
-// precision, only the small difference term is fp16 (with a' also rounded to fp16: one FHFMA
-// `fma.rn.f32.f16` per component, no conversion instruction).  Entry sizes 48 B / 144 B are odd multiples
-// of 16 B, which makes the LDS.128 gathers of neighbouring entries bank-conflict free.
+// precision, only the small difference term is fp16, and one LDS.128 delivers aligned (frame 2p, frame 2p+1)
+// register pairs for the packed fp32x2 FMA (FFMA2).  "Full" entries keep d in fp32 (16 F + 16 bytes).  Entry
+// sizes 48 / 144 / 80 / 208 B are odd multiples of 16 B, which keeps the LDS.128 gathers of neighbouring
+// entries free of bank conflicts.
 #pragma once
 
 #include <cuda_fp16.h>
