@@ -502,7 +502,9 @@ __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, f
 #pragma unroll
         for (int q = 0; q < F / 4; ++q) {
             if (4 * q >= nv) break;
-            chunk_mac(ld(2 * q), ld(2 * q + 1), ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
+            // the second frame pair of the chunk is not even loaded when the group has no valid frame in it
+            const uint4 m1 = nv - 4 * q > 2 ? ld(2 * q + 1) : make_uint4(0u, 0u, 0u, 0u);
+            chunk_mac(ld(2 * q), m1, ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
         }
     }
 }
