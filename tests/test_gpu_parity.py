@@ -309,3 +309,38 @@ def test_many_frames_cross_group_boundaries(torch_cuda):
     gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=25))
     assert info["launches_last_call"] == 2
     assert_parity(gpu, ref)
+
+
+SWEEP = [
+    # n_rows, n_cols, n_lat_xz, n_ax_xz, n_lat_yz, n_ax_yz, n_row_tx, n_col_tx, frames, dz scale, f_number
+    (9, 40, 5, 3, 7, 4, 1, 2, 1, 1.0, 0.0),
+    (33, 17, 97, 50, 61, 37, 2, 1, 5, 0.7, 0.0),
+    (16, 48, 200, 9, 150, 21, 3, 2, 13, 1.3, 1.2),
+    (40, 40, 31, 130, 31, 130, 5, 5, 4, 0.5, 0.0),
+    (12, 64, 385, 4, 383, 5, 2, 2, 3, 1.0, 2.0),
+]
+
+
+@pytest.mark.parametrize("shape", SWEEP)
+def test_shape_sweep_ring_kernel(torch_cuda, shape):
+    """Odd shapes through the ring kernel: fewer positions than one tile, one-row images, tiles that span many
+    strips, wide images, many frames, f-number masks -- window planning and the ragged tails."""
+    n_rows, n_cols, nlx, nax, nly, nay, kr, kc, nf, dzs, fnum = shape
+    d = synth.LAMBDA_M / 2
+    rng = np.random.default_rng(sum(shape[:9]))
+    cfg = synth.config(0).with_(
+        n_rows=n_rows, n_cols=n_cols, pitch=0.25e-3, n_samples=900,
+        row_tx_angles=tuple(np.radians(rng.uniform(-9, 9, kr))), col_tx_angles=tuple(np.radians(rng.uniform(-9, 9, kc))),
+        grid_xz=centred_grid(nlx, 0.6 * d, nax, 5e-3, dzs * d, ref=0.2e-3),
+        grid_yz=centred_grid(nly, 0.5 * d, nay, 5.5e-3, dzs * d, ref=-0.1e-3),
+        n_frames=nf, t_start=0.4e-6, t0=tuple(rng.uniform(-0.2e-6, 0.2e-6, kr + kc)), f_number=fnum)
+    ch = synth.random_channel(cfg, nf, seed=int(rng.integers(1 << 30)), amplitude=4000)
+    # full entries: nothing but fp32 rounding, so a planning / indexing mistake anywhere shows up at once
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=nf, precision=2))
+    assert info["kernel"] == 2 and info["precision"] == 2
+    assert_parity(gpu, ref, tol=2e-5)
+    # compact entries on the same noise-only data (no coherent maximum, as few as 40 terms per pixel): the fp16
+    # difference term bounds the error per term by 2^-13 |d| (DESIGN.md section 7), i.e. a few 1e-4 of such a maximum
+    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=nf, precision=1))
+    assert info["kernel"] == 2 and info["precision"] == 1
+    assert_parity(gpu, ref, tol=3e-4)
