@@ -88,6 +88,20 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
 // Compact-entry store of one frame's (mid, d/16): frames are paired (2p, 2p+1); the mid section holds
 // [re_2p, re_2p+1, im_2p, im_2p+1] per pair and the d section the half2 words [(dr_2p, dr_2p+1), (di_2p, di_2p+1)],
 // so that the DAS kernels read aligned (frame 2p, frame 2p+1) register pairs for FFMA2.
+// Full-entry store of one frame: the same frame-pair layout with fp32 differences,
+// mid: [re_2p, re_2p+1, im_2p, im_2p+1], then d: [dr_2p, dr_2p+1, di_2p, di_2p+1], then 16 bytes of padding.
+template <int F>
+__device__ __forceinline__ void store_full_entry(unsigned char *ep, int f, float mr, float mi, float dr, float di) {
+    const int p = f >> 1, h = f & 1;
+    float *mid = reinterpret_cast<float *>(ep) + 4 * p + h;
+    mid[0] = mr;
+    mid[2] = mi;
+    float *d = reinterpret_cast<float *>(ep + 8 * F) + 4 * p + h;
+    d[0] = dr;
+    d[2] = di;
+    if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
+}
+
 template <int F>
 __device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16) {
     const int p = f >> 1, h = f & 1;
@@ -230,9 +244,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             const float dr = ok ? ar[q + 1] - ar[q] : 0.f, di = ok ? ai[q + 1] - ai[q] : 0.f;
             unsigned char *ep = s_out + ent * EB;
             if (D32) {
-                reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
-                reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(dr, di);
-                if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
+                store_full_entry<F>(ep, f, mr, mi, dr, di);
             } else {
                 store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di);
             }
@@ -289,9 +301,7 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
         const float dr = ok ? b.x - a.x : 0.f, di = ok ? b.y - a.y : 0.f;                              // = (d)/2
         unsigned char *ep = s_out + ent * EB;
         if (D32) {
-            reinterpret_cast<float2 *>(ep)[f] = make_float2(mr, mi);
-            reinterpret_cast<float2 *>(ep + 8 * F)[f] = make_float2(2.f * dr, 2.f * di);
-            if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
+            store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
         } else {
             store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di);
         }
@@ -478,6 +488,18 @@ __device__ __forceinline__ void chunk_mac2(const uint4 &m0, const uint4 &m1, con
     }
 }
 
+// One frame pair of a full entry in FFMA2 (ring kernel): m = [re, re, im, im], d = [dr, dr, di, di], AA = (a', a').
+__device__ __forceinline__ void pair_mac2_full(const uint4 &m, const uint4 &d, unsigned long long AA, unsigned long long CC,
+                                               unsigned long long SS, unsigned long long NS, unsigned long long &aR,
+                                               unsigned long long &aI) {
+    const unsigned long long VR = ffma2(AA, pack_f2(__uint_as_float(d.x), __uint_as_float(d.y)),
+                                        pack_f2(__uint_as_float(m.x), __uint_as_float(m.y)));
+    const unsigned long long VI = ffma2(AA, pack_f2(__uint_as_float(d.z), __uint_as_float(d.w)),
+                                        pack_f2(__uint_as_float(m.z), __uint_as_float(m.w)));
+    aR = ffma2(CC, VR, aR); aR = ffma2(NS, VI, aR);
+    aI = ffma2(SS, VR, aI); aI = ffma2(CC, VI, aI);
+}
+
 // interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
 // v = mid + a' d  (a' in fp32; compact: d converted from fp16),  acc += (c + j s) v
 template <int F, bool D32, class LoadVec>
@@ -485,14 +507,14 @@ __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, f
                                           int nv = F) {
     if (D32) {
 #pragma unroll
-        for (int q = 0; q < F / 2; ++q) {
+        for (int q = 0; q < F / 2; ++q) {        // frame pair q: m = [re, re, im, im], d = [dr, dr, di, di]
             if (2 * q >= nv) break;
             const uint4 m = ld(q), d = ld(F / 2 + q);
             const float mv[4] = {__uint_as_float(m.x), __uint_as_float(m.y), __uint_as_float(m.z), __uint_as_float(m.w)};
             const float dv[4] = {__uint_as_float(d.x), __uint_as_float(d.y), __uint_as_float(d.z), __uint_as_float(d.w)};
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
-                const float vr = fmaf(A.al, dv[2 * i], mv[2 * i]), vi = fmaf(A.al, dv[2 * i + 1], mv[2 * i + 1]);
+                const float vr = fmaf(A.al, dv[i], mv[i]), vi = fmaf(A.al, dv[2 + i], mv[2 + i]);
                 const int f = 2 * q + i;
                 accr[f] = fmaf(c, vr, accr[f]); accr[f] = fmaf(-s, vi, accr[f]);
                 acci[f] = fmaf(s, vr, acci[f]); acci[f] = fmaf(c, vi, acci[f]);

@@ -236,20 +236,12 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
         for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 16u;
 
-        // accumulators: full entries as floats, compact entries as (frame 2p, frame 2p+1) pairs for FFMA2
-        float accr[D32 ? PX : 1][D32 ? F : 1], acci[D32 ? PX : 1][D32 ? F : 1];
-        unsigned long long accR2[D32 ? 1 : PX][D32 ? 1 : F / 2], accI2[D32 ? 1 : PX][D32 ? 1 : F / 2];
-        if constexpr (D32) {
+        // accumulators: (frame 2p, frame 2p+1) pairs of real / imaginary parts for FFMA2
+        unsigned long long accR2[PX][F / 2], accI2[PX][F / 2];
 #pragma unroll
-            for (int m = 0; m < PX; ++m)
+        for (int m = 0; m < PX; ++m)
 #pragma unroll
-                for (int f = 0; f < F; ++f) accr[m][f] = acci[m][f] = 0.f;
-        } else {
-#pragma unroll
-            for (int m = 0; m < PX; ++m)
-#pragma unroll
-                for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
-        }
+            for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
 
         for (int j = 0; j < n_rx; ++j) {
             float Hs[PX], Rr[PX], Ri[PX];
@@ -299,7 +291,12 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
                     for (int m = 0; m < PX; ++m) {
                         const PixCtx x = prep(m);
-                        entry_mac<F, true>([&](int i) { return lds128(x.addr + 16u * i); }, x.A, x.c, x.s, accr[m], acci[m]);
+                        const unsigned long long AA = pack_f2(x.A.al, x.A.al), CC = pack_f2(x.c, x.c), SS = pack_f2(x.s, x.s),
+                                                 NS = pack_f2(-x.s, -x.s);
+#pragma unroll
+                        for (int q = 0; q < F / 2; ++q)
+                            pair_mac2_full(lds128(x.addr + 16u * q), lds128(x.addr + 8u * F + 16u * q), AA, CC, SS, NS,
+                                           accR2[m][q], accI2[m][q]);
                     }
                 } else {
                     // software pipeline over (pixel, 4-frame chunk): the three LDS.128 of step i + 1 are issued
@@ -339,15 +336,10 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
                 for (int f = 0; f < F; ++f) {
                     const int fr = g * F + f;
-                    float re, im;
-                    if constexpr (D32) {
-                        re = accr[m][f]; im = acci[m][f];
-                    } else {
-                        float r0, r1, i0, i1;
-                        unpack_f2(accR2[m][f / 2], r0, r1);
-                        unpack_f2(accI2[m][f / 2], i0, i1);
-                        re = (f & 1) ? r1 : r0; im = (f & 1) ? i1 : i0;
-                    }
+                    float r0, r1, i0, i1;
+                    unpack_f2(accR2[m][f / 2], r0, r1);
+                    unpack_f2(accI2[m][f / 2], i0, i1);
+                    const float re = (f & 1) ? r1 : r0, im = (f & 1) ? i1 : i0;
                     if (fr < P.n_frames)
                         P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] = make_float2(re, im);
                 }
