@@ -326,12 +326,12 @@ cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_
     return F == 12 ? launch_demod_f<12, false>(P, D, blocks, st) : launch_demod_f<4, false>(P, D, blocks, st);
 }
 
-// sample range [s_lo, s_hi) of a record the pre-pass can read (rounded outwards to 64 samples)
+// sample range [s_lo, s_hi) of a record the pre-pass can read (rounded outwards to 16 samples = 32 bytes)
 void host_sample_range(const ulm_rca_plan &P, int &s_lo, int &s_hi) {
     const int chunks = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
-    s_lo = std::max(0, P.n_lo - P.half_len) / 64 * 64;
+    s_lo = std::max(0, P.n_lo - P.half_len) / 16 * 16;
     const long long hi = (long long)P.n_lo + (long long)chunks * ulm::kDemodChunk + P.half_len + 2;
-    s_hi = (int)std::min<long long>(P.n_samples, (std::max<long long>(hi, 0) + 63) / 64 * 64);
+    s_hi = (int)std::min<long long>(P.n_samples, (std::max<long long>(hi, 0) + 15) / 16 * 16);
     if (s_hi < s_lo) s_hi = s_lo;
 }
 
