@@ -82,6 +82,22 @@ def whole_job(frames_per_rank: int, world: int, ms_local: float, all_reduce_max=
     return world * frames_per_rank / (ms * 1e-3), ms
 
 
+def prepass_roofline(cfg, info, n_frames, demod_ms):
+    """HBM roofline of the staging pre-pass: algorithmic bytes = (2 B read + scratch bytes written) per touched
+    (sample, frame) of the receive aperture of every event; peak = measured copy bandwidth (MEASURED_PEAKS.json)."""
+    peak, src = 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peak, src = float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        pass
+    rows = len(cfg.row_tx_angles) * cfg.n_cols + len(cfg.col_tx_angles) * cfg.n_rows
+    byts = float(rows) * info["l_row"] * n_frames * (2 + info["scratch_bytes_per_sample"])
+    achieved = byts / (demod_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "kernel": "demod_quad_kernel / demod_kernel", "algorithmic_bytes": byts, "peak_source": src}
+
+
 def make_ensemble(cfg, torch, device):
     """Seeded synthetic ensemble in HBM: a few frames of the moving scene rendered on the host by synth/
     (the CPU echo simulator) and tiled over the n_frames-long buffer.  DAS cost does not depend on values."""
@@ -196,6 +212,7 @@ def run_ours(args):
                          "peak_source": "derived: 148 SM x 128 lanes x 2 x 1965 MHz (DESIGN.md); FFMA probe measured "
                                         "%.1f TFLOP/s on this box" % fp32_probe,
                          "whole_step_frac": FLOP_PER_GATHER * gathers / (ms_step * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS},
+            "roofline_prepass": prepass_roofline(cfg, info, n_frames, demod_ms),
             "cpu_baseline": cpu, "clocks": clocks,
             "e2e": {"value": world * n_frames / (e2e_ms_step * 1e-3), "unit": "frames/s",
                     "h2d_bytes_per_step": int(info["host_upload_bytes_per_frame"]) * n_frames,
