@@ -162,6 +162,17 @@ ulm_rca_status ulm_rca_plan_timing(const ulm_rca_plan *plan, int32_t n_calls, do
  * SM on cuda_stream, synchronises, and returns the measured TFLOP/s (2 flop per FMA) in *tflops. */
 ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream);
 
+/* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
+ * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets
+ * `t0_s` (NULL = 0), image grid `grid`.  Returns the number of tiles in *n_tiles, the stage length in entries in
+ * *window, and, when the arrays are non-NULL (n_tiles * n_rx ints each), the per-(tile, element) window offsets
+ * dj = floor(min receive excess over the tile) - 2 and stage lengths wj.  A tile is 384 consecutive positions of
+ * (strip of 4 depth rows) x (lateral index), strips outer.  ULM_RCA_EUNSUPPORTED if the ring kernel does not
+ * cover the shape. */
+ulm_rca_status ulm_rca_ring_probe(int32_t n_rx, float pitch_m, const float *angles_rad, const float *t0_s, int32_t n_tx,
+                                  float c_mps, float fs_hz, float t_start_s, const ulm_rca_grid *grid,
+                                  int32_t *n_tiles, int32_t *window, int32_t *dj, int32_t *wj);
+
 void ulm_rca_plan_destroy(ulm_rca_plan *plan); /* NULL-safe */
 
 const char *ulm_rca_last_error(void); /* thread-local, valid until the next failing call */

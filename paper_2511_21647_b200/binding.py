@@ -20,7 +20,8 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
 _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
-           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_plan_destroy",
+           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe",
+           "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
 
@@ -79,6 +80,10 @@ def load() -> C.CDLL:
     lib.ulm_rca_plan_timing.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
+    lib.ulm_rca_ring_probe.restype = C.c_int
+    lib.ulm_rca_ring_probe.argtypes = [i32, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float), i32, C.c_float,
+                                       C.c_float, C.c_float, C.POINTER(Grid), C.POINTER(i32), C.POINTER(i32),
+                                       C.POINTER(i32), C.POINTER(i32)]
     lib.ulm_rca_plan_destroy.restype = None
     lib.ulm_rca_plan_destroy.argtypes = [vp]
     lib.ulm_rca_last_error.restype = C.c_char_p
@@ -229,6 +234,25 @@ class Plan:
         nxz = self.grid_xz[0] * self.grid_xz[3]
         return (out_frame[:nxz].reshape(self.grid_xz[0], self.grid_xz[3]),
                 out_frame[nxz:].reshape(self.grid_yz[0], self.grid_yz[3]))
+
+
+def ring_probe(n_rx: int, pitch: float, angles: Sequence[float], c: float, fs: float, grid: tuple,
+               t0: Optional[Sequence[float]] = None, t_start: float = 0.0) -> dict:
+    """Host-only tile / window planning of the ring kernel for one aperture (ulm_rca_ring_probe)."""
+    lib = load()
+    aa, ap = _farr(list(angles))
+    ta, tp = _farr(t0)
+    g = Grid(*grid)
+    nt, w = C.c_int32(), C.c_int32()
+    _check(lib.ulm_rca_ring_probe(int(n_rx), float(pitch), ap, tp, len(angles), float(c), float(fs), float(t_start),
+                                  C.byref(g), C.byref(nt), C.byref(w), None, None))
+    dj = (C.c_int32 * (nt.value * n_rx))()
+    wj = (C.c_int32 * (nt.value * n_rx))()
+    _check(lib.ulm_rca_ring_probe(int(n_rx), float(pitch), ap, tp, len(angles), float(c), float(fs), float(t_start),
+                                  C.byref(g), C.byref(nt), C.byref(w), dj, wj))
+    return {"n_tiles": nt.value, "window": w.value,
+            "dj": np.array(dj, dtype=np.int64).reshape(nt.value, n_rx),
+            "wj": np.array(wj, dtype=np.int64).reshape(nt.value, n_rx)}
 
 
 def fp32_peak_tflops(stream=None) -> float:

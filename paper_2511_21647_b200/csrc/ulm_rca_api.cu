@@ -703,6 +703,28 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
     return ULM_RCA_OK;
 }
 
+ulm_rca_status ulm_rca_ring_probe(int32_t n_rx, float pitch_m, const float *angles_rad, const float *t0_s, int32_t n_tx,
+                                  float c_mps, float fs_hz, float t_start_s, const ulm_rca_grid *grid,
+                                  int32_t *n_tiles, int32_t *window, int32_t *dj, int32_t *wj) {
+    if (!angles_rad || !grid || !n_tiles || !window || n_rx <= 0 || n_tx <= 0) return fail(ULM_RCA_EINVAL, "bad argument");
+    if (ulm_rca_status s = check_grid(grid, "grid")) return s;
+    std::vector<double> ang(angles_rad, angles_rad + n_tx), t0(n_tx, 0.0);
+    if (t0_s) for (int k = 0; k < n_tx; ++k) t0[k] = t0_s[k];
+    ulm::RingApertureDesc D{n_tx, n_rx, grid->n_lat, grid->n_ax, grid->lat0_m, grid->dlat_m, grid->z0_m, grid->dz_m,
+                            grid->ref_m, ang.data(), t0.data()};
+    std::vector<int> tab;
+    int nt = 0;
+    const char *why = nullptr;
+    const int w = ulm::ring_plan_aperture(D, pitch_m, c_mps, fs_hz, t_start_s, tab, nt, &why);
+    if (w < 0) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
+    *n_tiles = nt;
+    *window = (w + 7) / 8 * 8;
+    const size_t n = (size_t)nt * n_rx;
+    if (dj) std::copy(tab.begin(), tab.begin() + n, dj);
+    if (wj) std::copy(tab.begin() + n, tab.begin() + 2 * n, wj);
+    return ULM_RCA_OK;
+}
+
 ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream) {
     if (!tflops) return fail(ULM_RCA_EINVAL, "tflops is NULL");
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -86,7 +86,7 @@ int main() {
     CK(cudaGetLastError());
     const double steps[] = {0.0, 0.25, 0.3, 0.4, 0.45, 0.5, 0.6, 0.75, 1.0, 1.5, 2.0};
     const double offs[] = {0.0, 0.35, 0.7};
-    const int strides[] = {8, 16, 144, 64, 128};
+    const int strides[] = {8, 16, 144, 120, 40, 112, 64, 128};
     for (int stride : strides) {
         for (double s : steps) for (double off : offs) {
             if (off != 0.0 && (s == 0.0 || s >= 1.0)) continue;
