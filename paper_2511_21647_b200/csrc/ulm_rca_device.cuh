@@ -10,14 +10,18 @@
 //   add-magic-constant trick on (u - 0.5).
 //
 // IQ scratch ("entries"): frames are processed in groups of F (4 or 12) and paired (2p, 2p+1).  For frame group g,
-// event e, receive element j and sample n the scratch holds ONE compact entry of 12 F bytes:
-//     mid section, 16 B per frame pair:  [re_2p, re_2p+1, im_2p, im_2p+1]  of  mid = (iq[n] + iq[n+1]) / 2   (fp32)
+// event e, receive element j and sample n the scratch holds ONE compact entry of 10 F bytes:
+//     mid section, 24 B per chunk of 4 frames (frame pairs a, b) of  mid = (iq[n] + iq[n+1]) / 2  as "fp24" = the top
+//       three bytes of the fp32 value (16 mantissa bits): words W0..W5 carry re_a0, re_a1, im_a0, im_a1, re_b0, re_b1 in
+//       their top three bytes; the low bytes of W0, W1, W2 are bytes 3, 2, 1 of im_b0 and those of W3, W4, W5 the same
+//       of im_b1 (two PRMT each to reassemble; the six direct values are used as loaded, their low mantissa byte
+//       being a byte of another value, i.e. a zero-mean error below 2^-16 relative)
 //     d section,    8 B per frame pair:  half2 (dr_2p, dr_2p+1), half2 (di_2p, di_2p+1)  of  d/16 = (iq[n+1] - iq[n]) / 16
-// so that the interpolated sample is mid + a' d with a' = a - 0.5 in [-0.5, 0.5]: the value carries fp32
-// precision, only the small difference term is fp16, and one LDS.128 delivers aligned (frame 2p, frame 2p+1)
-// register pairs for the packed fp32x2 FMA (FFMA2).  "Full" entries keep d in fp32 (16 F + 16 bytes).  Entry
-// sizes 48 / 144 / 80 / 208 B are odd multiples of 16 B, which keeps the LDS.128 gathers of neighbouring
-// entries free of bank conflicts.
+// so that the interpolated sample is mid + a' d with a' = a - 0.5 in [-0.5, 0.5]: the value carries 17 significant
+// bits, only the small difference term is fp16, and every LDS.64 delivers an aligned (frame 2p, frame 2p+1)
+// register pair for the packed fp32x2 FMA (FFMA2).  "Full" entries keep mid and d in fp32 (16 F + 16 bytes, LDS.128).
+// Compact entry sizes 40 / 120 B are odd multiples of 8 B: the LDS.64 gathers of the 16 lanes of a half-warp fall into
+// 16 different bank pairs whenever their entries differ; full entry sizes 80 / 208 B are odd multiples of 16 B.
 #pragma once
 
 #include <cuda_fp16.h>
@@ -32,11 +36,11 @@ constexpr int kMaxTaps = 129;
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kDScale = 0.0625f;           // d is stored / 16 (|d| can exceed the fp16 range) ...
 constexpr float kAlScale = 16.0f;            // ... and a' is multiplied by 16 before rounding to fp16
-constexpr int kDemodChunk = 127;             // entries per demodulation CTA (128 iq values)
+constexpr int kDemodChunk = 126;             // entries per demodulation CTA (even: every chunk of 10 F-byte entries starts 16-byte aligned)
 
-// D32 = false: compact entries (fp16 difference term, 12 F bytes); true: full entries (fp32 difference
-// term, 16 F bytes + 16 bytes of padding that keep the entry an odd multiple of 16 B)
-__host__ __device__ constexpr int entry_bytes(int F, bool D32) { return D32 ? 16 * F + 16 : 12 * F; }
+// D32 = false: compact entries (fp24 mid + fp16 difference term, 10 F bytes); true: full entries (fp32 mid and
+// difference term, 16 F bytes + 16 bytes of padding that keep the entry an odd multiple of 16 B)
+__host__ __device__ constexpr int entry_bytes(int F, bool D32) { return D32 ? 16 * F + 16 : 10 * F; }
 
 // Demodulation constants (per plan), in constant memory.
 struct DemodConst {
@@ -48,7 +52,7 @@ struct DemodConst {
 
 struct DemodParams {
     const int16_t *rf;       // [frame][event][channel][sample] (x2 for IQ input)
-    unsigned char *iq;       // entries: [group][event][rx elem (n_rx_max)][l_row][12 F bytes]
+    unsigned char *iq;       // entries: [group][event][rx elem (n_rx_max)][l_row][entry_bytes(F, D32)]
     const float2 *mixer;     // exp(-j 2 pi fc t_n) for n = mix_n0 .. (RF input only)
     int mix_n0;
     int n_frames, n_events, channels_per_event, n_samples;
@@ -85,9 +89,9 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
     return r;
 }
 
-// Compact-entry store of one frame's (mid, d/16): frames are paired (2p, 2p+1); the mid section holds
-// [re_2p, re_2p+1, im_2p, im_2p+1] per pair and the d section the half2 words [(dr_2p, dr_2p+1), (di_2p, di_2p+1)],
-// so that the DAS kernels read aligned (frame 2p, frame 2p+1) register pairs for FFMA2.
+// Compact-entry store of one frame's (mid, d/16) in the layout described at the top of this file (fp24 mid words
+// per 4-frame chunk, then the half2 words [(dr_2p, dr_2p+1), (di_2p, di_2p+1)] per frame pair), so that the DAS
+// kernels read aligned (frame 2p, frame 2p+1) register pairs for FFMA2.
 // Full-entry store of one frame: the same frame-pair layout with fp32 differences,
 // mid: [re_2p, re_2p+1, im_2p, im_2p+1], then d: [dr_2p, dr_2p+1, di_2p, di_2p+1], then 16 bytes of padding.
 template <int F>
@@ -104,25 +108,36 @@ __device__ __forceinline__ void store_full_entry(unsigned char *ep, int f, float
 
 template <int F>
 __device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16) {
-    const int p = f >> 1, h = f & 1;
-    float *mid = reinterpret_cast<float *>(ep) + 4 * p + h;
-    mid[0] = mr;
-    mid[2] = mi;
-    unsigned short *d = reinterpret_cast<unsigned short *>(ep + 8 * F) + 4 * p + h;
+    const int p = f >> 1, h = f & 1, pc = p & 1;
+    unsigned char *mid = ep + 24 * (p >> 1);                 // the 6 words of this 4-frame chunk
+    const uint32_t br = __float_as_uint(mr), bi = __float_as_uint(mi);
+    // direct slots: top three bytes of word s (truncation; the reader sees a foreign low byte, zero-mean)
+    const int sr = pc ? 4 + h : h;
+    mid[4 * sr + 1] = (unsigned char)(br >> 8);
+    *reinterpret_cast<unsigned short *>(mid + 4 * sr + 2) = (unsigned short)(br >> 16);
+    if (pc == 0) {
+        mid[4 * (2 + h) + 1] = (unsigned char)(bi >> 8);
+        *reinterpret_cast<unsigned short *>(mid + 4 * (2 + h) + 2) = (unsigned short)(bi >> 16);
+    } else {                                                 // im of pair b: spread over the low bytes of three words
+        mid[12 * h] = (unsigned char)(bi >> 24);
+        mid[12 * h + 4] = (unsigned char)(bi >> 16);
+        mid[12 * h + 8] = (unsigned char)(bi >> 8);
+    }
+    unsigned short *d = reinterpret_cast<unsigned short *>(ep + 6 * F) + 4 * p + h;
     d[0] = f2h_bits(dr16);
     d[2] = f2h_bits(di16);
 }
 
 // ---------------------------------------------------------------------------------------------------
 // Demodulation / staging pre-pass: int16 RF (or IQ) -> scratch entries over the touched
-// sample range only.  One CTA = one chunk of 127 entries of one (frame group, event, rx element) row, all F
+// sample range only.  One CTA = one chunk of 126 entries of one (frame group, event, rx element) row, all F
 // frames of the group:
 //   (1) the mixed samples x = rf * exp(-j 2 pi fc t) of the F frames go to shared memory;
 //   (2) thread (frame f, group of 8 entries) runs the FIR for 9 consecutive outputs with the inputs sliding
 //       through registers (dense taps straight from constant memory; HB = half-band filter, fs = 4 fc: the
 //       even taps other than the centre are exactly zero and are skipped at compile time), forms
 //       mid = (a + b)/2 and d = b - a and writes them into an image of the output block in shared memory;
-//   (3) one elected thread stores the block (127 x 12 F contiguous bytes) with one cp.async.bulk (TMA).
+//   (3) one elected thread stores the block (126 x 10 F contiguous bytes) with one cp.async.bulk (TMA).
 // NT = dense tap count 2L+1 (0: run-time L).  Lanes of a half-warp are the frames of one group, so every
 // shared-memory access of step (2) is conflict free (row stride of x = 1 mod 16 float2).
 // ---------------------------------------------------------------------------------------------------
@@ -144,7 +159,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
     const int XW = kDemodChunk + 2 + 2 * L;    // mixed samples per frame: iq[0..128] needs x[0 .. 128 + 2L]
     const int XS = demod_xs(L);                // row stride of s_x (float2)
-    unsigned char *s_out = s_raw;              // [127][EB] image of the output block
+    unsigned char *s_out = s_raw;              // [126][EB] image of the output block
     float2 *s_x = reinterpret_cast<float2 *>(s_raw + OUT_BYTES);   // [F][XS]
 
     // grid = (chunks per row, n_rx_max, groups * n_events)
@@ -445,46 +460,71 @@ __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsign
     return d;
 }
 
-// Four frames (two frame pairs) of a compact entry: m0 / m1 = [re_a, re_b, im_a, im_b] of pairs 0 / 1,
-// dd = [(dr, dr), (di, di)] half2 words of pair 0 then pair 1 (difference term / 16).
+// im_b0 / im_b1 of a compact chunk from the low bytes of its six mid words (two PRMT each)
+__device__ __forceinline__ uint32_t fp24_gather(uint32_t w0, uint32_t w1, uint32_t w2) {
+    return __byte_perm(__byte_perm(w0, w1, 0x0400), w2, 0x3245);
+}
+
+// Four frames (two frame pairs a, b) of a compact entry: w[0..5] = the mid words, dd[0..3] = half2 words
+// [(dr, dr), (di, di)] of pair a then pair b (difference term / 16).
 // Scalar version (generic kernel): v = mid + a16 * d with d converted to fp32 (the fp16 x fp32 product is exact
 // in the FMA), acc += (c + j s) v.  nv = number of valid frames among the four.
-__device__ __forceinline__ void chunk_mac(const uint4 &m0, const uint4 &m1, const uint4 &dd, const Alpha &A, float c,
+__device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t (&dd)[4], const Alpha &A, float c,
                                           float s, float *accr, float *acci, int nv = 4) {
-    const uint32_t mids[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
-    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
+    const uint32_t re[4] = {w[0], w[1], w[4], w[5]};
+    const uint32_t im[4] = {w[2], w[3], fp24_gather(w[0], w[1], w[2]), fp24_gather(w[3], w[4], w[5])};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         if (i >= nv) break;
         const int p = i >> 1, h = i & 1;
         unsigned short r0, r1, i0, i1;
-        split_h2(ds[2 * p], r0, r1);
-        split_h2(ds[2 * p + 1], i0, i1);
-        const float vr = fmaf(A.a16, h2f(h ? r1 : r0), __uint_as_float(mids[4 * p + h]));
-        const float vi = fmaf(A.a16, h2f(h ? i1 : i0), __uint_as_float(mids[4 * p + 2 + h]));
+        split_h2(dd[2 * p], r0, r1);
+        split_h2(dd[2 * p + 1], i0, i1);
+        const float vr = fmaf(A.a16, h2f(h ? r1 : r0), __uint_as_float(re[i]));
+        const float vi = fmaf(A.a16, h2f(h ? i1 : i0), __uint_as_float(im[i]));
         accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
         acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
     }
 }
 
-// Packed version (ring kernel): the interpolation and the complex multiply-accumulate of a frame pair run as
-// FFMA2 on (frame 2p, frame 2p+1) register pairs; aR / aI are pairs of real / imaginary accumulators;
-// AA = (a16, a16), CC = (c, c), SS = (s, s), NS = (-s, -s).  Each half is an ordinary round-to-nearest fp32 FMA,
-// so the results are bit-identical to chunk_mac.
-__device__ __forceinline__ void chunk_mac2(const uint4 &m0, const uint4 &m1, const uint4 &dd, unsigned long long AA,
+__device__ __forceinline__ void split_u2(unsigned long long v, uint32_t &lo, uint32_t &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long pack_u2(uint32_t lo, uint32_t hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+
+// Packed version (ring kernel): m01 / m23 / m45 = the mid words as loaded by three LDS.64 (already the register
+// pairs (re_a0, re_a1), (im_a0, im_a1), (re_b0, re_b1)), da / db = the d words of pairs a / b.  The interpolation
+// and the complex multiply-accumulate of a frame pair run as FFMA2 on (frame 2p, frame 2p+1) register pairs; aR / aI
+// are pairs of real / imaginary accumulators; AA = (a16, a16), CC = (c, c), SS = (s, s), NS = (-s, -s).  Each half is
+// an ordinary round-to-nearest fp32 FMA, so the results are bit-identical to chunk_mac.
+__device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long long m23, unsigned long long m45,
+                                           unsigned long long da, unsigned long long db, unsigned long long AA,
                                            unsigned long long CC, unsigned long long SS, unsigned long long NS,
                                            unsigned long long *aR, unsigned long long *aI) {
-    const uint32_t ds[4] = {dd.x, dd.y, dd.z, dd.w};
-#pragma unroll
-    for (int p = 0; p < 2; ++p) {
-        const uint4 &m = p ? m1 : m0;
-        unsigned short r0, r1, i0, i1;
-        split_h2(ds[2 * p], r0, r1);
-        split_h2(ds[2 * p + 1], i0, i1);
-        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), pack_f2(__uint_as_float(m.x), __uint_as_float(m.y)));
-        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), pack_f2(__uint_as_float(m.z), __uint_as_float(m.w)));
-        aR[p] = ffma2(CC, VR, aR[p]); aR[p] = ffma2(NS, VI, aR[p]);
-        aI[p] = ffma2(SS, VR, aI[p]); aI[p] = ffma2(CC, VI, aI[p]);
+    uint32_t w0, w1, w2, w3, w4, w5, d0, d1, d2, d3;
+    split_u2(m01, w0, w1); split_u2(m23, w2, w3); split_u2(m45, w4, w5);
+    split_u2(da, d0, d1); split_u2(db, d2, d3);
+    const unsigned long long m67 = pack_u2(fp24_gather(w0, w1, w2), fp24_gather(w3, w4, w5));
+    unsigned short r0, r1, i0, i1;
+    {
+        split_h2(d0, r0, r1);
+        split_h2(d1, i0, i1);
+        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), m01);
+        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), m23);
+        aR[0] = ffma2(CC, VR, aR[0]); aR[0] = ffma2(NS, VI, aR[0]);
+        aI[0] = ffma2(SS, VR, aI[0]); aI[0] = ffma2(CC, VI, aI[0]);
+    }
+    {
+        split_h2(d2, r0, r1);
+        split_h2(d3, i0, i1);
+        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), m45);
+        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), m67);
+        aR[1] = ffma2(CC, VR, aR[1]); aR[1] = ffma2(NS, VI, aR[1]);
+        aI[1] = ffma2(SS, VR, aI[1]); aI[1] = ffma2(CC, VI, aI[1]);
     }
 }
 
@@ -500,16 +540,18 @@ __device__ __forceinline__ void pair_mac2_full(const uint4 &m, const uint4 &d, u
     aI = ffma2(SS, VR, aI); aI = ffma2(CC, VI, aI);
 }
 
-// interpolate-and-accumulate of F frames from one entry (global or shared memory), shared by both DAS kernels:
-// v = mid + a' d  (a' in fp32; compact: d converted from fp16),  acc += (c + j s) v
-template <int F, bool D32, class LoadVec>
-__device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, float s, float *accr, float *acci,
-                                          int nv = F) {
+// interpolate-and-accumulate of F frames from one entry in global memory (generic kernel):
+// v = mid + a' d  (a' in fp32; compact: d converted from fp16),  acc += (c + j s) v.
+// Full entries are read as 16-byte units, compact entries (8-byte aligned) as 8-byte units.
+template <int F, bool D32>
+__device__ __forceinline__ void entry_mac(const unsigned char *ent, const Alpha &A, float c, float s, float *accr,
+                                          float *acci, int nv = F) {
     if (D32) {
+        const uint4 *e4 = reinterpret_cast<const uint4 *>(ent);
 #pragma unroll
         for (int q = 0; q < F / 2; ++q) {        // frame pair q: m = [re, re, im, im], d = [dr, dr, di, di]
             if (2 * q >= nv) break;
-            const uint4 m = ld(q), d = ld(F / 2 + q);
+            const uint4 m = __ldg(e4 + q), d = __ldg(e4 + F / 2 + q);
             const float mv[4] = {__uint_as_float(m.x), __uint_as_float(m.y), __uint_as_float(m.z), __uint_as_float(m.w)};
             const float dv[4] = {__uint_as_float(d.x), __uint_as_float(d.y), __uint_as_float(d.z), __uint_as_float(d.w)};
 #pragma unroll
@@ -521,12 +563,15 @@ __device__ __forceinline__ void entry_mac(LoadVec ld, const Alpha &A, float c, f
             }
         }
     } else {
+        const uint2 *e2 = reinterpret_cast<const uint2 *>(ent);
 #pragma unroll
         for (int q = 0; q < F / 4; ++q) {
             if (4 * q >= nv) break;
-            // the second frame pair of the chunk is not even loaded when the group has no valid frame in it
-            const uint4 m1 = nv - 4 * q > 2 ? ld(2 * q + 1) : make_uint4(0u, 0u, 0u, 0u);
-            chunk_mac(ld(2 * q), m1, ld(F / 2 + q), A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
+            const uint2 a = __ldg(e2 + 3 * q), b = __ldg(e2 + 3 * q + 1), cc = __ldg(e2 + 3 * q + 2);
+            const uint2 da = __ldg(e2 + (6 * F) / 8 + 2 * q), db = __ldg(e2 + (6 * F) / 8 + 2 * q + 1);
+            const uint32_t w[6] = {a.x, a.y, b.x, b.y, cc.x, cc.y};
+            const uint32_t dd[4] = {da.x, da.y, db.x, db.y};
+            chunk_mac(w, dd, A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
         }
     }
 }
@@ -580,9 +625,8 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             float s, c;
             sincos_cycles(fmaf(P.fcfs, upm, P.ph0[t]), s, c);
             if (APOD) { s *= w; c *= w; }
-            const uint4 *ent = reinterpret_cast<const uint4 *>(
-                P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32));
-            entry_mac<F, D32>([&](int i) { return __ldg(ent + i); }, make_alpha(al), c, s, accr, acci, nv);
+            const unsigned char *ent = P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32);
+            entry_mac<F, D32>(ent, make_alpha(al), c, s, accr, acci, nv);
         }
     }
     const long long o = P.out_base + (long long)il * P.s_lat + (long long)plane * P.s_plane +

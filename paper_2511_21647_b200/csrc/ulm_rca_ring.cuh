@@ -15,8 +15,9 @@
 // Pixel mapping: the image is cut into horizontal strips of PX rows; a consumer thread owns the PX
 // vertically adjacent pixels of one (strip, column) position and a tile is 384 consecutive positions, so the
 // lanes of a warp are lateral neighbours at the same depths: their sample indices form a slowly varying
-// monotone run and the LDS.128 gathers of a half-warp mostly fall into <= 8 distinct entries (one
-// shared-memory wavefront; entry size 12 F bytes = odd multiple of 16 B => no bank conflicts).
+// monotone run; compact entries (10 F bytes = odd multiple of 8 B) are gathered with LDS.64, whose 16 lanes of a
+// half-warp hit 16 different bank pairs or the same address (measured: 2 cycles per warp-level LDS.64 = 128 B/clk
+// up to one entry per lane, profiles/r01_smem_microbench.md); full entries (odd multiple of 16 B) with LDS.128.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -84,6 +85,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "LAB_DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// non-blocking phase test (acquire): true when the phase with the given parity has completed
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar)
@@ -91,6 +103,11 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 }
 __device__ __forceinline__ void consumer_bar() {
     asm volatile("bar.sync 1, %0;" ::"n"(kRingConsumers) : "memory");
+}
+__device__ __forceinline__ unsigned long long lds64(uint32_t addr) {
+    unsigned long long v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
 }
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
@@ -128,7 +145,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     __syncthreads();
 
     const int tiles_all = P.ap[0].n_tiles + P.ap[1].n_tiles;
-    uint32_t stage_ctr = 0;     // global stage counter (identical sequence in producer and consumers)
+    // ring position of the next stage (identical sequence in producer and consumers): slot and phase parity are
+    // carried along instead of dividing a stage counter by the run-time ring depth
+    uint32_t slot = 0, phase = 0;
 
     if (warp >= kRingConsumerWarps) {
         // ============ PRODUCER WARP GROUP: gives its registers to the consumers; one warp works ============
@@ -160,8 +179,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     if (lane == 0) {
                         const int st = sb + i;
                         const int j = st / n_tx, k = st - j * n_tx;
-                        const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
-                        const int s0 = max(0, min(s0_raw, P.l_row - wlen));
+                        // compact entries are 8-byte multiples: an even first entry keeps the copy 16-byte aligned
+                        // (the window has two spare entries at either end, ring_plan_aperture)
+                        const int s0 = max(0, min(s0_raw, P.l_row - wlen)) & (D32 ? ~0 : ~1);
                         mbar_wait(smem_u32(&s_empty[slot]), phase ^ 1);
                         s_hdr[slot] = s0_raw - s0 - kMagicBits;     // entry shift, with the magic-constant bits folded in
                         const uint32_t bar = smem_u32(&s_full[slot]);
@@ -170,7 +190,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                         const unsigned char *src = grp + (((size_t)(e0 + k) * P.n_rx_max + j) * P.l_row + s0) * EB;
                         bulk_g2s(smem_u32(smem) + slot * P.stage_stride, src, bytes, bar);
                     }
-                    ++stage_ctr;
+                    if (++slot == (uint32_t)NS) { slot = 0; phase ^= 1; }
                 }
             }
         }
@@ -243,6 +263,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 #pragma unroll
             for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
 
+        bool ready = false;      // the full barrier of the next stage was already seen complete
         for (int j = 0; j < n_rx; ++j) {
             float Hs[PX], Rr[PX], Ri[PX];
             {
@@ -266,16 +287,21 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 }
             }
             for (int k = 0; k < n_tx; ++k) {
-                const uint32_t slot = stage_ctr % NS, phase = (stage_ctr / NS) & 1;
-                mbar_wait(smem_u32(&s_full[slot]), phase);
+                // the table row of the first pixel does not depend on the ring: fetched before the barrier wait
+                const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
+                uint4 tbn = lds128(tk + tab_off[0]);
+                if (!ready) mbar_wait(smem_u32(&s_full[slot]), phase);
                 // entry address = stage base + EB * (rint(upm) + shift); hdr = shift - magic-constant bits
                 const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride;
                 const int hdr = s_hdr[slot];
-                const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
+                const uint32_t my_empty = smem_u32(&s_empty[slot]);
+                // ring position of the next stage; its barrier is tested now (non-blocking) and the answer is used
+                // at the top of the next iteration, so the latency of the test is hidden behind this stage's work
+                if (++slot == (uint32_t)NS) { slot = 0; phase ^= 1; }
+                ready = mbar_test(smem_u32(&s_full[slot]), phase);
                 // per-pixel setup of this stage: entry address, interpolation weight, phasor T_k(z) R(p, j)
                 struct PixCtx { uint32_t addr; Alpha A; float c, s; };
-                auto prep = [&](int m) {
-                    const uint4 tb = lds128(tk + tab_off[m]);
+                auto prep_tb = [&](int m, const uint4 &tb) {
                     const float upm = __uint_as_float(tb.x) + Hs[m];
                     const float tt_ = upm + kMagic;
                     const float al = upm - (tt_ - kMagic);
@@ -287,6 +313,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     x.s = fmaf(Tr, Ri[m], Ti * Rr[m]);
                     return x;
                 };
+                auto prep = [&](int m) { return prep_tb(m, lds128(tk + tab_off[m])); };
                 if constexpr (D32) {
 #pragma unroll
                     for (int m = 0; m < PX; ++m) {
@@ -299,31 +326,37 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                                            accR2[m][q], accI2[m][q]);
                     }
                 } else {
-                    // software pipeline over (pixel, 4-frame chunk): the three LDS.128 of step i + 1 are issued
-                    // before the 32 FMAs of step i
+                    // software pipeline over (pixel, 4-frame chunk): the five LDS.64 of step i + 1 (three mid word
+                    // pairs, two d word pairs) are issued before the 32 FMAs of step i
                     constexpr int NQ = F / 4, NSTEP = PX * NQ;
-                    uint4 buf[2][3];
-                    PixCtx cur = prep(0), nxt = cur;
-                    buf[0][0] = lds128(cur.addr); buf[0][1] = lds128(cur.addr + 16u); buf[0][2] = lds128(cur.addr + 8u * F);
+                    unsigned long long buf[2][5];
+                    PixCtx cur = prep_tb(0, tbn), nxt = cur;
+                    if (PX > 1) tbn = lds128(tk + tab_off[1]);
+                    buf[0][0] = lds64(cur.addr); buf[0][1] = lds64(cur.addr + 8u); buf[0][2] = lds64(cur.addr + 16u);
+                    buf[0][3] = lds64(cur.addr + 6u * F); buf[0][4] = lds64(cur.addr + 6u * F + 8u);
 #pragma unroll
                     for (int st = 0; st < NSTEP; ++st) {
                         const int m = st / NQ, q = st % NQ;
                         if (st + 1 < NSTEP) {
                             const int m1 = (st + 1) / NQ, q1 = (st + 1) % NQ;
-                            if (q1 == 0) nxt = prep(m1);
+                            if (q1 == 0) {
+                                // the table row of pixel m1 was requested a whole pixel (NQ chunks) earlier
+                                nxt = prep_tb(m1, tbn);
+                                if (m1 + 1 < PX) tbn = lds128(tk + tab_off[m1 + 1]);
+                            }
                             const uint32_t a1 = q1 == 0 ? nxt.addr : cur.addr;
-                            uint4 *b = buf[(st + 1) & 1];
-                            b[0] = lds128(a1 + 32u * q1); b[1] = lds128(a1 + 32u * q1 + 16u); b[2] = lds128(a1 + 8u * F + 16u * q1);
+                            unsigned long long *b = buf[(st + 1) & 1];
+                            b[0] = lds64(a1 + 24u * q1); b[1] = lds64(a1 + 24u * q1 + 8u); b[2] = lds64(a1 + 24u * q1 + 16u);
+                            b[3] = lds64(a1 + 6u * F + 16u * q1); b[4] = lds64(a1 + 6u * F + 16u * q1 + 8u);
                         }
-                        const uint4 *b = buf[st & 1];
-                        chunk_mac2(b[0], b[1], b[2], pack_f2(cur.A.a16, cur.A.a16), pack_f2(cur.c, cur.c),
+                        const unsigned long long *b = buf[st & 1];
+                        chunk_mac2(b[0], b[1], b[2], b[3], b[4], pack_f2(cur.A.a16, cur.A.a16), pack_f2(cur.c, cur.c),
                                    pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
                         if (q == NQ - 1) cur = nxt;
                     }
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&s_empty[slot]));
-                ++stage_ctr;
+                if (lane == 0) mbar_arrive(my_empty);
             }
         }
         // projection write: one float2 per pixel and frame
