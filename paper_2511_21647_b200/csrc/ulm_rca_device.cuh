@@ -35,7 +35,7 @@ constexpr int kMagicBits = 0x4B400000;
 constexpr int kMaxTaps = 129;
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kDScale = 0.0625f;           // d is stored / 16 (|d| can exceed the fp16 range) ...
-constexpr float kAlScale = 16.0f;            // ... and a' is multiplied by 16 before rounding to fp16
+constexpr float kAlScale = 16.0f;            // ... and a' is multiplied by 16 before it is rounded to fp16
 constexpr int kDemodChunk = 126;             // entries per demodulation CTA (even: every chunk of 10 F-byte entries starts 16-byte aligned)
 
 // D32 = false: compact entries (fp24 mid + fp16 difference term, 10 F bytes); true: full entries (fp32 mid and
@@ -431,15 +431,18 @@ struct DasParams {
     int n_frames;                    // frames in this batch
 };
 
-// the interpolation weight a' = a - 0.5 of one gather, fp32: al for full entries, a16 = 16 a' for compact
-// entries (whose difference term is stored / 16)
+// the interpolation weight a' = a - 0.5 of one gather: al (fp32) for full entries; ah = 16 a' rounded to fp16 for
+// compact entries, whose difference term is stored / 16 in fp16 -- there the whole interpolation
+// v = mid + (16 a') (d / 16) is ONE mixed-precision FMA per component (FHFMA: fp16 x fp16 product exact, fp32 addend,
+// one rounding), so the only errors are the fp16 roundings of the two factors
 struct Alpha {
-    float al, a16;
+    float al;
+    unsigned short ah;
 };
 __device__ __forceinline__ Alpha make_alpha(float al) {
     Alpha a;
     a.al = al;
-    a.a16 = kAlScale * al;
+    a.ah = f2h_bits(kAlScale * al);
     return a;
 }
 // fp16 -> fp32 as 1.0h * h + 0 on the FMA pipe (FHFMA runs at the full FP32 rate; HADD2.F32 does not)
@@ -467,8 +470,8 @@ __device__ __forceinline__ uint32_t fp24_gather(uint32_t w0, uint32_t w1, uint32
 
 // Four frames (two frame pairs a, b) of a compact entry: w[0..5] = the mid words, dd[0..3] = half2 words
 // [(dr, dr), (di, di)] of pair a then pair b (difference term / 16).
-// Scalar version (generic kernel): v = mid + a16 * d with d converted to fp32 (the fp16 x fp32 product is exact
-// in the FMA), acc += (c + j s) v.  nv = number of valid frames among the four.
+// Scalar version (generic kernel): v = mid + ah * d (one FHFMA per component), acc += (c + j s) v.
+// nv = number of valid frames among the four.
 __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t (&dd)[4], const Alpha &A, float c,
                                           float s, float *accr, float *acci, int nv = 4) {
     const uint32_t re[4] = {w[0], w[1], w[4], w[5]};
@@ -480,8 +483,8 @@ __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t
         unsigned short r0, r1, i0, i1;
         split_h2(dd[2 * p], r0, r1);
         split_h2(dd[2 * p + 1], i0, i1);
-        const float vr = fmaf(A.a16, h2f(h ? r1 : r0), __uint_as_float(re[i]));
-        const float vi = fmaf(A.a16, h2f(h ? i1 : i0), __uint_as_float(im[i]));
+        const float vr = fhfma(A.ah, h ? r1 : r0, __uint_as_float(re[i]));
+        const float vi = fhfma(A.ah, h ? i1 : i0, __uint_as_float(im[i]));
         accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
         acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
     }
@@ -497,32 +500,32 @@ __device__ __forceinline__ unsigned long long pack_u2(uint32_t lo, uint32_t hi) 
 }
 
 // Packed version (ring kernel): m01 / m23 / m45 = the mid words as loaded by three LDS.64 (already the register
-// pairs (re_a0, re_a1), (im_a0, im_a1), (re_b0, re_b1)), da / db = the d words of pairs a / b.  The interpolation
-// and the complex multiply-accumulate of a frame pair run as FFMA2 on (frame 2p, frame 2p+1) register pairs; aR / aI
-// are pairs of real / imaginary accumulators; AA = (a16, a16), CC = (c, c), SS = (s, s), NS = (-s, -s).  Each half is
-// an ordinary round-to-nearest fp32 FMA, so the results are bit-identical to chunk_mac.
+// pairs (re_a0, re_a1), (im_a0, im_a1), (re_b0, re_b1)), da / db = the d words of pairs a / b.  The interpolation is
+// one FHFMA per component and frame, the complex multiply-accumulate of a frame pair runs as FFMA2 on
+// (frame 2p, frame 2p+1) register pairs; aR / aI are pairs of real / imaginary accumulators; CC = (c, c), SS = (s, s),
+// NS = (-s, -s).  Each half is an ordinary round-to-nearest fp32 FMA, so the results are bit-identical to chunk_mac.
 __device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long long m23, unsigned long long m45,
-                                           unsigned long long da, unsigned long long db, unsigned long long AA,
+                                           unsigned long long da, unsigned long long db, unsigned short ah,
                                            unsigned long long CC, unsigned long long SS, unsigned long long NS,
                                            unsigned long long *aR, unsigned long long *aI) {
     uint32_t w0, w1, w2, w3, w4, w5, d0, d1, d2, d3;
     split_u2(m01, w0, w1); split_u2(m23, w2, w3); split_u2(m45, w4, w5);
     split_u2(da, d0, d1); split_u2(db, d2, d3);
-    const unsigned long long m67 = pack_u2(fp24_gather(w0, w1, w2), fp24_gather(w3, w4, w5));
     unsigned short r0, r1, i0, i1;
     {
         split_h2(d0, r0, r1);
         split_h2(d1, i0, i1);
-        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), m01);
-        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), m23);
+        const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w0)), fhfma(ah, r1, __uint_as_float(w1)));
+        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(w2)), fhfma(ah, i1, __uint_as_float(w3)));
         aR[0] = ffma2(CC, VR, aR[0]); aR[0] = ffma2(NS, VI, aR[0]);
         aI[0] = ffma2(SS, VR, aI[0]); aI[0] = ffma2(CC, VI, aI[0]);
     }
     {
         split_h2(d2, r0, r1);
         split_h2(d3, i0, i1);
-        const unsigned long long VR = ffma2(AA, pack_f2(h2f(r0), h2f(r1)), m45);
-        const unsigned long long VI = ffma2(AA, pack_f2(h2f(i0), h2f(i1)), m67);
+        const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w4)), fhfma(ah, r1, __uint_as_float(w5)));
+        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(fp24_gather(w0, w1, w2))),
+                                              fhfma(ah, i1, __uint_as_float(fp24_gather(w3, w4, w5))));
         aR[1] = ffma2(CC, VR, aR[1]); aR[1] = ffma2(NS, VI, aR[1]);
         aI[1] = ffma2(SS, VR, aI[1]); aI[1] = ffma2(CC, VI, aI[1]);
     }

@@ -350,7 +350,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                             b[3] = lds64(a1 + 6u * F + 16u * q1); b[4] = lds64(a1 + 6u * F + 16u * q1 + 8u);
                         }
                         const unsigned long long *b = buf[st & 1];
-                        chunk_mac2(b[0], b[1], b[2], b[3], b[4], pack_f2(cur.A.a16, cur.A.a16), pack_f2(cur.c, cur.c),
+                        chunk_mac2(b[0], b[1], b[2], b[3], b[4], cur.A.ah, pack_f2(cur.c, cur.c),
                                    pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
                         if (q == NQ - 1) cur = nxt;
                     }

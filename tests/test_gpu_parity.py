@@ -14,6 +14,13 @@ from synth import centred_grid
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-4
+# White-noise channel data has no coherent echo, so its image maximum is an incoherent sum and the per-term format
+# error of the compact scratch entries (fp16 difference term and fp16 interpolation weight, <= 2^-12 |d| per term,
+# DESIGN.md section 7) is measured against a maximum ~sqrt(N) times smaller than on echo data.  Every white-noise case
+# is therefore checked twice against the same oracle result: with full entries at NOISE_TOL_FULL (sharp enough to
+# expose any planning / indexing / edge error) and with the entries the plan would pick at NOISE_TOL_COMPACT.
+NOISE_TOL_FULL = 2e-5
+NOISE_TOL_COMPACT = 1.5e-4
 
 
 @pytest.fixture(scope="module")
@@ -36,6 +43,28 @@ def run_pair(torch, cfg, ch, plan_extra=None, **overrides):
         torch.cuda.synchronize()
         info = plan.info()
     return out.cpu().numpy(), ref, info
+
+
+def run_gpu(torch, kw, ch, plan_extra=None):
+    from paper_2511_21647_b200 import Plan
+    with Plan(**kw, **(plan_extra or {})) as plan:
+        out = plan.beamform(torch.from_numpy(np.ascontiguousarray(ch)).cuda())
+        torch.cuda.synchronize()
+        info = plan.info()
+    return out.cpu().numpy(), info
+
+
+def check_noise(torch, cfg, ch, plan_extra=None, **overrides):
+    """White-noise input: full entries at NOISE_TOL_FULL, then the requested plan at its format bound."""
+    kw = rounded_kwargs(cfg, **overrides)
+    ref = oracle.beamform(oracle.OracleParams(**kw), ch)
+    extra = dict(plan_extra or {})
+    full, info_full = run_gpu(torch, kw, ch, dict(extra, precision=2))
+    assert info_full["precision"] == 2
+    assert_parity(full, ref, tol=NOISE_TOL_FULL)
+    gpu, info = run_gpu(torch, kw, ch, extra)
+    assert_parity(gpu, ref, tol=NOISE_TOL_FULL if info["precision"] == 2 else NOISE_TOL_COMPACT)
+    return gpu, ref, info
 
 
 def assert_parity(gpu, ref, tol=TOL):
@@ -105,22 +134,26 @@ def test_small_variants(torch_cuda, kernel, case):
         k = np.array([1, 4, 6, 4, 1], dtype=np.float64) / 16
         sm = np.apply_along_axis(lambda v: np.convolve(v, k, mode="same"), -2, ch.astype(np.float64))
         ch = np.round(sm).astype(np.int16)
-    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel, **extra))
+    gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel, **extra))
     assert info["precision"] == (2 if case in ("iq", "rf_full") else 1)
-    assert_parity(gpu, ref)
 
 
 def test_per_angle_slices(torch_cuda):
     cfg = small(compound=0)
     ch = synth.random_channel(cfg, 2, seed=5, amplitude=6000)
-    gpu, ref, _ = run_pair(torch_cuda, cfg, ch)
-    assert_parity(gpu, ref)
-    # and the slices add up to the compounded images
-    gpu1, ref1, _ = run_pair(torch_cuda, cfg.with_(compound=1), ch)
+    check_noise(torch_cuda, cfg, ch)
+    # and the slices add up to the compounded images (full entries: the ring and the generic kernel differ by fp32
+    # rounding only; with compact entries a delay that differs in the last fp32 bit can round the fp16 weight the
+    # other way, so the two kernels agree to the format bound, not to 1e-5)
     nxz = cfg.grid_xz[0] * cfg.grid_xz[3]
     kr = len(cfg.row_tx_angles)
-    s = gpu[:, :kr * nxz].reshape(2, kr, nxz).sum(1)
-    assert np.abs(s - gpu1[:, :nxz]).max() <= 1e-5 * np.abs(gpu1).max()
+    for precision, bound in [(2, 1e-5), (1, NOISE_TOL_COMPACT)]:
+        kw = rounded_kwargs(cfg)
+        gpu, _ = run_gpu(torch_cuda, kw, ch, dict(precision=precision))
+        gpu1, info1 = run_gpu(torch_cuda, rounded_kwargs(cfg.with_(compound=1)), ch, dict(precision=precision))
+        assert info1["kernel"] == 2
+        s = gpu[:, :kr * nxz].reshape(2, kr, nxz).sum(1)
+        assert np.abs(s - gpu1[:, :nxz]).max() <= bound * np.abs(gpu1).max()
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -128,10 +161,8 @@ def test_batching_and_ragged_frame_counts(torch_cuda, kernel):
     """n_frames > max_frames is processed in batches; odd frame counts leave a ragged last group."""
     cfg = small(n_frames=11)
     ch = synth.random_channel(cfg, 11, seed=23, amplitude=6000)
-    gpu, ref, _ = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=4, kernel=kernel))
-    assert_parity(gpu, ref)
-    gpu, ref, _ = run_pair(torch_cuda, cfg, ch[:1], plan_extra=dict(max_frames=4, kernel=kernel))
-    assert_parity(gpu, ref)
+    check_noise(torch_cuda, cfg, ch, plan_extra=dict(max_frames=4, kernel=kernel))
+    check_noise(torch_cuda, cfg, ch[:1], plan_extra=dict(max_frames=4, kernel=kernel))
 
 
 def test_zero_frames_and_bad_buffers(torch_cuda):
@@ -293,9 +324,8 @@ def test_fallback_to_generic_kernel_when_the_ring_does_not_cover_the_shape(torch
                 col_tx_angles=tuple(np.radians([4.0])), t0=(0.1e-6, -0.1e-6, 0.2e-6),
                 grid_xz=centred_grid(21, d, 17, 6e-3, d), grid_yz=centred_grid(9, d, 13, 6e-3, d))
     ch = synth.random_channel(cfg, 2, seed=3, amplitude=6000)
-    gpu, ref, info = run_pair(torch_cuda, cfg, ch)
+    gpu, ref, info = check_noise(torch_cuda, cfg, ch)
     assert info["kernel"] == 1
-    assert_parity(gpu, ref)
     with pytest.raises(UlmRcaError) as ei:
         Plan(**rounded_kwargs(cfg), kernel=2)
     assert ei.value.status == 4
@@ -306,9 +336,8 @@ def test_many_frames_cross_group_boundaries(torch_cuda):
     cfg = small(n_frames=25)
     ch = synth.random_channel(cfg, 25, seed=29, amplitude=3000)
     ch = (ch.astype(np.int32) + synth.random_channel(cfg, 25, seed=30, amplitude=3000)).astype(np.int16)
-    gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=25))
+    gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(max_frames=25))
     assert info["launches_last_call"] == 2
-    assert_parity(gpu, ref)
 
 
 SWEEP = [
