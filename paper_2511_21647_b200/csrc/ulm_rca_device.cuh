@@ -13,7 +13,7 @@
 // event e, receive element j and sample n the scratch holds ONE compact entry of 10 F bytes:
 //     mid section, 24 B per chunk of 4 frames (frame pairs a, b) of  mid = (iq[n] + iq[n+1]) / 2  as "fp24" = the top
 //       three bytes of the fp32 value (16 mantissa bits): words W0..W5 carry re_a0, re_a1, im_a0, im_a1, re_b0, re_b1 in
-//       their top three bytes; the low bytes of W0, W1, W2 are bytes 3, 2, 1 of im_b0 and those of W3, W4, W5 the same
+//       their top three bytes; the low bytes of W0, W2, W4 are bytes 3, 2, 1 of im_b0 and those of W1, W3, W5 the same
 //       of im_b1 (two PRMT each to reassemble; the six direct values are used as loaded, their low mantissa byte
 //       being a byte of another value, i.e. a zero-mean error below 2^-16 relative)
 //     d section,    8 B per frame pair:  half2 (dr_2p, dr_2p+1), half2 (di_2p, di_2p+1)  of  d/16 = (iq[n+1] - iq[n]) / 16
@@ -106,26 +106,28 @@ __device__ __forceinline__ void store_full_entry(unsigned char *ep, int f, float
     if (f == 0) *reinterpret_cast<uint4 *>(ep + 16 * F) = make_uint4(0u, 0u, 0u, 0u);
 }
 
+// Warp-cooperative: EVERY thread with f < F of the warp must call it for the same entry slot (the threads of a
+// 4-frame chunk are adjacent lanes); `valid` guards the stores only.  Lane i of a chunk (frame 4c + i) holds
+// (re_i, im_i): lanes 0 / 1 write the words W_i = re_i | byte 3 and W_{2+i} = im_i | byte 2 of im_{i+2} (fetched with
+// one shuffle), lanes 2 / 3 write W_{2+i} = re_i | byte 1 of their own im_i -- whole 32-bit stores, no byte stores.
 template <int F>
-__device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16) {
-    const int p = f >> 1, h = f & 1, pc = p & 1;
-    unsigned char *mid = ep + 24 * (p >> 1);                 // the 6 words of this 4-frame chunk
+__device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16,
+                                                    bool valid) {
+    constexpr unsigned kMask = F == 12 ? 0x0FFF0FFFu : 0xFFFFFFFFu;      // lanes with f < F (demod_threads_per_group)
+    const int i = f & 3, p = f >> 1, h = f & 1;
     const uint32_t br = __float_as_uint(mr), bi = __float_as_uint(mi);
-    // direct slots: top three bytes of word s (truncation; the reader sees a foreign low byte, zero-mean)
-    const int sr = pc ? 4 + h : h;
-    mid[4 * sr + 1] = (unsigned char)(br >> 8);
-    *reinterpret_cast<unsigned short *>(mid + 4 * sr + 2) = (unsigned short)(br >> 16);
-    if (pc == 0) {
-        mid[4 * (2 + h) + 1] = (unsigned char)(bi >> 8);
-        *reinterpret_cast<unsigned short *>(mid + 4 * (2 + h) + 2) = (unsigned short)(bi >> 16);
-    } else {                                                 // im of pair b: spread over the low bytes of three words
-        mid[12 * h] = (unsigned char)(bi >> 24);
-        mid[12 * h + 4] = (unsigned char)(bi >> 16);
-        mid[12 * h + 8] = (unsigned char)(bi >> 8);
+    const int lane = threadIdx.x & 31;
+    const uint32_t v = __shfl_sync(kMask, bi, i < 2 ? lane + 2 : lane);   // im of frame 4c + i + 2 (lanes 0, 1) or own
+    uint32_t *mid = reinterpret_cast<uint32_t *>(ep + 24 * (f >> 2));
+    const uint32_t wa = __byte_perm(br, v, i < 2 ? 0x3217 : 0x3215);      // re | v.b3   or   re | own im.b1
+    const uint32_t wb = __byte_perm(bi, v, 0x3216);                       // im | v.b2 (lanes 0, 1)
+    if (valid) {
+        mid[i < 2 ? i : i + 2] = wa;
+        if (i < 2) mid[2 + i] = wb;
+        unsigned short *d = reinterpret_cast<unsigned short *>(ep + 6 * F) + 4 * p + h;
+        d[0] = f2h_bits(dr16);
+        d[2] = f2h_bits(di16);
     }
-    unsigned short *d = reinterpret_cast<unsigned short *>(ep + 6 * F) + 4 * p + h;
-    d[0] = f2h_bits(dr16);
-    d[2] = f2h_bits(di16);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -179,20 +181,24 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
         const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
         const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
         const int fr0 = g * F + h * FH;
-        const long long rec0 = ((long long)fr0 * P.n_events + e) * P.channels_per_event * (long long)P.n_samples +
-                               (long long)ch * P.n_samples;
+        const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+        // record address formed once; the frames are reached by stepping (no per-frame 64-bit products)
+        const long long rec0 = (long long)min(fr0, P.n_frames - 1) * frame_stride +
+                               ((long long)e * P.channels_per_event + ch) * (long long)P.n_samples;
         for (int i = i0; i < XW; i += 128) {
             const int n = base - L + i;
             const bool inb = n >= 0 && n < P.n_samples;
             float2 *dst = s_x + (h * FH) * XS + i;
             // unconditional loads from clamped addresses, all issued before the first use
-            const long long src = rec0 + min(max(n, 0), P.n_samples - 1);
-            const int f_last = min(FH - 1, P.n_frames - 1 - fr0);
+            long long src = rec0 + min(max(n, 0), P.n_samples - 1);
             float re[FH], im[FH];
             if (IQ_INPUT) {
                 short2 q[FH];
 #pragma unroll
-                for (int f = 0; f < FH; ++f) q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src + min(f, f_last) * frame_stride);
+                for (int f = 0; f < FH; ++f) {
+                    q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src);
+                    if (f < f_last) src += frame_stride;
+                }
 #pragma unroll
                 for (int f = 0; f < FH; ++f) {
                     const bool ok = inb && f <= f_last;
@@ -201,7 +207,10 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
             } else {
                 int q[FH];
 #pragma unroll
-                for (int f = 0; f < FH; ++f) q[f] = __ldg(P.rf + src + min(f, f_last) * frame_stride);
+                for (int f = 0; f < FH; ++f) {
+                    q[f] = __ldg(P.rf + src);
+                    if (f < f_last) src += frame_stride;
+                }
 #pragma unroll
                 for (int f = 0; f < FH; ++f) { re[f] = (inb && f <= f_last) ? (float)q[f] : 0.f; im[f] = 0.f; }
             }
@@ -217,7 +226,9 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     // (2) FIR: iq[base + r] = sum_{i = r .. r + 2L} gd[r + 2L - i] x[i]   (x index relative to base - L)
     const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
     const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
-    if (f < F && grp * R < n_ent) {
+    // every lane with f < F of a warp that holds at least one valid entry runs the whole loop (the compact store is
+    // warp-cooperative); entries past n_ent are computed from whatever the staging buffer holds and never stored
+    if (f < F && ((threadIdx.x & ~31) / TPG) * R < n_ent) {
         const int r0 = grp * R;
         const float2 *x = s_x + f * XS + r0;
         float ar[R + 1], ai[R + 1];
@@ -252,16 +263,16 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
 #pragma unroll
         for (int q = 0; q < R; ++q) {
             const int ent = r0 + q;
-            if (ent >= n_ent) break;
+            const bool valid = ent < n_ent;
             const int n = base + ent;
             const bool ok = n >= 0 && n + 1 <= P.n_samples - 1;      // edge rule: both taps inside the record
             const float mr = ok ? 0.5f * (ar[q] + ar[q + 1]) : 0.f, mi = ok ? 0.5f * (ai[q] + ai[q + 1]) : 0.f;
             const float dr = ok ? ar[q + 1] - ar[q] : 0.f, di = ok ? ai[q + 1] - ai[q] : 0.f;
             unsigned char *ep = s_out + ent * EB;
             if (D32) {
-                store_full_entry<F>(ep, f, mr, mi, dr, di);
+                if (valid) store_full_entry<F>(ep, f, mr, mi, dr, di);
             } else {
-                store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di);
+                store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di, valid);
             }
         }
     }
@@ -308,7 +319,7 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
         const int ent = r0 + q;
-        if (ent >= n_ent) break;
+        const bool valid = ent < n_ent;
         const int n = base + ent;
         const bool ok = n >= 0 && n + 1 <= n_samples - 1;      // edge rule: both taps inside the record
         const float2 a = quad_rot(PB + q, A[q], B[q]), b = quad_rot(PB + q + 1, A[q + 1], B[q + 1]);   // halved iq[n], iq[n+1]
@@ -316,9 +327,9 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
         const float dr = ok ? b.x - a.x : 0.f, di = ok ? b.y - a.y : 0.f;                              // = (d)/2
         unsigned char *ep = s_out + ent * EB;
         if (D32) {
-            store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
+            if (valid) store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
         } else {
-            store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di);
+            store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di, valid);
         }
     }
 }
@@ -343,13 +354,15 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
     const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
     const int base = P.n_lo + chunk * kDemodChunk;
 
-    // (1) raw samples as float: half h of the CTA takes frames [h FH, (h+1) FH), a thread takes samples i0, i0 + 128
+    // (1) raw samples as float: half h of the CTA takes frames [h FH, (h+1) FH), a thread takes samples i0, i0 + 128.
+    // The record address is formed once; the frames are reached by stepping a pointer (no per-frame 64-bit products).
     {
         const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
         const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
         const int fr0 = g * F + h * FH;
-        const int16_t *rec = P.rf + ((long long)fr0 * P.n_events + e) * P.channels_per_event * (long long)P.n_samples +
-                             (long long)ch * P.n_samples;
+        const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+        const int16_t *rec = P.rf + (long long)min(fr0, P.n_frames - 1) * frame_stride +
+                             ((long long)e * P.channels_per_event + ch) * (long long)P.n_samples;
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
             const int i = i0 + rep * 128;
@@ -360,10 +373,12 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
                 // unconditional loads from clamped addresses, all issued before the first use (out-of-range
                 // samples and frames are zeroed afterwards)
                 const int16_t *src = rec + min(max(n, 0), P.n_samples - 1);
-                const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // >= 0: the group has at least one frame
                 int raw[FH];
 #pragma unroll
-                for (int f = 0; f < FH; ++f) raw[f] = __ldg(src + min(f, f_last) * frame_stride);
+                for (int f = 0; f < FH; ++f) {
+                    raw[f] = __ldg(src);
+                    if (f < f_last) src += frame_stride;
+                }
 #pragma unroll
                 for (int f = 0; f < FH; ++f) dst[f * XS] = (inb && f <= f_last) ? (float)raw[f] : 0.f;
             }
@@ -374,7 +389,9 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
     // (2) real FIRs A, B for 9 consecutive outputs, rotation, mid / d into the output image
     const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
     const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
-    if (f < F && grp * 8 < n_ent) {
+    // every lane with f < F of a warp that holds at least one valid entry runs the whole loop (the compact store is
+    // warp-cooperative); entries past n_ent are computed from whatever the staging buffer holds and never stored
+    if (f < F && ((threadIdx.x & ~31) / TPG) * 8 < n_ent) {
         const int r0 = grp * 8;
         const float *x = s_x + f * XS + r0 + (r0 >> 1);         // r0 + 4 (r0 >> 3)
         float A[9], B[9];
@@ -475,7 +492,7 @@ __device__ __forceinline__ uint32_t fp24_gather(uint32_t w0, uint32_t w1, uint32
 __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t (&dd)[4], const Alpha &A, float c,
                                           float s, float *accr, float *acci, int nv = 4) {
     const uint32_t re[4] = {w[0], w[1], w[4], w[5]};
-    const uint32_t im[4] = {w[2], w[3], fp24_gather(w[0], w[1], w[2]), fp24_gather(w[3], w[4], w[5])};
+    const uint32_t im[4] = {w[2], w[3], fp24_gather(w[0], w[2], w[4]), fp24_gather(w[1], w[3], w[5])};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         if (i >= nv) break;
@@ -524,8 +541,8 @@ __device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long
         split_h2(d2, r0, r1);
         split_h2(d3, i0, i1);
         const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w4)), fhfma(ah, r1, __uint_as_float(w5)));
-        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(fp24_gather(w0, w1, w2))),
-                                              fhfma(ah, i1, __uint_as_float(fp24_gather(w3, w4, w5))));
+        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(fp24_gather(w0, w2, w4))),
+                                              fhfma(ah, i1, __uint_as_float(fp24_gather(w1, w3, w5))));
         aR[1] = ffma2(CC, VR, aR[1]); aR[1] = ffma2(NS, VI, aR[1]);
         aI[1] = ffma2(SS, VR, aI[1]); aI[1] = ffma2(CC, VI, aI[1]);
     }
