@@ -16,10 +16,10 @@
 //       their top three bytes; the low bytes of W0, W2, W4 are bytes 3, 2, 1 of im_b0 and those of W1, W3, W5 the same
 //       of im_b1 (two PRMT each to reassemble; the six direct values are used as loaded, their low mantissa byte
 //       being a byte of another value, i.e. a zero-mean error below 2^-16 relative)
-//     d section,    8 B per frame pair:  half2 (dr_2p, dr_2p+1), half2 (di_2p, di_2p+1)  of  d/16 = (iq[n+1] - iq[n]) / 16
+//     d section,    4 B per frame:  half2 (dr, di)  of  d/16 = (iq[n+1] - iq[n]) / 16
 // so that the interpolated sample is mid + a' d with a' = a - 0.5 in [-0.5, 0.5]: the value carries 17 significant
-// bits, only the small difference term is fp16, and every LDS.64 delivers an aligned (frame 2p, frame 2p+1)
-// register pair for the packed fp32x2 FMA (FFMA2).  "Full" entries keep mid and d in fp32 (16 F + 16 bytes, LDS.128).
+// bits, only the small difference term is fp16, and every LDS.64 of the mid section delivers an aligned
+// (frame 2p, frame 2p+1) register pair for the packed fp32x2 FMA (FFMA2).  "Full" entries keep mid and d in fp32 (16 F + 16 bytes, LDS.128).
 // Compact entry sizes 40 / 120 B are odd multiples of 8 B: the LDS.64 gathers of the 16 lanes of a half-warp fall into
 // 16 different bank pairs whenever their entries differ; full entry sizes 80 / 208 B are odd multiples of 16 B.
 #pragma once
@@ -36,6 +36,7 @@ constexpr int kMaxTaps = 129;
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kDScale = 0.0625f;           // d is stored / 16 (|d| can exceed the fp16 range) ...
 constexpr float kAlScale = 16.0f;            // ... and a' is multiplied by 16 before it is rounded to fp16
+constexpr int kDemodSlots = 128;             // entry slots of the shared-memory image of a chunk (16 thread groups x 8)
 constexpr int kDemodChunk = 126;             // entries per demodulation CTA (even: every chunk of 10 F-byte entries starts 16-byte aligned)
 
 // D32 = false: compact entries (fp24 mid + fp16 difference term, 10 F bytes); true: full entries (fp32 mid and
@@ -90,8 +91,8 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
 }
 
 // Compact-entry store of one frame's (mid, d/16) in the layout described at the top of this file (fp24 mid words
-// per 4-frame chunk, then the half2 words [(dr_2p, dr_2p+1), (di_2p, di_2p+1)] per frame pair), so that the DAS
-// kernels read aligned (frame 2p, frame 2p+1) register pairs for FFMA2.
+// per 4-frame chunk, then one half2 word (dr, di) per frame), so that the DAS kernels read aligned
+// (frame 2p, frame 2p+1) register pairs for FFMA2.
 // Full-entry store of one frame: the same frame-pair layout with fp32 differences,
 // mid: [re_2p, re_2p+1, im_2p, im_2p+1], then d: [dr_2p, dr_2p+1, di_2p, di_2p+1], then 16 bytes of padding.
 template <int F>
@@ -107,26 +108,35 @@ __device__ __forceinline__ void store_full_entry(unsigned char *ep, int f, float
 }
 
 // Warp-cooperative: EVERY thread with f < F of the warp must call it for the same entry slot (the threads of a
-// 4-frame chunk are adjacent lanes); `valid` guards the stores only.  Lane i of a chunk (frame 4c + i) holds
+// 4-frame chunk are adjacent lanes).  Lane i of a chunk (frame 4c + i) holds
 // (re_i, im_i): lanes 0 / 1 write the words W_i = re_i | byte 3 and W_{2+i} = im_i | byte 2 of im_{i+2} (fetched with
 // one shuffle), lanes 2 / 3 write W_{2+i} = re_i | byte 1 of their own im_i -- whole 32-bit stores, no byte stores.
 template <int F>
-__device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16,
-                                                    bool valid) {
+__device__ __forceinline__ void store_compact_entry(unsigned char *ep, int f, float mr, float mi, float dr16, float di16) {
     constexpr unsigned kMask = F == 12 ? 0x0FFF0FFFu : 0xFFFFFFFFu;      // lanes with f < F (demod_threads_per_group)
-    const int i = f & 3, p = f >> 1, h = f & 1;
+    const int i = f & 3;
     const uint32_t br = __float_as_uint(mr), bi = __float_as_uint(mi);
     const int lane = threadIdx.x & 31;
     const uint32_t v = __shfl_sync(kMask, bi, i < 2 ? lane + 2 : lane);   // im of frame 4c + i + 2 (lanes 0, 1) or own
     uint32_t *mid = reinterpret_cast<uint32_t *>(ep + 24 * (f >> 2));
     const uint32_t wa = __byte_perm(br, v, i < 2 ? 0x3217 : 0x3215);      // re | v.b3   or   re | own im.b1
     const uint32_t wb = __byte_perm(bi, v, 0x3216);                       // im | v.b2 (lanes 0, 1)
-    if (valid) {
-        mid[i < 2 ? i : i + 2] = wa;
-        if (i < 2) mid[2 + i] = wb;
-        unsigned short *d = reinterpret_cast<unsigned short *>(ep + 6 * F) + 4 * p + h;
-        d[0] = f2h_bits(dr16);
-        d[2] = f2h_bits(di16);
+    mid[i < 2 ? i : i + 2] = wa;
+    if (i < 2) mid[2 + i] = wb;
+    reinterpret_cast<uint32_t *>(ep + 6 * F)[f] = pack_h2(dr16, di16);
+}
+
+// Edge rule of the interpolation (a term is 0 unless 0 <= n and n + 1 <= Ns - 1), applied to the
+// shared-memory image of a chunk after it is written: entries whose two taps are not both inside the record are
+// zeroed (all-zero words are zeros in every entry format).  Only the chunks that touch an end of the record do any
+// work here.  Must be called by all threads of the CTA.
+__device__ __forceinline__ void zero_edge_entries(unsigned char *s_out, int eb, int n_ent, int base, int n_samples) {
+    if (base >= 0 && base + n_ent <= n_samples - 1) return;     // block-uniform
+    __syncthreads();
+    const int words = eb / 4;
+    for (int idx = threadIdx.x; idx < n_ent * words; idx += blockDim.x) {
+        const int n = base + idx / words;
+        if (!(n >= 0 && n + 1 <= n_samples - 1)) reinterpret_cast<uint32_t *>(s_out)[idx] = 0u;
     }
 }
 
@@ -148,14 +158,14 @@ __constant__ DemodConst c_demod[1];
 __host__ __device__ constexpr int demod_threads_per_group(int F) { return F == 12 ? 16 : F; }
 __host__ __device__ inline int demod_xs(int L) { return ((kDemodChunk + 2 + 2 * L) + 14) / 16 * 16 + 1; }
 __host__ __device__ inline int demod_smem_bytes(int F, bool D32, int L) {
-    return (kDemodChunk * entry_bytes(F, D32) + 127) / 128 * 128 + F * demod_xs(L) * 8;
+    return kDemodSlots * entry_bytes(F, D32) + F * demod_xs(L) * 8;
 }
 
 template <int NT, bool HB, bool IQ_INPUT, int F, bool D32>
 __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
-    constexpr int OUT_BYTES = (kDemodChunk * EB + 127) / 128 * 128;
+    constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
     constexpr int R = 8;                       // entries per thread
     constexpr int TPG = demod_threads_per_group(F);
     const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
@@ -262,21 +272,19 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
         }
 #pragma unroll
         for (int q = 0; q < R; ++q) {
-            const int ent = r0 + q;
-            const bool valid = ent < n_ent;
-            const int n = base + ent;
-            const bool ok = n >= 0 && n + 1 <= P.n_samples - 1;      // edge rule: both taps inside the record
-            const float mr = ok ? 0.5f * (ar[q] + ar[q + 1]) : 0.f, mi = ok ? 0.5f * (ai[q] + ai[q + 1]) : 0.f;
-            const float dr = ok ? ar[q + 1] - ar[q] : 0.f, di = ok ? ai[q + 1] - ai[q] : 0.f;
+            const int ent = r0 + q;               // < kDemodSlots: slots past n_ent are written but never copied out
+            const float mr = 0.5f * (ar[q] + ar[q + 1]), mi = 0.5f * (ai[q] + ai[q + 1]);
+            const float dr = ar[q + 1] - ar[q], di = ai[q + 1] - ai[q];
             unsigned char *ep = s_out + ent * EB;
             if (D32) {
-                if (valid) store_full_entry<F>(ep, f, mr, mi, dr, di);
+                store_full_entry<F>(ep, f, mr, mi, dr, di);
             } else {
-                store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di, valid);
+                store_compact_entry<F>(ep, f, mr, mi, kDScale * dr, kDScale * di);
             }
         }
     }
     // (3) one bulk store of the block: generic-proxy writes -> async proxy, then TMA shared -> global
+    zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -299,7 +307,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ constexpr int demod_quad_xs() { return 225; }    // >= 1.5 * 145 + 4, = 1 mod 32 (words)
 __host__ __device__ inline int demod_quad_smem_bytes(int F, bool D32) {
-    return (kDemodChunk * entry_bytes(F, D32) + 127) / 128 * 128 + F * demod_quad_xs() * 4;
+    return kDemodSlots * entry_bytes(F, D32) + F * demod_quad_xs() * 4;
 }
 
 // rotation by (-j)^p of A + jB
@@ -313,23 +321,20 @@ __device__ __forceinline__ float2 quad_rot(int p, float A, float B) {
 }
 
 template <int PB, int F, bool D32>
-__device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float (&B)[9], int r0, int n_ent, int base,
-                                                int n_samples, int f, unsigned char *s_out) {
+__device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float (&B)[9], int r0, int f,
+                                                unsigned char *s_out) {
     constexpr int EB = entry_bytes(F, D32);
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-        const int ent = r0 + q;
-        const bool valid = ent < n_ent;
-        const int n = base + ent;
-        const bool ok = n >= 0 && n + 1 <= n_samples - 1;      // edge rule: both taps inside the record
+        const int ent = r0 + q;                   // < kDemodSlots: slots past n_ent are written but never copied out
         const float2 a = quad_rot(PB + q, A[q], B[q]), b = quad_rot(PB + q + 1, A[q + 1], B[q + 1]);   // halved iq[n], iq[n+1]
-        const float mr = ok ? a.x + b.x : 0.f, mi = ok ? a.y + b.y : 0.f;
-        const float dr = ok ? b.x - a.x : 0.f, di = ok ? b.y - a.y : 0.f;                              // = (d)/2
+        const float mr = a.x + b.x, mi = a.y + b.y;
+        const float dr = b.x - a.x, di = b.y - a.y;                                                    // = (d)/2
         unsigned char *ep = s_out + ent * EB;
         if (D32) {
-            if (valid) store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
+            store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
         } else {
-            store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di, valid);
+            store_compact_entry<F>(ep, f, mr, mi, 2.f * kDScale * dr, 2.f * kDScale * di);
         }
     }
 }
@@ -338,7 +343,7 @@ template <int F, bool D32>
 __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
-    constexpr int OUT_BYTES = (kDemodChunk * EB + 127) / 128 * 128;
+    constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
     constexpr int L = 8, XW = kDemodChunk + 2 + 2 * L, XS = demod_quad_xs();
     constexpr int TPG = demod_threads_per_group(F), FH = F / 2;
     unsigned char *s_out = s_raw;
@@ -409,12 +414,13 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
         }
         const int pb = (base + r0 + c_demod[0].q0) & 3;          // (-j)^(n + q0) at the first output
         switch (pb) {
-            case 0: demod_quad_emit<0, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
-            case 1: demod_quad_emit<1, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
-            case 2: demod_quad_emit<2, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
-            default: demod_quad_emit<3, F, D32>(A, B, r0, n_ent, base, P.n_samples, f, s_out); break;
+            case 0: demod_quad_emit<0, F, D32>(A, B, r0, f, s_out); break;
+            case 1: demod_quad_emit<1, F, D32>(A, B, r0, f, s_out); break;
+            case 2: demod_quad_emit<2, F, D32>(A, B, r0, f, s_out); break;
+            default: demod_quad_emit<3, F, D32>(A, B, r0, f, s_out); break;
         }
     }
+    zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -485,8 +491,8 @@ __device__ __forceinline__ uint32_t fp24_gather(uint32_t w0, uint32_t w1, uint32
     return __byte_perm(__byte_perm(w0, w1, 0x0400), w2, 0x3245);
 }
 
-// Four frames (two frame pairs a, b) of a compact entry: w[0..5] = the mid words, dd[0..3] = half2 words
-// [(dr, dr), (di, di)] of pair a then pair b (difference term / 16).
+// Four frames (two frame pairs a, b) of a compact entry: w[0..5] = the mid words, dd[0..3] = the half2 words (dr, di)
+// of the four frames (difference term / 16).
 // Scalar version (generic kernel): v = mid + ah * d (one FHFMA per component), acc += (c + j s) v.
 // nv = number of valid frames among the four.
 __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t (&dd)[4], const Alpha &A, float c,
@@ -496,12 +502,10 @@ __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         if (i >= nv) break;
-        const int p = i >> 1, h = i & 1;
-        unsigned short r0, r1, i0, i1;
-        split_h2(dd[2 * p], r0, r1);
-        split_h2(dd[2 * p + 1], i0, i1);
-        const float vr = fhfma(A.ah, h ? r1 : r0, __uint_as_float(re[i]));
-        const float vi = fhfma(A.ah, h ? i1 : i0, __uint_as_float(im[i]));
+        unsigned short dr, di;
+        split_h2(dd[i], dr, di);
+        const float vr = fhfma(A.ah, dr, __uint_as_float(re[i]));
+        const float vi = fhfma(A.ah, di, __uint_as_float(im[i]));
         accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
         acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
     }
@@ -530,16 +534,16 @@ __device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long
     split_u2(da, d0, d1); split_u2(db, d2, d3);
     unsigned short r0, r1, i0, i1;
     {
-        split_h2(d0, r0, r1);
-        split_h2(d1, i0, i1);
+        split_h2(d0, r0, i0);
+        split_h2(d1, r1, i1);
         const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w0)), fhfma(ah, r1, __uint_as_float(w1)));
         const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(w2)), fhfma(ah, i1, __uint_as_float(w3)));
         aR[0] = ffma2(CC, VR, aR[0]); aR[0] = ffma2(NS, VI, aR[0]);
         aI[0] = ffma2(SS, VR, aI[0]); aI[0] = ffma2(CC, VI, aI[0]);
     }
     {
-        split_h2(d2, r0, r1);
-        split_h2(d3, i0, i1);
+        split_h2(d2, r0, i0);
+        split_h2(d3, r1, i1);
         const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w4)), fhfma(ah, r1, __uint_as_float(w5)));
         const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(fp24_gather(w0, w2, w4))),
                                               fhfma(ah, i1, __uint_as_float(fp24_gather(w1, w3, w5))));
