@@ -62,7 +62,7 @@ struct Grid {
 // transmit-side tables of one aperture for a list of reference coordinates ("planes")
 struct TxTables {
     int n_planes = 0;
-    DeviceBuf n0, f0m, ph0, tph;
+    DeviceBuf n0, f0m;
 };
 
 struct Aperture {
@@ -93,7 +93,7 @@ struct ulm_rca_plan {
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
     bool d32 = false;             // full (fp32) difference term in the scratch
-    bool quad = false;            // fs = 4 fc exactly, default 17 taps, mixer = (-j)^(n + q0): real-arithmetic pre-pass
+    bool quad = false;            // fs = 4 fc exactly, default 17 taps, analytic signal from two real filters
     bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
@@ -152,8 +152,7 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
                             TxTables &T) {
     const size_t n = refs.size() * (size_t)A.n_tx * A.g.n_ax;
     std::vector<int> n0(n);
-    std::vector<float> f0m(n), ph0(n);
-    std::vector<float2> tph(n);
+    std::vector<float> f0m(n);
     size_t i = 0;
     for (double ref : refs)
         for (int k = 0; k < A.n_tx; ++k)
@@ -162,20 +161,11 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
                 const double fl = std::floor(u0);
                 n0[i] = (int)fl - P.n_lo;
                 f0m[i] = (float)(u0 - fl - 0.5);
-                // phase of the full delay in cycles: (fc/fs) u + fc t_start, u = n0_abs + 0.5 + (f0m + H)
-                const double cyc = (P.fc / P.fs) * (fl + 0.5) + P.fc * P.t_start;
-                ph0[i] = (float)(cyc - std::floor(cyc));
-                // transmit phasor of the ring kernel: exp(j 2 pi (fc/fs U0 + fc t_start))
-                double cu = (P.fc / P.fs) * u0 + P.fc * P.t_start;
-                cu -= std::floor(cu);
-                tph[i] = make_float2((float)std::cos(2 * M_PI * cu), (float)std::sin(2 * M_PI * cu));
             }
     T.n_planes = (int)refs.size();
     cudaError_t e;
     if ((e = T.n0.upload(n0)) != cudaSuccess) return e;
-    if ((e = T.f0m.upload(f0m)) != cudaSuccess) return e;
-    if ((e = T.tph.upload(tph)) != cudaSuccess) return e;
-    return T.ph0.upload(ph0);
+    return T.f0m.upload(f0m);
 }
 
 ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
@@ -204,11 +194,9 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
     P.half_band = true;
     for (int t = 0; t <= 2 * L; ++t)
         if (t != L && ((t - L) & 1) == 0 && D.gd[t] != 0.f) P.half_band = false;
-    // quadrature sampling: fs = 4 fc exactly and fc t_start a multiple of 1/4 cycle
-    const double q4 = 4.0 * P.fc * P.t_start;
-    P.quad = P.half_band && L == 8 && P.fs == 4.0 * P.fc && std::fabs(q4 - std::round(q4)) < 1e-9 && std::fabs(q4) < 1e9;
+    // quadrature sampling: fs = 4 fc exactly (the analytic signal needs no mixer, so any t_start qualifies)
+    P.quad = P.half_band && L == 8 && P.fs == 4.0 * P.fc;
     if (P.quad) {
-        D.q0 = (int)(((long long)std::llround(q4) % 4 + 4) % 4);
         for (int t = 0; t <= 2 * L; ++t) {
             const int m = t - L;
             const int m4 = ((m % 4) + 4) % 4;
@@ -257,7 +245,7 @@ ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTabl
     D.xm = A.xm.as<float>(); D.zm = A.zm.as<float>(); D.ejm = A.ejm.as<float>();
     D.win = A.win.as<float>();
     D.two_f = (float)(2.0 * P.f_number);
-    D.n0 = T.n0.as<int>(); D.f0m = T.f0m.as<float>(); D.ph0 = T.ph0.as<float>();
+    D.n0 = T.n0.as<int>(); D.f0m = T.f0m.as<float>();
     D.fcfs = (float)(P.fc / P.fs);
     D.n_planes = T.n_planes;
     return D;
@@ -447,7 +435,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
 
     if (ulm_rca_status s = build_demod(P, opt->demod_taps)) return s;
     CUDA_TRY(cudaMemcpyToSymbol(ulm::c_demod, &P.demod, sizeof(P.demod)));
-    if (P.input_kind == 0) {
+    {   // exp(-j 2 pi fc t_n): mixes RF input down; its conjugate rho_n rotates every scratch entry (both input kinds)
         P.mix_n0 = P.n_lo - P.half_len;
         const int n_mix = P.l_row + 2 * P.half_len + 264;
         std::vector<float2> mix(n_mix);
@@ -564,7 +552,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
                 R.e0 = A.e0; R.n_tx = A.n_tx; R.n_rx = A.n_rx; R.n_lat = A.g.n_lat; R.n_ax = A.g.n_ax;
                 R.xs = A.xs.as<float>(); R.zs = A.zs.as<float>(); R.ejs = A.ejs.as<float>();
                 R.xm = A.xm.as<float>(); R.zm = A.zm.as<float>(); R.ejm = A.ejm.as<float>(); R.win = A.win.as<float>();
-                R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>(); R.tph = A.proj.tph.as<float2>();
+                R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
                 R.out_base = A.out_base;
             }
             P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, group_frames(nb), P.d32, P.apod, st);

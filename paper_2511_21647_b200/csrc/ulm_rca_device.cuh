@@ -8,6 +8,12 @@
 //     H  = (sqrt(dx^2 + z^2) - z) fs/c = dx_s^2 / (sqrt(dx_s^2 + z_s^2) + z_s)   -- device, fp32, <= ~400
 //   so no fp32 quantity ever carries the full ~1300-sample delay.  floor(u) is taken with the
 //   add-magic-constant trick on (u - 0.5).
+//   Phase rotation: exp(j 2 pi fc tau) with tau = t_n + a / fs (n = floor(u), a = u - n) factors into
+//   rho_n = exp(j 2 pi fc t_n), which depends on the sample only and is applied ONCE by the pre-pass to the
+//   scratch entry of sample n, and E(a) = exp(j 2 pi (fc/fs) a), a in [0, 1], the only phasor the DAS kernels
+//   evaluate (per pixel, element and angle; shared by all frames).  With th = 2 pi fc / fs:
+//     term = E(a) [ (1 - a) A_n + a B_n ],   A_n = iq[n] rho_n = s[n],   B_n = iq[n+1] rho_n = s[n+1] exp(-j th),
+//   s = the analytic RF signal.  Entries hold mid = (A_n + B_n)/2 and d = B_n - A_n.
 //
 // IQ scratch ("entries"): frames are processed in groups of F (4 or 12) and paired (2p, 2p+1).  For frame group g,
 // event e, receive element j and sample n the scratch holds ONE compact entry of 10 F bytes:
@@ -48,13 +54,12 @@ struct DemodConst {
     int half_len;            // L
     float gd[kMaxTaps];      // dense taps: gd[t] = 2 h[t - L], t = 0..2L   ({1} for IQ input)
     float qd[17];            // quadrature path (fs = 4 fc, L = 8): qd[8] = h[0], qd[t] = h[m] j^(m-1) for odd m = t - 8
-    int q0;                  // quadrature path: mixer[n] = (-j)^(n + q0)
 };
 
 struct DemodParams {
     const int16_t *rf;       // [frame][event][channel][sample] (x2 for IQ input)
     unsigned char *iq;       // entries: [group][event][rx elem (n_rx_max)][l_row][entry_bytes(F, D32)]
-    const float2 *mixer;     // exp(-j 2 pi fc t_n) for n = mix_n0 .. (RF input only)
+    const float2 *mixer;     // exp(-j 2 pi fc t_n) for n = mix_n0 ..  (mixing of RF input; its conjugate is rho_n)
     int mix_n0;
     int n_frames, n_events, channels_per_event, n_samples;
     int n_row_tx, n_rows, n_cols, n_rx_max;
@@ -273,8 +278,12 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
 #pragma unroll
         for (int q = 0; q < R; ++q) {
             const int ent = r0 + q;               // < kDemodSlots: slots past n_ent are written but never copied out
-            const float mr = 0.5f * (ar[q] + ar[q + 1]), mi = 0.5f * (ai[q] + ai[q + 1]);
-            const float dr = ar[q + 1] - ar[q], di = ai[q + 1] - ai[q];
+            const float m0r = 0.5f * (ar[q] + ar[q + 1]), m0i = 0.5f * (ai[q] + ai[q + 1]);
+            const float d0r = ar[q + 1] - ar[q], d0i = ai[q + 1] - ai[q];
+            // rotate by rho_n = conj(mixer[n]) (one broadcast load per entry: all frames share n)
+            const float2 mx = __ldg(P.mixer + (base + ent - P.mix_n0));
+            const float mr = fmaf(m0r, mx.x, m0i * mx.y), mi = fmaf(m0i, mx.x, -m0r * mx.y);
+            const float dr = fmaf(d0r, mx.x, d0i * mx.y), di = fmaf(d0i, mx.x, -d0r * mx.y);
             unsigned char *ep = s_out + ent * EB;
             if (D32) {
                 store_full_entry<F>(ep, f, mr, mi, dr, di);
@@ -298,11 +307,11 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Quadrature-sampled variant of the pre-pass (RF input, fs = 4 fc exactly, default 17-tap filter): the mixer
-// is (-j)^(n + q0), so  iq[n] = (-j)^(n + q0) (A + j B)  with the REAL filters  A = g[0] rf[n],
+// Quadrature-sampled variant of the pre-pass (RF input, fs = 4 fc exactly, default 17-tap filter): the analytic
+// signal is  s[n] = iq[n] rho_n = A + j B  with the REAL filters  A = g[0] rf[n],
 // B = sum_{m odd} g[m] j^(m-1) rf[n-m]  (the even taps of the half-band filter are exactly zero): 9 real FMAs
-// per output instead of 34 complex ones, and the rotation is a compile-time swap/negation.  The taps are
-// stored halved (qd = g/2) so that mid = a' + b' and d/16 = (b' - a')/8 need no further scaling.
+// per output instead of 34 complex ones, no mixer and no rotation at all (A_n = s[n], B_n = s[n+1] (-j) = B' - jA').
+// The taps are stored halved (qd = g/2) so that mid = a' + b' and d/16 = (b' - a')/8 need no further scaling.
 // Same CTA decomposition, shared-memory image and TMA store as demod_kernel.
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ constexpr int demod_quad_xs() { return 225; }    // >= 1.5 * 145 + 4, = 1 mod 32 (words)
@@ -310,26 +319,16 @@ __host__ __device__ inline int demod_quad_smem_bytes(int F, bool D32) {
     return kDemodSlots * entry_bytes(F, D32) + F * demod_quad_xs() * 4;
 }
 
-// rotation by (-j)^p of A + jB
-__device__ __forceinline__ float2 quad_rot(int p, float A, float B) {
-    switch (p & 3) {
-        case 0: return make_float2(A, B);
-        case 1: return make_float2(B, -A);
-        case 2: return make_float2(-A, -B);
-        default: return make_float2(-B, A);
-    }
-}
-
-template <int PB, int F, bool D32>
+template <int F, bool D32>
 __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float (&B)[9], int r0, int f,
                                                 unsigned char *s_out) {
     constexpr int EB = entry_bytes(F, D32);
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
         const int ent = r0 + q;                   // < kDemodSlots: slots past n_ent are written but never copied out
-        const float2 a = quad_rot(PB + q, A[q], B[q]), b = quad_rot(PB + q + 1, A[q + 1], B[q + 1]);   // halved iq[n], iq[n+1]
-        const float mr = a.x + b.x, mi = a.y + b.y;
-        const float dr = b.x - a.x, di = b.y - a.y;                                                    // = (d)/2
+        // halved A_n = s[n] = A + jB and B_n = s[n+1] exp(-j pi/2) = B' - jA'
+        const float mr = A[q] + B[q + 1], mi = B[q] - A[q + 1];
+        const float dr = B[q + 1] - A[q], di = -A[q + 1] - B[q];                                       // = (d)/2
         unsigned char *ep = s_out + ent * EB;
         if (D32) {
             store_full_entry<F>(ep, f, mr, mi, 2.f * dr, 2.f * di);
@@ -412,13 +411,7 @@ __global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
                 else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(c_demod[0].qd[t], xv, B[q]);
             }
         }
-        const int pb = (base + r0 + c_demod[0].q0) & 3;          // (-j)^(n + q0) at the first output
-        switch (pb) {
-            case 0: demod_quad_emit<0, F, D32>(A, B, r0, f, s_out); break;
-            case 1: demod_quad_emit<1, F, D32>(A, B, r0, f, s_out); break;
-            case 2: demod_quad_emit<2, F, D32>(A, B, r0, f, s_out); break;
-            default: demod_quad_emit<3, F, D32>(A, B, r0, f, s_out); break;
-        }
+        demod_quad_emit<F, D32>(A, B, r0, f, s_out);
     }
     zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -444,7 +437,6 @@ struct DasParams {
     float two_f;                     // 2 * f_number (0 = no mask)
     const int *n0;                   // [plane][k][iz]  floor(U0) - n_lo
     const float *f0m;                // [plane][k][iz]  U0 - floor(U0) - 0.5
-    const float *ph0;                // [plane][k][iz]  cycles
     float fcfs;
     float2 *out;                     // frame 0 of this batch
     long long out_frame_stride;      // float2 per frame
@@ -647,7 +639,7 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             const float al = upm - (tt - kMagic);
             const int idx = P.n0[t] + (__float_as_int(tt) - kMagicBits);
             float s, c;
-            sincos_cycles(fmaf(P.fcfs, upm, P.ph0[t]), s, c);
+            __sincosf(fmaf(kTwoPi * P.fcfs, al, 0.5f * kTwoPi * P.fcfs), &s, &c);     // E(a), a = al + 0.5 in [0, 1]
             if (APOD) { s *= w; c *= w; }
             const unsigned char *ent = P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32);
             entry_mac<F, D32>(ent, make_alpha(al), c, s, accr, acci, nv);

@@ -7,10 +7,10 @@
 // brought from the IQ scratch into a shared-memory ring by one elected producer thread with one
 // cp.async.bulk (TMA, SASS UBLKCP) completing on an mbarrier; 12 consumer warps gather from it.
 // Everything that does not depend on the frame -- receive delay H(p, j), sample index, interpolation
-// weight, phase rotation, apodisation -- is computed once per (pixel, j, k) and reused for the F frames,
-// whose accumulators stay in registers; the angle sum is taken in the same registers (the transmit phase
-// T_k(z) comes from a per-tile table, the receive phasor R(p, j) is computed once per (pixel, j)), so one
-// float2 per pixel and frame is written at the end and no per-angle image or volume ever reaches HBM.
+// weight, phase rotation E(a) of the fractional delay (the sample's own phase is already in the entry), apodisation --
+// is computed once per (pixel, j, k) and reused for the F frames, whose accumulators stay in registers; the angle
+// sum is taken in the same registers, so one float2 per pixel and frame is written at the end and no per-angle
+// image or volume ever reaches HBM.
 //
 // Pixel mapping: the image is cut into horizontal strips of PX rows; a consumer thread owns the PX
 // vertically adjacent pixels of one (strip, column) position and a tile is 384 consecutive positions, so the
@@ -41,7 +41,6 @@ struct RingApertureArgs {
     const float *xs, *zs, *ejs, *xm, *zm, *ejm, *win;
     const int *n0;           // [k][iz] floor(U0) - n_lo
     const float *f0m;        // [k][iz] U0 - floor(U0) - 0.5
-    const float2 *tph;       // [k][iz] exp(j 2 pi (fc/fs U0 + fc t_start))
     long long out_base;
     // filled by ring_launch from RingTables:
     const int *dj;           // [tile][j] floor(min H over the tile) - 2
@@ -125,7 +124,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     constexpr int EB = entry_bytes(F, D32);
     const int NS = P.n_stages;
     unsigned char *p_misc = smem + (size_t)NS * P.stage_stride;
-    float4 *s_tab = reinterpret_cast<float4 *>(p_misc);                    // [k][row] {bt, T.re, T.im, -}
+    // [k][row] {frac(U0_k(z_row)) - 0.5, floor(U0_k(z_row)) - floor(U0_k(z_iz0))}: the integer row offset is added
+    // to the entry index in integer arithmetic, so the fp32 delay sum carries only the fraction and H
+    float2 *s_tab = reinterpret_cast<float2 *>(p_misc);
     float *s_ejs = reinterpret_cast<float *>(s_tab + kRingMaxTab);         // [n_rx]
     float *s_win = s_ejs + kRingMaxRx;
     float *s_ejm = s_win + kRingMaxRx;
@@ -200,7 +201,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     // ===================================== CONSUMER WARPS =====================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRingConsumerRegs));
     const int t = threadIdx.x;
-    const float fcfs = P.fcfs;
+    const float th = kTwoPi * P.fcfs;       // 2 pi fc / fs
     for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
         const int g = w / tiles_all;
         int tt = w - g * tiles_all;
@@ -218,12 +219,10 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         {
             const int *n0 = ULM_AP(n0);
             const float *f0m = ULM_AP(f0m);
-            const float2 *tph = ULM_AP(tph);
             for (int i = t; i < n_tx * rows; i += kRingConsumers) {
                 const int k = i / rows, r = i - k * rows;
                 const int base = k * n_ax + iz0;
-                const float2 T = tph[base + r];
-                s_tab[k * rows_cap + r] = make_float4((float)(n0[base + r] - n0[base]) + f0m[base + r], T.x, T.y, 0.f);
+                s_tab[k * rows_cap + r] = make_float2(f0m[base + r], __int_as_float(n0[base + r] - n0[base]));
             }
             const float *ejs = ULM_AP(ejs), *win = ULM_AP(win), *ejm = ULM_AP(ejm);
             const int *dj = ULM_AP(dj) + (size_t)tt * n_rx;
@@ -254,7 +253,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         // rows past the image bottom re-read the last table row (their results are never stored)
         uint32_t tab_off[PX];
 #pragma unroll
-        for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 16u;
+        for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 8u;
 
         // accumulators: (frame 2p, frame 2p+1) pairs of real / imaginary parts for FFMA2
         unsigned long long accR2[PX][F / 2], accI2[PX][F / 2];
@@ -265,7 +264,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 
         bool ready = false;      // the full barrier of the next stage was already seen complete
         for (int j = 0; j < n_rx; ++j) {
-            float Hs[PX], Rr[PX], Ri[PX];
+            float Hs[PX], wv[PX];
             {
                 const float dxs = xs - s_ejs[j];
                 const float dx2 = dxs * dxs;
@@ -275,21 +274,19 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     const float den = sqrtf(fmaf(zs[m], zs[m], dx2)) + zs[m];
                     const float H = den > 0.f ? __fdividef(dx2, den) : 0.f;
                     Hs[m] = H - djf;
-                    sincos_cycles(fcfs * H, Ri[m], Rr[m]);
                     if (APOD) {
-                        float wv = s_win[j];
+                        wv[m] = s_win[j];
                         if (P.two_f > 0.f) {
                             const float lhs = __fmul_rn(fabsf(__fsub_rn(xm, s_ejm[j])), P.two_f);
-                            if (!(lhs <= zm[m])) wv = 0.f;
+                            if (!(lhs <= zm[m])) wv[m] = 0.f;
                         }
-                        Rr[m] *= wv; Ri[m] *= wv;
                     }
                 }
             }
             for (int k = 0; k < n_tx; ++k) {
                 // the table row of the first pixel does not depend on the ring: fetched before the barrier wait
-                const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 16u;
-                uint4 tbn = lds128(tk + tab_off[0]);
+                const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 8u;
+                unsigned long long tbn = lds64(tk + tab_off[0]);
                 if (!ready) mbar_wait(smem_u32(&s_full[slot]), phase);
                 // entry address = stage base + EB * (rint(upm) + shift); hdr = shift - magic-constant bits
                 const uint32_t cbase = smem_u32(smem) + slot * P.stage_stride;
@@ -301,19 +298,21 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 ready = mbar_test(smem_u32(&s_full[slot]), phase);
                 // per-pixel setup of this stage: entry address, interpolation weight, phasor T_k(z) R(p, j)
                 struct PixCtx { uint32_t addr; Alpha A; float c, s; };
-                auto prep_tb = [&](int m, const uint4 &tb) {
-                    const float upm = __uint_as_float(tb.x) + Hs[m];
+                auto prep_tb = [&](int m, unsigned long long tb) {
+                    uint32_t fbits, ioff;
+                    split_u2(tb, fbits, ioff);
+                    const float upm = __uint_as_float(fbits) + Hs[m];
                     const float tt_ = upm + kMagic;
                     const float al = upm - (tt_ - kMagic);
-                    const float Tr = __uint_as_float(tb.y), Ti = __uint_as_float(tb.z);
                     PixCtx x;
-                    x.addr = (uint32_t)(__float_as_int(tt_) + hdr) * EB + cbase;
+                    x.addr = (uint32_t)(__float_as_int(tt_) + (int)ioff + hdr) * EB + cbase;
                     x.A = make_alpha(al);
-                    x.c = fmaf(Tr, Rr[m], -Ti * Ri[m]);
-                    x.s = fmaf(Tr, Ri[m], Ti * Rr[m]);
+                    // E(a) = exp(j 2 pi (fc/fs) a), a = al + 0.5 in [0, 1]: the whole phase rotation of this gather
+                    __sincosf(fmaf(th, al, 0.5f * th), &x.s, &x.c);
+                    if (APOD) { x.c *= wv[m]; x.s *= wv[m]; }
                     return x;
                 };
-                auto prep = [&](int m) { return prep_tb(m, lds128(tk + tab_off[m])); };
+                auto prep = [&](int m) { return prep_tb(m, lds64(tk + tab_off[m])); };
                 if constexpr (D32) {
 #pragma unroll
                     for (int m = 0; m < PX; ++m) {
@@ -331,7 +330,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     constexpr int NQ = F / 4, NSTEP = PX * NQ;
                     unsigned long long buf[2][5];
                     PixCtx cur = prep_tb(0, tbn), nxt = cur;
-                    if (PX > 1) tbn = lds128(tk + tab_off[1]);
+                    if (PX > 1) tbn = lds64(tk + tab_off[1]);
                     buf[0][0] = lds64(cur.addr); buf[0][1] = lds64(cur.addr + 8u); buf[0][2] = lds64(cur.addr + 16u);
                     buf[0][3] = lds64(cur.addr + 6u * F); buf[0][4] = lds64(cur.addr + 6u * F + 8u);
 #pragma unroll
@@ -342,7 +341,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                             if (q1 == 0) {
                                 // the table row of pixel m1 was requested a whole pixel (NQ chunks) earlier
                                 nxt = prep_tb(m1, tbn);
-                                if (m1 + 1 < PX) tbn = lds128(tk + tab_off[m1 + 1]);
+                                if (m1 + 1 < PX) tbn = lds64(tk + tab_off[m1 + 1]);
                             }
                             const uint32_t a1 = q1 == 0 ? nxt.addr : cur.addr;
                             unsigned long long *b = buf[(st + 1) & 1];

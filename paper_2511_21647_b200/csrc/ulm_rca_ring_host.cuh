@@ -12,7 +12,7 @@ namespace ulm {
 
 constexpr int kSmemLimit = 232448;   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 constexpr int kRingPx = 4;           // rows per strip = pixels per consumer thread
-constexpr int kRingMisc = kRingMaxTab * 16 + 4 * kRingMaxRx * 4 + kRingMaxStages * 4 + 2 * kRingMaxStages * 8 + 64;
+constexpr int kRingMisc = kRingMaxTab * 8 + 4 * kRingMaxRx * 4 + kRingMaxStages * 4 + 2 * kRingMaxStages * 8 + 64;
 
 struct RingConfig {
     int window = 0;      // entries per stage
