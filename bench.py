@@ -227,7 +227,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
 # capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {2: 17.339170e9 + 0.150121e9}     # profiles/r01_v3_ncu.md
+TRAFFIC_BYTES = {2: 10.794359e9 + 0.136630e9}     # profiles/r01_v4_ncu.md
 
 
 def run_volume(args):

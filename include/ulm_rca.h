@@ -84,11 +84,13 @@ typedef struct {
                                    0 = 32.  Larger calls are processed in batches of this size.        */
     int32_t build_volume;       /* 1 = also prepare ulm_rca_beamform_volume (needs equal axial grids)  */
     int32_t kernel;             /* 0 = auto; 1 = generic gather kernel; 2 = shared-memory ring kernel  */
-    int32_t precision;          /* storage of the interpolation difference term iq[n+1] - iq[n] in the
-                                   staged IQ scratch: 1 = compact (fp16; error <= ~2^-13 |difference|
-                                   per term: meant for band-limited data), 2 = full (fp32), 0 = auto:
-                                   compact for RF input (the library's own low-pass band-limits it),
-                                   full for IQ input (spectrum unknown)                                 */
+    int32_t precision;          /* format of the staged IQ scratch entries (mid = (a+b)/2, d = b-a of two
+                                   neighbouring samples): 1 = compact, 10 bytes per (sample, frame): mid with
+                                   17 significant bits, d and the interpolation weight in fp16 (error
+                                   <= ~2^-12 |d| per term: within 1e-4 of the image maximum on echo data,
+                                   meant for band-limited input), 2 = full (fp32 throughout, 16 bytes),
+                                   0 = auto: compact for RF input (the library's own low-pass band-limits
+                                   it), full for IQ input (spectrum unknown)                            */
     int32_t reserved[4];        /* must be 0                                                           */
 } ulm_rca_options;
 
