@@ -339,7 +339,7 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
 }
 
 template <int F, bool D32>
-__global__ void __launch_bounds__(256) demod_quad_kernel(DemodParams P) {
+__global__ void __launch_bounds__(256, 8) demod_quad_kernel(DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
     constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
