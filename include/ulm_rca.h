@@ -111,7 +111,12 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geometry,
                                    const ulm_rca_options *options, ulm_rca_plan **out);
 
 /*
- * Beamform n_frames frames (steps 0-3).  Enqueues on cuda_stream (a cudaStream_t passed as void*, NULL =
+ * Beamform n_frames frames (steps 0-3).  With compound == 1, transmit events of an aperture whose transmit delay on
+ * the reference slice is identical at every depth -- mirror angles +theta / -theta about a centred slice (ref_m = 0)
+ * with equal t0 -- share the sample index, the interpolation weight and the phase of every (pixel, element) term, so
+ * by linearity their channel data are added before demodulation and beamformed as one event ("folding"; detected at
+ * plan creation by comparing the fp64 delay tables, exact up to the rounding order of the sums).
+ * Enqueues on cuda_stream (a cudaStream_t passed as void*, NULL =
  * the legacy default stream) and returns without synchronising; results are valid once the caller has
  * synchronised that stream.  Never allocates.
  *   d_channel : int16 [frame][event][channel][sample] (x2 interleaved for IQ input), device memory
@@ -151,7 +156,9 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [6] window entries per stage (W)  [7] ring stages  [8] tiles per projection (x-z)
  *   [9] dynamic shared memory bytes   [10] kernels launched by the last beamform call
  *   [11] tiles per projection (y-z)   [12] precision in use (1 compact / 2 full)
- *   [13] scratch bytes per (sample, frame)   [14] bytes per frame ulm_rca_beamform_host uploads */
+ *   [13] scratch bytes per (sample, frame)   [14] bytes per frame ulm_rca_beamform_host uploads
+ *   [15] transmit events beamformed per frame by ulm_rca_beamform after folding (see below; = n_row_tx + n_col_tx
+ *        when nothing folds) */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this

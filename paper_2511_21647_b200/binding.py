@@ -105,7 +105,7 @@ def _farr(v):
 
 
 INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
-             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame"]
+             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame", "events_executed"]
 
 
 class Plan:

@@ -70,8 +70,17 @@ struct Aperture {
     int n_tx = 0, n_rx = 0, e0 = 0;
     Grid g;
     std::vector<double> angles, t0;
+    // Folded view of the transmit events for the compounded projection (compound = 1): events whose transmit delay
+    // U0_k(z) on the reference slice is identical for every depth (mirror angles +-theta about a centred slice with
+    // equal t0) have the same sample index, interpolation weight and phase for every (pixel, element), so by
+    // linearity their channel data are added in the pre-pass and beamformed as ONE event.  fk[v] = the real event k
+    // that represents folded event v, fk2[v] = its partner (-1: none), fe0 = index of the aperture's first folded
+    // event among all folded events.  Identity when nothing folds.
+    std::vector<int> fk, fk2;
+    int fe0 = 0;
+    std::vector<double> fangles, ft0;
     DeviceBuf xs, zs, ejs, xm, zm, ejm, win;
-    TxTables proj;      // 1 plane: the reference slice
+    TxTables proj;      // 1 plane: the reference slice; one table row block per FOLDED event
     TxTables vol;       // volume comparator: one plane per pixel of the other lateral axis
     ulm::RingTables ring;
     long long out_base = 0;
@@ -84,6 +93,8 @@ struct ulm_rca_plan {
     double pitch = 0, c = 0, fs = 0, fc = 0, t_start = 0, f_number = 0;
     int input_kind = 0, cpe = 0, n_samples = 0, compound = 1, max_frames = 32, build_volume = 0;
     int n_events = 0, n_rx_max = 0, half_len = 0;
+    int nv_events = 0;            // folded events of the projection path (= n_events when nothing folds)
+    DeviceBuf ev_fold, ev_id;     // short2 per scratch event row: the (first, second or -1) real events it holds
     bool apod = false;
     Aperture ap[2];               // [0] x-z (row-tx), [1] y-z (column-tx)
     int n_lo = 0, l_row = 0;      // IQ scratch origin / entries per row
@@ -149,13 +160,13 @@ void sample_range(const ulm_rca_plan &P, const Aperture &A, const std::vector<do
 }
 
 cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs,
-                            TxTables &T) {
-    const size_t n = refs.size() * (size_t)A.n_tx * A.g.n_ax;
+                            const std::vector<int> &ks, TxTables &T) {
+    const size_t n = refs.size() * ks.size() * A.g.n_ax;
     std::vector<int> n0(n);
     std::vector<float> f0m(n);
     size_t i = 0;
     for (double ref : refs)
-        for (int k = 0; k < A.n_tx; ++k)
+        for (int k : ks)
             for (int iz = 0; iz < A.g.n_ax; ++iz, ++i) {
                 const double u0 = u0_of(P, A, k, ref, A.g.z(iz));
                 const double fl = std::floor(u0);
@@ -236,11 +247,13 @@ ulm_rca_status upload_aperture(ulm_rca_plan &P, Aperture &A, const float *window
     return ULM_RCA_OK;
 }
 
-ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTables &T) {
+// folded = the scratch holds the folded events of the projection path (T = A.proj), else all real events
+ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTables &T, bool folded) {
     ulm::DasParams D{};
     D.iq = P.iq.as<unsigned char>();
-    D.l_row = P.l_row; D.n_rx_max = P.n_rx_max; D.n_events = P.n_events;
-    D.e0 = A.e0; D.n_tx = A.n_tx; D.n_rx = A.n_rx; D.n_lat = A.g.n_lat; D.n_ax = A.g.n_ax;
+    D.l_row = P.l_row; D.n_rx_max = P.n_rx_max; D.n_events = folded ? P.nv_events : P.n_events;
+    D.e0 = folded ? A.fe0 : A.e0; D.n_tx = folded ? (int)A.fk.size() : A.n_tx;
+    D.n_rx = A.n_rx; D.n_lat = A.g.n_lat; D.n_ax = A.g.n_ax;
     D.xs = A.xs.as<float>(); D.zs = A.zs.as<float>(); D.ejs = A.ejs.as<float>();
     D.xm = A.xm.as<float>(); D.zm = A.zm.as<float>(); D.ejm = A.ejm.as<float>();
     D.win = A.win.as<float>();
@@ -299,11 +312,14 @@ cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim
     return launch_demod_t<0, false, false, F, D32>(D, L, blocks, st);
 }
 
-cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, cudaStream_t st) {
+cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, bool folded, cudaStream_t st) {
     ulm::DemodParams D{};
     D.rf = d_channel; D.iq = P.iq.as<unsigned char>(); D.mixer = P.mixer.as<float2>(); D.mix_n0 = P.mix_n0;
-    D.n_frames = n_frames; D.n_events = P.n_events; D.channels_per_event = P.cpe; D.n_samples = P.n_samples;
-    D.n_row_tx = P.ap[0].n_tx; D.n_rows = P.n_rows; D.n_cols = P.n_cols; D.n_rx_max = P.n_rx_max;
+    D.n_frames = n_frames; D.n_events_real = P.n_events; D.channels_per_event = P.cpe; D.n_samples = P.n_samples;
+    D.n_events = folded ? P.nv_events : P.n_events;
+    D.ev_map = folded ? P.ev_fold.as<short2>() : P.ev_id.as<short2>();
+    D.n_row_tx = folded ? (int)P.ap[0].fk.size() : P.ap[0].n_tx;
+    D.n_rows = P.n_rows; D.n_cols = P.n_cols; D.n_rx_max = P.n_rx_max;
     D.full_channels = P.cpe == P.n_rows + P.n_cols;
     D.n_lo = P.n_lo; D.l_row = P.l_row;
     D.chunks_per_row = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
@@ -350,6 +366,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         return fail(ULM_RCA_EINVAL, "geometry: need n_rows, n_cols, pitch > 0");
     if (geo->n_rows > 4096 || geo->n_cols > 4096) return fail(ULM_RCA_EINVAL, "geometry: too many elements");
     if (n_row_tx < 0 || n_col_tx < 0 || n_row_tx + n_col_tx == 0) return fail(ULM_RCA_EINVAL, "need at least one transmit event");
+    if ((long long)n_row_tx + n_col_tx > 32767) return fail(ULM_RCA_EINVAL, "too many transmit events");
     if ((n_row_tx > 0 && !row_tx) || (n_col_tx > 0 && !col_tx)) return fail(ULM_RCA_EINVAL, "angle array is NULL");
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
@@ -455,12 +472,47 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         CUDA_TRY(P.mixer.upload(mix));
     }
 
+    // fold transmit events with identical reference-slice delays (see Aperture::fk); scratch event maps
+    {
+        std::vector<short2> map_fold, map_id;
+        for (int a = 0; a < 2; ++a) {
+            Aperture &A = P.ap[a];
+            std::vector<char> used(A.n_tx, 0);
+            A.fe0 = (int)map_fold.size();
+            for (int k = 0; k < A.n_tx; ++k) {
+                map_id.push_back(make_short2((short)(A.e0 + k), (short)-1));
+                if (used[k]) continue;
+                int partner = -1;
+                for (int k2 = k + 1; k2 < A.n_tx && P.compound && partner < 0; ++k2) {
+                    if (used[k2]) continue;
+                    double dmax = 0;
+                    for (int iz = 0; iz < A.g.n_ax; ++iz)
+                        dmax = std::max(dmax, std::fabs(u0_of(P, A, k, A.g.ref, A.g.z(iz)) - u0_of(P, A, k2, A.g.ref, A.g.z(iz))));
+                    if (dmax <= 1e-9) partner = k2;      // samples: far below the fp32 resolution of the delay
+                }
+                if (partner >= 0) used[partner] = 1;
+                A.fk.push_back(k);
+                A.fk2.push_back(partner);
+                A.fangles.push_back(A.angles[k]);
+                A.ft0.push_back(A.t0[k]);
+                map_fold.push_back(make_short2((short)(A.e0 + k), (short)(partner >= 0 ? A.e0 + partner : -1)));
+            }
+        }
+        P.nv_events = (int)map_fold.size();
+        CUDA_TRY(P.ev_fold.upload(map_fold));
+        CUDA_TRY(P.ev_id.upload(map_id));
+    }
+
     for (int a = 0; a < 2; ++a) {
         Aperture &A = P.ap[a];
         const float *win = opt->elem_window ? opt->elem_window + (a == 0 ? 0 : P.n_cols) : nullptr;
         if (ulm_rca_status s = upload_aperture(P, A, win)) return s;
-        CUDA_TRY(build_tx_tables(P, A, {A.g.ref}, A.proj));
-        if (P.build_volume) CUDA_TRY(build_tx_tables(P, A, vol_refs[a], A.vol));
+        CUDA_TRY(build_tx_tables(P, A, {A.g.ref}, A.fk, A.proj));
+        if (P.build_volume) {
+            std::vector<int> all(A.n_tx);
+            for (int k = 0; k < A.n_tx; ++k) all[k] = k;
+            CUDA_TRY(build_tx_tables(P, A, vol_refs[a], all, A.vol));
+        }
     }
 
     P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * P.n_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
@@ -473,8 +525,8 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         ulm::RingApertureDesc desc[2];
         for (int a = 0; a < 2; ++a) {
             const Aperture &A = P.ap[a];
-            desc[a] = ulm::RingApertureDesc{A.n_tx, A.n_rx, A.g.n_lat, A.g.n_ax, A.g.lat0, A.g.dlat, A.g.z0, A.g.dz,
-                                            A.g.ref, A.angles.data(), A.t0.data()};
+            desc[a] = ulm::RingApertureDesc{(int)A.fk.size(), A.n_rx, A.g.n_lat, A.g.n_ax, A.g.lat0, A.g.dlat, A.g.z0, A.g.dz,
+                                            A.g.ref, A.fangles.data(), A.ft0.data()};
         }
         const char *why = nullptr;
         const bool ok = ulm::ring_plan(desc, P.pitch, P.c, P.fs, P.t_start, P.l_row, P.ring, P.ap[0].ring,
@@ -503,13 +555,13 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *ch, size_t *
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n) {
     if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
     const bool ring = plan->kernel == 2, d32 = plan->d32;
-    const int64_t vals[15] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
+    const int64_t vals[16] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
                               ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
                               ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
                               ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
                               ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : 1, ulm::entry_bytes(12, d32) / 12,
-                              (int64_t)host_upload_bytes_per_frame(*plan)};
-    for (int i = 0; i < n && i < 15; ++i) v[i] = vals[i];
+                              (int64_t)host_upload_bytes_per_frame(*plan), plan->nv_events};
+    for (int i = 0; i < n && i < 16; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
 }
 
@@ -533,7 +585,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
         const int tb = P.timed_batches[slot] < ulm_rca_plan::kTimedBatches ? P.timed_batches[slot] : -1;
         if (tb >= 0) cudaEventRecord(P.ev[slot][tb][0], st);
-        CUDA_TRY(launch_demod(P, in, nb, st));
+        CUDA_TRY(launch_demod(P, in, nb, true, st));
         if (tb >= 0) cudaEventRecord(P.ev[slot][tb][1], st);
         for (int a = 0; a < 2; ++a) {     // an aperture without transmit events: its image is all zeros
             const Aperture &A = P.ap[a];
@@ -543,13 +595,13 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         }
         if (P.kernel == 2) {
             ulm::RingLaunch L{};
-            L.iq = P.iq.as<unsigned char>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.n_events;
+            L.iq = P.iq.as<unsigned char>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.nv_events;
             L.out = outp; L.out_frame_stride = P.out_per_frame; L.n_frames = nb;
             L.fcfs = (float)(P.fc / P.fs); L.two_f = (float)(2.0 * P.f_number);
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];
                 ulm::RingApertureArgs &R = L.ap[a];
-                R.e0 = A.e0; R.n_tx = A.n_tx; R.n_rx = A.n_rx; R.n_lat = A.g.n_lat; R.n_ax = A.g.n_ax;
+                R.e0 = A.fe0; R.n_tx = (int)A.fk.size(); R.n_rx = A.n_rx; R.n_lat = A.g.n_lat; R.n_ax = A.g.n_ax;
                 R.xs = A.xs.as<float>(); R.zs = A.zs.as<float>(); R.ejs = A.ejs.as<float>();
                 R.xm = A.xm.as<float>(); R.zm = A.zm.as<float>(); R.ejm = A.ejm.as<float>(); R.win = A.win.as<float>();
                 R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
@@ -559,7 +611,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         } else {
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];
-                ulm::DasParams D = das_params(P, A, A.proj);
+                ulm::DasParams D = das_params(P, A, A.proj, true);
                 D.out = outp; D.out_frame_stride = P.out_per_frame; D.out_base = A.out_base;
                 D.s_lat = A.g.n_ax; D.s_plane = 0; D.s_k = (long long)A.g.n_lat * A.g.n_ax;
                 D.per_angle = P.compound ? 0 : 1; D.accumulate = 0; D.n_frames = nb;
@@ -609,11 +661,11 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
         const int nb = std::min(P.max_frames, n_frames - f0);
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out_volume) + (long long)f0 * P.vol_per_frame;
-        CUDA_TRY(launch_demod(P, in, nb, st));
+        CUDA_TRY(launch_demod(P, in, nb, false, st));
         // V_RC: lateral = x, planes = y; then V_CR accumulated on top: lateral = y, planes = x
         for (int a = 0; a < 2; ++a) {
             const Aperture &A = P.ap[a];
-            ulm::DasParams D = das_params(P, A, A.vol);
+            ulm::DasParams D = das_params(P, A, A.vol, false);
             D.out = outp; D.out_frame_stride = P.vol_per_frame; D.out_base = 0;
             D.s_lat = a == 0 ? (long long)ny * nz : nz;
             D.s_plane = a == 0 ? nz : (long long)ny * nz;

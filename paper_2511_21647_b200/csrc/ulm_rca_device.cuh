@@ -61,7 +61,9 @@ struct DemodParams {
     unsigned char *iq;       // entries: [group][event][rx elem (n_rx_max)][l_row][entry_bytes(F, D32)]
     const float2 *mixer;     // exp(-j 2 pi fc t_n) for n = mix_n0 ..  (mixing of RF input; its conjugate is rho_n)
     int mix_n0;
-    int n_frames, n_events, channels_per_event, n_samples;
+    int n_frames, n_events, channels_per_event, n_samples;   // n_events = event rows of the scratch (folded or real)
+    int n_events_real;       // events per frame of the channel data
+    const short2 *ev_map;    // [n_events] the real events (first, second or -1) whose channel data are added into a row
     int n_row_tx, n_rows, n_cols, n_rx_max;
     int full_channels;       // 1: channels_per_event = n_rows + n_cols
     int n_lo, l_row;         // scratch origin (absolute sample of entry 0) and entries per row
@@ -194,12 +196,14 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     {
         constexpr int FH = F / 2;
         const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
-        const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
+        const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
         const int fr0 = g * F + h * FH;
         const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+        const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
         // record address formed once; the frames are reached by stepping (no per-frame 64-bit products)
         const long long rec0 = (long long)min(fr0, P.n_frames - 1) * frame_stride +
-                               ((long long)e * P.channels_per_event + ch) * (long long)P.n_samples;
+                               ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
+        const long long off_b = ev.y >= 0 ? (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples : 0;
         for (int i = i0; i < XW; i += 128) {
             const int n = base - L + i;
             const bool inb = n >= 0 && n < P.n_samples;
@@ -219,11 +223,22 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
                     const bool ok = inb && f <= f_last;
                     re[f] = ok ? (float)q[f].x : 0.f; im[f] = ok ? (float)q[f].y : 0.f;
                 }
+                if (ev.y >= 0) {             // folded pair: everything downstream is linear, add the second record
+                    src = rec0 + off_b + min(max(n, 0), P.n_samples - 1);
+#pragma unroll
+                    for (int f = 0; f < FH; ++f) {
+                        q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src);
+                        if (f < f_last) src += frame_stride;
+                    }
+#pragma unroll
+                    for (int f = 0; f < FH; ++f)
+                        if (inb && f <= f_last) { re[f] += (float)q[f].x; im[f] += (float)q[f].y; }
+                }
             } else {
                 int q[FH];
 #pragma unroll
                 for (int f = 0; f < FH; ++f) {
-                    q[f] = __ldg(P.rf + src);
+                    q[f] = (int)__ldg(P.rf + src) + (ev.y >= 0 ? (int)__ldg(P.rf + src + off_b) : 0);
                     if (f < f_last) src += frame_stride;
                 }
 #pragma unroll
@@ -362,11 +377,13 @@ __global__ void __launch_bounds__(256, 8) demod_quad_kernel(DemodParams P) {
     // The record address is formed once; the frames are reached by stepping a pointer (no per-frame 64-bit products).
     {
         const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
-        const long long frame_stride = (long long)P.n_events * P.channels_per_event * P.n_samples;
+        const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
         const int fr0 = g * F + h * FH;
         const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+        const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
         const int16_t *rec = P.rf + (long long)min(fr0, P.n_frames - 1) * frame_stride +
-                             ((long long)e * P.channels_per_event + ch) * (long long)P.n_samples;
+                             ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
+        const long long off_b = (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples;
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
             const int i = i0 + rep * 128;
@@ -378,10 +395,22 @@ __global__ void __launch_bounds__(256, 8) demod_quad_kernel(DemodParams P) {
                 // samples and frames are zeroed afterwards)
                 const int16_t *src = rec + min(max(n, 0), P.n_samples - 1);
                 int raw[FH];
+                if (ev.y >= 0) {             // folded pair: the FIR is linear, so the two records are added first
+                    int rawb[FH];            // (all 2 FH loads are issued before the first add)
 #pragma unroll
-                for (int f = 0; f < FH; ++f) {
-                    raw[f] = __ldg(src);
-                    if (f < f_last) src += frame_stride;
+                    for (int f = 0; f < FH; ++f) {
+                        raw[f] = __ldg(src);
+                        rawb[f] = __ldg(src + off_b);
+                        if (f < f_last) src += frame_stride;
+                    }
+#pragma unroll
+                    for (int f = 0; f < FH; ++f) raw[f] += rawb[f];
+                } else {
+#pragma unroll
+                    for (int f = 0; f < FH; ++f) {
+                        raw[f] = __ldg(src);
+                        if (f < f_last) src += frame_stride;
+                    }
                 }
 #pragma unroll
                 for (int f = 0; f < FH; ++f) dst[f * XS] = (inb && f <= f_last) ? (float)raw[f] : 0.f;
