@@ -303,7 +303,11 @@ cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim
     const int L = P.half_len;
     if (P.input_kind == 1) return launch_demod_t<1, false, true, F, D32>(D, 0, blocks, st);
     if (P.quad) {
-        ulm::demod_quad_kernel<F, D32><<<blocks, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
+        // one CTA per scratch row walks all of its chunks (software-pipelined loads) when there are enough rows to
+        // fill the GPU; few rows (single-frame calls) keep one CTA per chunk
+        dim3 qb = blocks;
+        if ((long long)blocks.y * blocks.z >= 2048) qb.x = 1;
+        ulm::demod_quad_kernel<F, D32><<<qb, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
         return cudaSuccess;
     }
     if (L == 8) return P.half_band ? launch_demod_t<17, true, false, F, D32>(D, L, blocks, st)
@@ -324,7 +328,7 @@ cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_
     D.n_lo = P.n_lo; D.l_row = P.l_row;
     D.chunks_per_row = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
     const int F = group_frames(n_frames);
-    const dim3 blocks((unsigned)D.chunks_per_row, (unsigned)P.n_rx_max, (unsigned)(((n_frames + F - 1) / F) * P.n_events));
+    const dim3 blocks((unsigned)D.chunks_per_row, (unsigned)P.n_rx_max, (unsigned)(((n_frames + F - 1) / F) * D.n_events));
     ++P.last_launches;
     if (P.d32) return F == 12 ? launch_demod_f<12, true>(P, D, blocks, st) : launch_demod_f<4, true>(P, D, blocks, st);
     return F == 12 ? launch_demod_f<12, false>(P, D, blocks, st) : launch_demod_f<4, false>(P, D, blocks, st);

@@ -354,7 +354,7 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
 }
 
 template <int F, bool D32>
-__global__ void __launch_bounds__(256, 8) demod_quad_kernel(DemodParams P) {
+__global__ void __launch_bounds__(256, 4) demod_quad_kernel(DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
     constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
@@ -363,96 +363,104 @@ __global__ void __launch_bounds__(256, 8) demod_quad_kernel(DemodParams P) {
     unsigned char *s_out = s_raw;
     float *s_x = reinterpret_cast<float *>(s_raw + OUT_BYTES);      // [F][XS], sample i at i + 4 (i >> 3)
 
-    // grid = (chunks per row, n_rx_max, groups * n_events)
-    const int chunk = blockIdx.x, j = blockIdx.y;
+    // grid = (chunk lanes, n_rx_max, groups * n_events): a CTA walks the chunks blockIdx.x, blockIdx.x + gridDim.x, ...
+    // of its row; the global loads of the next chunk are in flight while the current one is filtered and stored
+    const int j = blockIdx.y;
     const int g = blockIdx.z / P.n_events, e = blockIdx.z - g * P.n_events;
     const long long row = (long long)blockIdx.z * P.n_rx_max + j;     // (group * n_events + e) * n_rx_max + j
     const int row_tx = e < P.n_row_tx;
     const int n_rx = row_tx ? P.n_cols : P.n_rows;
     if (j >= n_rx) return;
     const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
-    const int base = P.n_lo + chunk * kDemodChunk;
 
-    // (1) raw samples as float: half h of the CTA takes frames [h FH, (h+1) FH), a thread takes samples i0, i0 + 128.
+    // (1) raw samples: half h of the CTA takes frames [h FH, (h+1) FH), a thread takes samples i0 and (i0 < 16) i0 + 128.
     // The record address is formed once; the frames are reached by stepping a pointer (no per-frame 64-bit products).
-    {
-        const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
-        const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
-        const int fr0 = g * F + h * FH;
-        const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
-        const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
-        const int16_t *rec = P.rf + (long long)min(fr0, P.n_frames - 1) * frame_stride +
-                             ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
-        const long long off_b = (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples;
+    const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
+    const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
+    const int fr0 = g * F + h * FH;
+    const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+    const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
+    const bool two = ev.y >= 0;                                  // folded pair: the FIR is linear, the records are added
+    const int16_t *rec = P.rf + (long long)min(fr0, P.n_frames - 1) * frame_stride +
+                         ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
+    const long long off_b = two ? (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples : 0;
+    const bool second = i0 + 128 < XW;
+    int ra[2][FH], rb[2][FH];        // prefetched samples of the next chunk: [sample column][frame], first / second event
+    // unconditional loads from clamped addresses (out-of-range samples and frames are zeroed when they are consumed)
+    auto issue_loads = [&](int chunk) {
+        const int base = P.n_lo + chunk * kDemodChunk;
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
+            if (rep == 1 && !second) break;
+            const int n = base - L + i0 + rep * 128;
+            const int16_t *src = rec + min(max(n, 0), P.n_samples - 1);
+#pragma unroll
+            for (int f = 0; f < FH; ++f) {
+                ra[rep][f] = __ldg(src);
+                rb[rep][f] = two ? (int)__ldg(src + off_b) : 0;
+                if (f < f_last) src += frame_stride;
+            }
+        }
+    };
+    auto store_x = [&](int chunk) {
+        const int base = P.n_lo + chunk * kDemodChunk;
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            if (rep == 1 && !second) break;
             const int i = i0 + rep * 128;
-            if (i < XW) {
-                const int n = base - L + i;
-                const bool inb = n >= 0 && n < P.n_samples;
-                float *dst = s_x + (h * FH) * XS + i + 4 * (i >> 3);
-                // unconditional loads from clamped addresses, all issued before the first use (out-of-range
-                // samples and frames are zeroed afterwards)
-                const int16_t *src = rec + min(max(n, 0), P.n_samples - 1);
-                int raw[FH];
-                if (ev.y >= 0) {             // folded pair: the FIR is linear, so the two records are added first
-                    int rawb[FH];            // (all 2 FH loads are issued before the first add)
+            const int n = base - L + i;
+            const bool inb = n >= 0 && n < P.n_samples;
+            float *dst = s_x + (h * FH) * XS + i + 4 * (i >> 3);
 #pragma unroll
-                    for (int f = 0; f < FH; ++f) {
-                        raw[f] = __ldg(src);
-                        rawb[f] = __ldg(src + off_b);
-                        if (f < f_last) src += frame_stride;
-                    }
-#pragma unroll
-                    for (int f = 0; f < FH; ++f) raw[f] += rawb[f];
-                } else {
-#pragma unroll
-                    for (int f = 0; f < FH; ++f) {
-                        raw[f] = __ldg(src);
-                        if (f < f_last) src += frame_stride;
-                    }
-                }
-#pragma unroll
-                for (int f = 0; f < FH; ++f) dst[f * XS] = (inb && f <= f_last) ? (float)raw[f] : 0.f;
-            }
+            for (int f = 0; f < FH; ++f) dst[f * XS] = (inb && f <= f_last) ? (float)(ra[rep][f] + rb[rep][f]) : 0.f;
         }
-    }
-    __syncthreads();
+    };
 
-    // (2) real FIRs A, B for 9 consecutive outputs, rotation, mid / d into the output image
-    const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
     const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
-    // every lane with f < F of a warp that holds at least one valid entry runs the whole loop (the compact store is
-    // warp-cooperative); entries past n_ent are computed from whatever the staging buffer holds and never stored
-    if (f < F && ((threadIdx.x & ~31) / TPG) * 8 < n_ent) {
-        const int r0 = grp * 8;
-        const float *x = s_x + f * XS + r0 + (r0 >> 1);         // r0 + 4 (r0 >> 3)
-        float A[9], B[9];
+    int chunk = blockIdx.x;
+    if (chunk < P.chunks_per_row) issue_loads(chunk);
+    for (; chunk < P.chunks_per_row; chunk += gridDim.x) {
+        const int base = P.n_lo + chunk * kDemodChunk;
+        store_x(chunk);                                      // consumes the prefetched registers
+        if (chunk + (int)gridDim.x < P.chunks_per_row) issue_loads(chunk + gridDim.x);
+        // the image of the previous chunk must have been read by its bulk store before it is overwritten
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+
+        // (2) real FIRs A, B for 9 consecutive outputs, mid / d into the output image
+        const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
+        // every lane with f < F of a warp that holds at least one valid entry runs the whole loop (the compact store is
+        // warp-cooperative); entries past n_ent are computed from whatever the staging buffer holds and never stored
+        if (f < F && ((threadIdx.x & ~31) / TPG) * 8 < n_ent) {
+            const int r0 = grp * 8;
+            const float *x = s_x + f * XS + r0 + (r0 >> 1);         // r0 + 4 (r0 >> 3)
+            float A[9], B[9];
 #pragma unroll
-        for (int q = 0; q < 9; ++q) B[q] = 0.f;
+            for (int q = 0; q < 9; ++q) B[q] = 0.f;
 #pragma unroll
-        for (int u = 0; u < 9 + 2 * L; ++u) {
-            const float xv = x[u + 4 * (u >> 3)];
+            for (int u = 0; u < 9 + 2 * L; ++u) {
+                const float xv = x[u + 4 * (u >> 3)];
 #pragma unroll
-            for (int q = 0; q < 9; ++q) {
-                const int t = q - u + 2 * L;                    // tap m = t - L
-                if (t == L) A[q] = c_demod[0].qd[L] * xv;
-                else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(c_demod[0].qd[t], xv, B[q]);
+                for (int q = 0; q < 9; ++q) {
+                    const int t = q - u + 2 * L;                    // tap m = t - L
+                    if (t == L) A[q] = c_demod[0].qd[L] * xv;
+                    else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(c_demod[0].qd[t], xv, B[q]);
+                }
             }
+            demod_quad_emit<F, D32>(A, B, r0, f, s_out);
         }
-        demod_quad_emit<F, D32>(A, B, r0, f, s_out);
+        zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();                                     // image complete; everybody is done reading s_x
+        if (threadIdx.x == 0) {
+            unsigned char *dst = P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB;
+            const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_out);
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"((uint32_t)(n_ent * EB))
+                         : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
     }
-    zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned char *dst = P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB;
-        const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_out);
-        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"((uint32_t)(n_ent * EB))
-                     : "memory");
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-    }
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // One aperture (image) of the generic DAS kernel.

@@ -98,6 +98,7 @@ def test_config0_full(torch_cuda, kernel):
     ch = synth.render(cfg)
     gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel))
     worst = assert_parity(gpu, ref)
+    assert info["events_executed"] == 4       # the +-5 degree events of each aperture fold (centred slices, t0 = 0)
     print("cfg0 kernel=%d worst rel err %.3e  info %s" % (info["kernel"], worst, info))
 
 
@@ -158,6 +159,37 @@ def test_per_angle_slices(torch_cuda):
         assert info1["kernel"] == 2
         s = gpu[:, :kr * nxz].reshape(2, kr, nxz).sum(1)
         assert np.abs(s - gpu1[:, :nxz]).max() <= bound * np.abs(gpu1).max()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_event_folding(torch_cuda, kernel):
+    """Transmit events with identical reference-slice delays (mirror angles about a centred slice, equal t0) are
+    added in the pre-pass and beamformed once; the oracle sums every event separately.  Folding must happen exactly
+    when the delays coincide -- and the result must not depend on it."""
+    d = synth.LAMBDA_M / 2
+    gx, gy = centred_grid(37, d, 53, 6e-3, d, ref=0.0), centred_grid(29, 1.2 * d, 41, 6.5e-3, 0.8 * d, ref=0.0)
+    mirror = tuple(np.radians([-6.0, 2.0, 6.0]))
+    cases = [
+        # (overrides, events executed): the +-6 degree pair of the row-tx aperture folds, nothing else does
+        (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=(0.1e-6, -0.1e-6, 0.1e-6, 0.3e-6, -0.25e-6)), 4),
+        # a centred slice but different t0 inside the pair: no folding
+        (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=(0.1e-6, -0.1e-6, 0.2e-6, 0.3e-6, -0.25e-6)), 5),
+        # equal t0 but an off-centre reference slice (ref sin(theta) differs in sign): no folding
+        (dict(row_tx_angles=mirror, t0=(0.1e-6, -0.1e-6, 0.1e-6, 0.3e-6, -0.25e-6)), 5),
+        # both apertures fold, one of them to a single event; duplicated angles fold too
+        (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=tuple(np.radians([-3.0, 3.0])),
+              col_tx_angles=tuple(np.radians([5.0, 0.0, 0.0, -5.0])), t0=None), 3),
+    ]
+    for over, n_exec in cases:
+        cfg = small(**over)
+        ch = synth.random_channel(cfg, cfg.n_frames, seed=77, amplitude=6000)
+        gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel))
+        assert info["events_executed"] == n_exec, (over, info)
+    # per-angle output never folds
+    cfg = small(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=None, compound=0)
+    ch = synth.random_channel(cfg, cfg.n_frames, seed=78, amplitude=6000)
+    gpu, ref, info = check_noise(torch_cuda, cfg, ch)
+    assert info["events_executed"] == 5
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
