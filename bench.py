@@ -239,7 +239,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
 # capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {2: 10.794359e9 + 0.136630e9}     # profiles/r01_v4_ncu.md
+TRAFFIC_BYTES = {2: 3.666862e9 + 0.136388e9}     # profiles/r01_v5_ncu.md
 
 
 def run_volume(args):

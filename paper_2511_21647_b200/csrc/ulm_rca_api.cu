@@ -106,6 +106,7 @@ struct ulm_rca_plan {
     bool d32 = false;             // full (fp32) difference term in the scratch
     bool quad = false;            // fs = 4 fc exactly, default 17 taps, analytic signal from two real filters
     bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
+    bool quarter_band = false;    // every fourth demodulation tap except the centre is exactly zero (fs = 8 fc)
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
     mutable long long last_launches = 0;
@@ -202,9 +203,11 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
         D.gd[t] = std::fabs(g) < 1e-13 ? 0.f : (float)g;     // exact zeros of the sinc (every 2nd tap at fs = 4 fc)
     }
     P.half_len = D.half_len = L;
-    P.half_band = true;
-    for (int t = 0; t <= 2 * L; ++t)
+    P.half_band = P.quarter_band = true;
+    for (int t = 0; t <= 2 * L; ++t) {
         if (t != L && ((t - L) & 1) == 0 && D.gd[t] != 0.f) P.half_band = false;
+        if (t != L && ((t - L) % 4) == 0 && D.gd[t] != 0.f) P.quarter_band = false;
+    }
     // quadrature sampling: fs = 4 fc exactly (the analytic signal needs no mixer, so any t_start qualifies)
     P.quad = P.half_band && L == 8 && P.fs == 4.0 * P.fc;
     if (P.quad) {
@@ -287,21 +290,21 @@ void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames
     else launch_generic_f<4>(P, D, n_frames, st);
 }
 
-template <int NT, bool HB, bool IQ, int F, bool D32>
+template <int NT, int ZS, bool IQ, int F, bool D32>
 cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, dim3 blocks, cudaStream_t st) {
     const size_t smem = (size_t)ulm::demod_smem_bytes(F, D32, L);
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, HB, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, ZS, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    ulm::demod_kernel<NT, HB, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
+    ulm::demod_kernel<NT, ZS, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
     return cudaSuccess;
 }
 
 template <int F, bool D32>
 cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim3 blocks, cudaStream_t st) {
     const int L = P.half_len;
-    if (P.input_kind == 1) return launch_demod_t<1, false, true, F, D32>(D, 0, blocks, st);
+    if (P.input_kind == 1) return launch_demod_t<1, 0, true, F, D32>(D, 0, blocks, st);
     if (P.quad) {
         // one CTA per scratch row walks all of its chunks (software-pipelined loads) when there are enough rows to
         // fill the GPU; few rows (single-frame calls) keep one CTA per chunk
@@ -310,10 +313,11 @@ cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim
         ulm::demod_quad_kernel<F, D32><<<qb, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
         return cudaSuccess;
     }
-    if (L == 8) return P.half_band ? launch_demod_t<17, true, false, F, D32>(D, L, blocks, st)
-                                   : launch_demod_t<17, false, false, F, D32>(D, L, blocks, st);
-    if (L == 16) return launch_demod_t<33, false, false, F, D32>(D, L, blocks, st);
-    return launch_demod_t<0, false, false, F, D32>(D, L, blocks, st);
+    if (L == 8) return P.half_band ? launch_demod_t<17, 2, false, F, D32>(D, L, blocks, st)
+                                   : launch_demod_t<17, 0, false, F, D32>(D, L, blocks, st);
+    if (L == 16) return P.quarter_band ? launch_demod_t<33, 4, false, F, D32>(D, L, blocks, st)
+                                       : launch_demod_t<33, 0, false, F, D32>(D, L, blocks, st);
+    return launch_demod_t<0, 0, false, F, D32>(D, L, blocks, st);
 }
 
 cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_frames, bool folded, cudaStream_t st) {

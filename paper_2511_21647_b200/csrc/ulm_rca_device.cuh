@@ -153,8 +153,9 @@ __device__ __forceinline__ void zero_edge_entries(unsigned char *s_out, int eb, 
 // frames of the group:
 //   (1) the mixed samples x = rf * exp(-j 2 pi fc t) of the F frames go to shared memory;
 //   (2) thread (frame f, group of 8 entries) runs the FIR for 9 consecutive outputs with the inputs sliding
-//       through registers (dense taps straight from constant memory; HB = half-band filter, fs = 4 fc: the
-//       even taps other than the centre are exactly zero and are skipped at compile time), forms
+//       through registers (dense taps straight from constant memory; ZS = 2: half-band filter, fs = 4 fc: the
+//       even taps other than the centre are exactly zero and are skipped at compile time; ZS = 4: every fourth tap,
+//       fs = 8 fc), forms
 //       mid = (a + b)/2 and d = b - a and writes them into an image of the output block in shared memory;
 //   (3) one elected thread stores the block (126 x 10 F contiguous bytes) with one cp.async.bulk (TMA).
 // NT = dense tap count 2L+1 (0: run-time L).  Lanes of a half-warp are the frames of one group, so every
@@ -168,7 +169,7 @@ __host__ __device__ inline int demod_smem_bytes(int F, bool D32, int L) {
     return kDemodSlots * entry_bytes(F, D32) + F * demod_xs(L) * 8;
 }
 
-template <int NT, bool HB, bool IQ_INPUT, int F, bool D32>
+template <int NT, int ZS, bool IQ_INPUT, int F, bool D32>
 __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
 #pragma unroll
                 for (int q = 0; q <= R; ++q) {
                     const int t = q - u + (NT - 1);
-                    if (t >= 0 && t < NT && !(HB && t != NT / 2 && ((t - NT / 2) & 1) == 0)) {
+                    if (t >= 0 && t < NT && !(ZS > 0 && t != NT / 2 && ((t - NT / 2) % ZS) == 0)) {
                         ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
                         ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
                     }
