@@ -70,12 +70,6 @@ struct DemodParams {
     int chunks_per_row;
 };
 
-__device__ __forceinline__ void sincos_cycles(float cyc, float &s, float &c) {
-    // cyc in cycles, |cyc| < 2^22.  Reduce to [-0.5, 0.5] exactly, then the MUFU approximations
-    // (abs error ~4e-7 on the reduced argument).
-    float r = cyc - ((cyc + kMagic) - kMagic);
-    __sincosf(kTwoPi * r, &s, &c);
-}
 
 // d(f32) = a(f16) * b(f16) + c(f32), one FHFMA on sm_100a
 __device__ __forceinline__ float fhfma(unsigned short a, unsigned short b, float c) {
@@ -498,8 +492,6 @@ __device__ __forceinline__ Alpha make_alpha(float al) {
     a.ah = f2h_bits(kAlScale * al);
     return a;
 }
-// fp16 -> fp32 as 1.0h * h + 0 on the FMA pipe (FHFMA runs at the full FP32 rate; HADD2.F32 does not)
-__device__ __forceinline__ float h2f(unsigned short h) { return fhfma((unsigned short)0x3C00, h, 0.f); }
 
 // packed fp32x2 helpers (sm_100 FFMA2: two fp32 FMAs in one issue slot)
 __device__ __forceinline__ unsigned long long pack_f2(float lo, float hi) {
@@ -543,11 +535,6 @@ __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t
 
 __device__ __forceinline__ void split_u2(unsigned long long v, uint32_t &lo, uint32_t &hi) {
     asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(v));
-}
-__device__ __forceinline__ unsigned long long pack_u2(uint32_t lo, uint32_t hi) {
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
-    return r;
 }
 
 // Packed version (ring kernel): m01 / m23 / m45 = the mid words as loaded by three LDS.64 (already the register
