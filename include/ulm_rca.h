@@ -182,6 +182,14 @@ ulm_rca_status ulm_rca_ring_probe(int32_t n_rx, float pitch_m, const float *angl
                                   float c_mps, float fs_hz, float t_start_s, const ulm_rca_grid *grid,
                                   int32_t *n_tiles, int32_t *window, int32_t *dj, int32_t *wj);
 
+/* Host-only view of the event folding ulm_rca_plan_create applies to ONE aperture when compound == 1 (no CUDA device
+ * needed; used by the CPU tests of the host logic): for the transmit angles `angles_rad[n_tx]` with offsets `t0_s`
+ * (NULL = 0) and the reference slice / depth rows of `grid`, partner[k] receives the index of the later event whose
+ * channel data are added to event k's (identical transmit delay on every depth row), -1 if event k is beamformed
+ * alone, -2 if event k itself has been folded into an earlier event. */
+ulm_rca_status ulm_rca_fold_probe(const float *angles_rad, const float *t0_s, int32_t n_tx, float c_mps, float fs_hz,
+                                  const ulm_rca_grid *grid, int32_t *partner);
+
 void ulm_rca_plan_destroy(ulm_rca_plan *plan); /* NULL-safe */
 
 const char *ulm_rca_last_error(void); /* thread-local, valid until the next failing call */

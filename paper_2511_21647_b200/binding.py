@@ -20,7 +20,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = range(5)
 _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
-           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe",
+           "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -84,6 +84,9 @@ def load() -> C.CDLL:
     lib.ulm_rca_ring_probe.argtypes = [i32, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float), i32, C.c_float,
                                        C.c_float, C.c_float, C.POINTER(Grid), C.POINTER(i32), C.POINTER(i32),
                                        C.POINTER(i32), C.POINTER(i32)]
+    lib.ulm_rca_fold_probe.restype = C.c_int
+    lib.ulm_rca_fold_probe.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), i32, C.c_float, C.c_float,
+                                       C.POINTER(Grid), C.POINTER(i32)]
     lib.ulm_rca_plan_destroy.restype = None
     lib.ulm_rca_plan_destroy.argtypes = [vp]
     lib.ulm_rca_last_error.restype = C.c_char_p
@@ -253,6 +256,18 @@ def ring_probe(n_rx: int, pitch: float, angles: Sequence[float], c: float, fs: f
     return {"n_tiles": nt.value, "window": w.value,
             "dj": np.array(dj, dtype=np.int64).reshape(nt.value, n_rx),
             "wj": np.array(wj, dtype=np.int64).reshape(nt.value, n_rx)}
+
+
+def fold_probe(angles: Sequence[float], c: float, fs: float, grid: tuple,
+               t0: Optional[Sequence[float]] = None) -> list:
+    """Host-only event folding of one aperture (ulm_rca_fold_probe): partner index, -1 (alone) or -2 (folded away)."""
+    lib = load()
+    aa, ap = _farr(list(angles))
+    ta, tp = _farr(t0)
+    g = Grid(*grid)
+    out = (C.c_int32 * len(angles))()
+    _check(lib.ulm_rca_fold_probe(ap, tp, len(angles), float(c), float(fs), C.byref(g), out))
+    return [int(v) for v in out]
 
 
 def fp32_peak_tflops(stream=None) -> float:

@@ -160,6 +160,27 @@ void sample_range(const ulm_rca_plan &P, const Aperture &A, const std::vector<do
             }
 }
 
+// Folding of one aperture's transmit events (host only, fp64): partner[k] = the later event folded into event k
+// (-1: none), -2 for an event that is itself the partner of an earlier one.  Two events fold when their transmit
+// delay on the reference slice, U0_k(z) = (t0_k + (z cos th_k + ref sin th_k)/c + z/c - t_start) fs, agrees to
+// 1e-9 samples on every depth row (far below the fp32 resolution of the delay); greedy, first match wins.
+std::vector<int> fold_partners(const std::vector<double> &angles, const std::vector<double> &t0, double c, double fs,
+                               double ref, double z0, double dz, int n_ax, bool enable) {
+    const int n = (int)angles.size();
+    std::vector<int> partner(n, -1);
+    auto u0 = [&](int k, double z) { return (t0[k] + (z * std::cos(angles[k]) + ref * std::sin(angles[k])) / c + z / c) * fs; };
+    for (int k = 0; k < n && enable; ++k) {
+        if (partner[k] == -2) continue;
+        for (int k2 = k + 1; k2 < n; ++k2) {
+            if (partner[k2] != -1) continue;
+            double dmax = 0;
+            for (int iz = 0; iz < n_ax; ++iz) dmax = std::max(dmax, std::fabs(u0(k, z0 + iz * dz) - u0(k2, z0 + iz * dz)));
+            if (dmax <= 1e-9) { partner[k] = k2; partner[k2] = -2; break; }
+        }
+    }
+    return partner;
+}
+
 cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs,
                             const std::vector<int> &ks, TxTables &T) {
     const size_t n = refs.size() * ks.size() * A.g.n_ax;
@@ -485,25 +506,17 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         std::vector<short2> map_fold, map_id;
         for (int a = 0; a < 2; ++a) {
             Aperture &A = P.ap[a];
-            std::vector<char> used(A.n_tx, 0);
+            const std::vector<int> partner = fold_partners(A.angles, A.t0, P.c, P.fs, A.g.ref, A.g.z0, A.g.dz, A.g.n_ax,
+                                                           P.compound != 0);
             A.fe0 = (int)map_fold.size();
             for (int k = 0; k < A.n_tx; ++k) {
                 map_id.push_back(make_short2((short)(A.e0 + k), (short)-1));
-                if (used[k]) continue;
-                int partner = -1;
-                for (int k2 = k + 1; k2 < A.n_tx && P.compound && partner < 0; ++k2) {
-                    if (used[k2]) continue;
-                    double dmax = 0;
-                    for (int iz = 0; iz < A.g.n_ax; ++iz)
-                        dmax = std::max(dmax, std::fabs(u0_of(P, A, k, A.g.ref, A.g.z(iz)) - u0_of(P, A, k2, A.g.ref, A.g.z(iz))));
-                    if (dmax <= 1e-9) partner = k2;      // samples: far below the fp32 resolution of the delay
-                }
-                if (partner >= 0) used[partner] = 1;
+                if (partner[k] == -2) continue;
                 A.fk.push_back(k);
-                A.fk2.push_back(partner);
+                A.fk2.push_back(partner[k]);
                 A.fangles.push_back(A.angles[k]);
                 A.ft0.push_back(A.t0[k]);
-                map_fold.push_back(make_short2((short)(A.e0 + k), (short)(partner >= 0 ? A.e0 + partner : -1)));
+                map_fold.push_back(make_short2((short)(A.e0 + k), (short)(partner[k] >= 0 ? A.e0 + partner[k] : -1)));
             }
         }
         P.nv_events = (int)map_fold.size();
@@ -770,6 +783,18 @@ ulm_rca_status ulm_rca_ring_probe(int32_t n_rx, float pitch_m, const float *angl
     const size_t n = (size_t)nt * n_rx;
     if (dj) std::copy(tab.begin(), tab.begin() + n, dj);
     if (wj) std::copy(tab.begin() + n, tab.begin() + 2 * n, wj);
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_fold_probe(const float *angles_rad, const float *t0_s, int32_t n_tx, float c_mps, float fs_hz,
+                                  const ulm_rca_grid *grid, int32_t *partner) {
+    if (!angles_rad || !grid || !partner || n_tx <= 0) return fail(ULM_RCA_EINVAL, "bad argument");
+    if (ulm_rca_status s = check_grid(grid, "grid")) return s;
+    if (!finite_pos(c_mps) || !finite_pos(fs_hz)) return fail(ULM_RCA_EINVAL, "c, fs must be finite and > 0");
+    std::vector<double> ang(angles_rad, angles_rad + n_tx), t0(n_tx, 0.0);
+    if (t0_s) for (int k = 0; k < n_tx; ++k) t0[k] = t0_s[k];
+    const std::vector<int> p = fold_partners(ang, t0, c_mps, fs_hz, grid->ref_m, grid->z0_m, grid->dz_m, grid->n_ax, true);
+    std::copy(p.begin(), p.end(), partner);
     return ULM_RCA_OK;
 }
 

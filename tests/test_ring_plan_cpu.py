@@ -71,3 +71,28 @@ def test_ring_probe_rejects_unsupported_shapes():
     from paper_2511_21647_b200 import UlmRcaError, ring_probe
     with pytest.raises(UlmRcaError):
         ring_probe(300, 0.2e-3, [0.0], 1540.0, 20e6, (16, 0.0, 0.1e-3, 16, 10e-3, 0.1e-3, 0.0))   # > 256 elements
+
+
+def test_event_folding_host_logic():
+    """Transmit events fold exactly when their reference-slice delays coincide on every depth row: mirror angles
+    about a centred slice with equal t0 (ulm_rca_fold_probe; DESIGN.md section 6 "event folding")."""
+    from paper_2511_21647_b200 import fold_probe
+    c, fs = 1540.0, 20e6
+    centred = (64, -4.8e-3, 0.15e-3, 96, 5e-3, 0.154e-3, 0.0)
+    off = centred[:6] + (0.4e-3,)
+    a11 = [float(np.float32(np.radians(a))) for a in np.linspace(-10, 10, 11)]
+    # the 11 angles of configs 1-3: five mirror pairs + the unpaired 0 degrees
+    assert fold_probe(a11, c, fs, centred) == [10, 9, 8, 7, 6, -1, -2, -2, -2, -2, -2]
+    # off-centre reference slice: ref sin(theta) changes sign inside a pair -> nothing folds
+    assert fold_probe(a11, c, fs, off) == [-1] * 11
+    # a different t0 inside a pair keeps it apart; equal t0 folds; duplicates fold; the middle one stays alone
+    ang = [float(np.float32(np.radians(a))) for a in (-6.0, 2.0, 6.0)]
+    assert fold_probe(ang, c, fs, centred, t0=[1e-7, -1e-7, 1e-7]) == [2, -1, -2]
+    assert fold_probe(ang, c, fs, centred, t0=[1e-7, -1e-7, 2e-7]) == [-1, -1, -1]
+    assert fold_probe([0.05, 0.0, 0.0, -0.05], c, fs, centred) == [3, 2, -2, -2]
+    # an off-centre slice whose t0 difference cancels ref sin(theta) exactly in fp64 is a fold as well ...
+    th = float(np.float32(np.radians(6.0)))
+    dt = 2 * off[6] * np.sin(th) / c
+    exact = fold_probe([-th, th], c, fs, off, t0=[dt, 0.0])
+    # ... but t0 travels through the C-ABI as fp32, so the compensation is only approximate and must NOT fold
+    assert exact == [-1, -1]
