@@ -176,9 +176,13 @@ def test_event_folding(torch_cuda, kernel):
         (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=(0.1e-6, -0.1e-6, 0.2e-6, 0.3e-6, -0.25e-6)), 5),
         # equal t0 but an off-centre reference slice (ref sin(theta) differs in sign): no folding
         (dict(row_tx_angles=mirror, t0=(0.1e-6, -0.1e-6, 0.1e-6, 0.3e-6, -0.25e-6)), 5),
-        # both apertures fold, one of them to a single event; duplicated angles fold too
+        # both apertures fold, one of them to a single event; duplicated angles fold too; f-number mask + window
         (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=tuple(np.radians([-3.0, 3.0])),
-              col_tx_angles=tuple(np.radians([5.0, 0.0, 0.0, -5.0])), t0=None), 3),
+              col_tx_angles=tuple(np.radians([5.0, 0.0, 0.0, -5.0])), t0=None, f_number=1.5,
+              elem_window=tuple(np.hanning(22)[1:-1].tolist() + np.hanning(26)[1:-1].tolist())), 3),
+        # the generic pre-pass (fs != 4 fc) and IQ input add the folded records too; 13 frames = a full 12-frame group + 1
+        (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=None, fs=25e6, fc=5.21e6, n_frames=13), 4),
+        (dict(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=None, input_kind=1), 4),
     ]
     for over, n_exec in cases:
         cfg = small(**over)
@@ -250,12 +254,16 @@ def test_linearity_on_gpu(torch_cuda, precision, bound):
 def test_host_entry_matches_device_entry(torch_cuda):
     torch = torch_cuda
     from paper_2511_21647_b200 import Plan
-    cfg = small()
-    ch = synth.random_channel(cfg, 3, seed=8, amplitude=6000)
-    with Plan(**rounded_kwargs(cfg)) as plan:
-        dev = plan.beamform(torch.from_numpy(ch).cuda()).cpu().numpy()
-        host = plan.beamform_host(ch)
-    np.testing.assert_array_equal(dev, host)
+    d = synth.LAMBDA_M / 2
+    folded = dict(grid_xz=centred_grid(37, d, 53, 6e-3, d), grid_yz=centred_grid(29, 1.2 * d, 41, 6.5e-3, 0.8 * d),
+                  row_tx_angles=tuple(np.radians([-6.0, 2.0, 6.0])), t0=None)
+    for over in (dict(), folded):
+        cfg = small(**over)
+        ch = synth.random_channel(cfg, 3, seed=8, amplitude=6000)
+        with Plan(**rounded_kwargs(cfg)) as plan:
+            dev = plan.beamform(torch.from_numpy(ch).cuda()).cpu().numpy()
+            host = plan.beamform_host(ch)
+        np.testing.assert_array_equal(dev, host)
 
 
 def test_volume_small(torch_cuda):
