@@ -205,6 +205,29 @@ def test_batching_and_ragged_frame_counts(torch_cuda, kernel):
     check_noise(torch_cuda, cfg, ch[:1], plan_extra=dict(max_frames=4, kernel=kernel))
 
 
+def test_plan_reuse_and_determinism(torch_cuda):
+    """One plan, calls of different sizes in turn (4-frame and 12-frame scratch groups alternate, batches of
+    max_frames), every call repeated: results are bitwise reproducible (no atomics anywhere on the path) and do not
+    depend on what the scratch held before."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfg = small(n_frames=17)
+    ch = torch.from_numpy(synth.random_channel(cfg, 17, seed=91, amplitude=6000)).cuda()
+    with Plan(**rounded_kwargs(cfg), max_frames=13) as plan:
+        ref17 = plan.beamform(ch).cpu().numpy()
+        for n in (3, 17, 1, 12, 13, 4, 17):
+            a = plan.beamform(ch[:n]).cpu().numpy()
+            b = plan.beamform(ch[:n]).cpu().numpy()
+            np.testing.assert_array_equal(a, b)
+            if n > 4:      # the same frames in the same 12-frame groups: identical arithmetic
+                np.testing.assert_array_equal(a[:12], ref17[:12])
+            else:
+                # 4-frame groups.  With compact entries the low mantissa byte of a direct fp24 value is a byte of
+                # another frame of its 4-frame chunk (DESIGN.md section 5), so a frame's result depends, below
+                # 2^-16 per term, on which frames share the chunk (here: frame 3 is absent): format level, not 0
+                assert np.abs(a - ref17[:n]).max() <= 5e-5 * np.abs(ref17).max()
+
+
 def test_zero_frames_and_bad_buffers(torch_cuda):
     torch = torch_cuda
     from paper_2511_21647_b200 import Plan
