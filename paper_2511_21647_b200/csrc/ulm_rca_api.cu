@@ -318,6 +318,8 @@ cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, dim3 blocks, cudaSt
         cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, ZS, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
+    // as in the quadrature kernel: one CTA per scratch row walks its chunks when there are enough rows
+    if ((long long)blocks.y * blocks.z >= 2048) blocks.x = 1;
     ulm::demod_kernel<NT, ZS, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
     return cudaSuccess;
 }

@@ -176,81 +176,91 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     unsigned char *s_out = s_raw;              // [126][EB] image of the output block
     float2 *s_x = reinterpret_cast<float2 *>(s_raw + OUT_BYTES);   // [F][XS]
 
-    // grid = (chunks per row, n_rx_max, groups * n_events)
-    const int chunk = blockIdx.x, j = blockIdx.y;
+    // grid = (chunk lanes, n_rx_max, groups * n_events): a CTA walks the chunks blockIdx.x, blockIdx.x + gridDim.x, ...
+    // of its row; the global loads of the next chunk are in flight while the current one is filtered and stored
+    const int j = blockIdx.y;
     const int g = blockIdx.z / P.n_events, e = blockIdx.z - g * P.n_events;
     const long long row = (long long)blockIdx.z * P.n_rx_max + j;     // (group * n_events + e) * n_rx_max + j
     const int row_tx = e < P.n_row_tx;
     const int n_rx = row_tx ? P.n_cols : P.n_rows;
     if (j >= n_rx) return;                      // rows of the shorter aperture stay unused
     const int ch = row_tx ? (P.full_channels ? P.n_rows + j : j) : j;
-    const int base = P.n_lo + chunk * kDemodChunk;   // absolute sample of this chunk's first iq value
 
-    // (1) mixed samples: half h of the CTA takes frames [h F/2, (h+1) F/2), a thread takes samples i0, i0 + 128, ...;
-    // all global loads of a sample column are issued before the first shared-memory store
-    {
-        constexpr int FH = F / 2;
-        const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
-        const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
-        const int fr0 = g * F + h * FH;
-        const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
-        const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
-        // record address formed once; the frames are reached by stepping (no per-frame 64-bit products)
-        const long long rec0 = (long long)min(fr0, P.n_frames - 1) * frame_stride +
-                               ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
-        const long long off_b = ev.y >= 0 ? (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples : 0;
-        for (int i = i0; i < XW; i += 128) {
+    // (1) mixed samples: half h of the CTA takes frames [h F/2, (h+1) F/2), a thread takes the sample columns i0 and
+    // i0 + 128 (XW <= 256); the record address is formed once, the frames are reached by stepping
+    constexpr int FH = F / 2;
+    const int h = threadIdx.x >> 7, i0 = threadIdx.x & 127;
+    const long long frame_stride = (long long)P.n_events_real * P.channels_per_event * P.n_samples;
+    const int fr0 = g * F + h * FH;
+    const int f_last = min(FH - 1, P.n_frames - 1 - fr0);       // < 0: this half of the group has no frame at all
+    const short2 ev = __ldg(P.ev_map + e);                      // real event(s) folded into this scratch row
+    const bool two = ev.y >= 0;                                  // folded pair: everything downstream is linear
+    const long long rec0 = (long long)min(fr0, P.n_frames - 1) * frame_stride +
+                           ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
+    const long long off_b = two ? (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples : 0;
+    const bool second = i0 + 128 < XW;
+    // prefetched samples of the next chunk: [sample column][frame], first / second event (IQ input: packed re | im)
+    int ra[2][FH], rb[2][FH];
+    auto issue_loads = [&](int chunk) {
+        const int base = P.n_lo + chunk * kDemodChunk;
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            if (rep == 1 && !second) break;
+            const int n = base - L + i0 + rep * 128;
+            long long src = rec0 + min(max(n, 0), P.n_samples - 1);     // clamped: the loads are unconditional
+#pragma unroll
+            for (int f = 0; f < FH; ++f) {
+                if (IQ_INPUT) {
+                    ra[rep][f] = __ldg(reinterpret_cast<const int *>(P.rf) + src);
+                    rb[rep][f] = two ? __ldg(reinterpret_cast<const int *>(P.rf) + src + off_b) : 0;
+                } else {
+                    ra[rep][f] = __ldg(P.rf + src);
+                    rb[rep][f] = two ? (int)__ldg(P.rf + src + off_b) : 0;
+                }
+                if (f < f_last) src += frame_stride;
+            }
+        }
+    };
+    auto store_x = [&](int chunk) {
+        const int base = P.n_lo + chunk * kDemodChunk;
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            if (rep == 1 && !second) break;
+            const int i = i0 + rep * 128;
             const int n = base - L + i;
             const bool inb = n >= 0 && n < P.n_samples;
             float2 *dst = s_x + (h * FH) * XS + i;
-            // unconditional loads from clamped addresses, all issued before the first use
-            long long src = rec0 + min(max(n, 0), P.n_samples - 1);
-            float re[FH], im[FH];
-            if (IQ_INPUT) {
-                short2 q[FH];
-#pragma unroll
-                for (int f = 0; f < FH; ++f) {
-                    q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src);
-                    if (f < f_last) src += frame_stride;
-                }
-#pragma unroll
-                for (int f = 0; f < FH; ++f) {
-                    const bool ok = inb && f <= f_last;
-                    re[f] = ok ? (float)q[f].x : 0.f; im[f] = ok ? (float)q[f].y : 0.f;
-                }
-                if (ev.y >= 0) {             // folded pair: everything downstream is linear, add the second record
-                    src = rec0 + off_b + min(max(n, 0), P.n_samples - 1);
-#pragma unroll
-                    for (int f = 0; f < FH; ++f) {
-                        q[f] = __ldg(reinterpret_cast<const short2 *>(P.rf) + src);
-                        if (f < f_last) src += frame_stride;
-                    }
-#pragma unroll
-                    for (int f = 0; f < FH; ++f)
-                        if (inb && f <= f_last) { re[f] += (float)q[f].x; im[f] += (float)q[f].y; }
-                }
-            } else {
-                int q[FH];
-#pragma unroll
-                for (int f = 0; f < FH; ++f) {
-                    q[f] = (int)__ldg(P.rf + src) + (ev.y >= 0 ? (int)__ldg(P.rf + src + off_b) : 0);
-                    if (f < f_last) src += frame_stride;
-                }
-#pragma unroll
-                for (int f = 0; f < FH; ++f) { re[f] = (inb && f <= f_last) ? (float)q[f] : 0.f; im[f] = 0.f; }
-            }
             float2 m = make_float2(1.f, 0.f);
             if (!IQ_INPUT && inb) m = __ldg(P.mixer + (n - P.mix_n0));
 #pragma unroll
-            for (int f = 0; f < FH; ++f)
-                dst[f * XS] = IQ_INPUT ? make_float2(re[f], im[f]) : make_float2(re[f] * m.x, re[f] * m.y);
+            for (int f = 0; f < FH; ++f) {
+                const bool ok = inb && f <= f_last;
+                if (IQ_INPUT) {
+                    const int a = ra[rep][f], b = rb[rep][f];
+                    const float re = (float)((short)(a & 0xffff) + (short)(b & 0xffff));
+                    const float im = (float)((a >> 16) + (b >> 16));
+                    dst[f * XS] = ok ? make_float2(re, im) : make_float2(0.f, 0.f);
+                } else {
+                    const float re = ok ? (float)(ra[rep][f] + rb[rep][f]) : 0.f;
+                    dst[f * XS] = make_float2(re * m.x, re * m.y);
+                }
+            }
         }
-    }
+    };
+
+    const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
+    int chunk = blockIdx.x;
+    if (chunk < P.chunks_per_row) issue_loads(chunk);
+    for (; chunk < P.chunks_per_row; chunk += gridDim.x) {
+    const int base = P.n_lo + chunk * kDemodChunk;   // absolute sample of this chunk's first iq value
+    store_x(chunk);                                  // consumes the prefetched registers
+    if (chunk + (int)gridDim.x < P.chunks_per_row) issue_loads(chunk + gridDim.x);
+    // the image of the previous chunk must have been read by its bulk store before it is overwritten
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     __syncthreads();
 
     // (2) FIR: iq[base + r] = sum_{i = r .. r + 2L} gd[r + 2L - i] x[i]   (x index relative to base - L)
     const int n_ent = min(kDemodChunk, P.l_row - chunk * kDemodChunk);
-    const int f = threadIdx.x % TPG, grp = threadIdx.x / TPG;
     // every lane with f < F of a warp that holds at least one valid entry runs the whole loop (the compact store is
     // warp-cooperative); entries past n_ent are computed from whatever the staging buffer holds and never stored
     if (f < F && ((threadIdx.x & ~31) / TPG) * R < n_ent) {
@@ -305,15 +315,16 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
     // (3) one bulk store of the block: generic-proxy writes -> async proxy, then TMA shared -> global
     zero_edge_entries(s_out, EB, n_ent, base, P.n_samples);
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
+    __syncthreads();                                 // image complete; everybody is done reading s_x
     if (threadIdx.x == 0) {
         unsigned char *dst = P.iq + ((size_t)row * P.l_row + (size_t)chunk * kDemodChunk) * EB;
         const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_out);
         asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"((uint32_t)(n_ent * EB))
                      : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     }
+    }   // chunk loop
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // ---------------------------------------------------------------------------------------------------
