@@ -83,7 +83,8 @@ typedef struct {
     int32_t max_frames;         /* largest n_frames a call will pass (sizes the plan's IQ scratch);
                                    0 = 32.  Larger calls are processed in batches of this size.        */
     int32_t build_volume;       /* 1 = also prepare ulm_rca_beamform_volume (needs equal axial grids)  */
-    int32_t kernel;             /* 0 = auto; 1 = generic gather kernel; 2 = shared-memory ring kernel  */
+    int32_t kernel;             /* 0 = auto (ring kernel where the shape fits); 1 = generic gather kernel;
+                                   2 = shared-memory ring kernel or ULM_RCA_EUNSUPPORTED                 */
     int32_t precision;          /* format of the staged IQ scratch entries (mid = (a+b)/2, d = b-a of two
                                    neighbouring samples): 1 = compact, 10 bytes per (sample, frame): mid with
                                    17 significant bits, d and the interpolation weight in fp16 (error

@@ -541,10 +541,10 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * P.n_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
     CUDA_TRY(cudaMalloc(&P.iq.p, P.iq_bytes));
 
-    // kernel choice: the shared-memory ring kernel covers compounded projections; everything else
-    // (per-angle slices, the volume, shapes whose window does not fit) takes the generic kernel.
+    // kernel choice: the shared-memory ring kernel covers the projections (compounded, or one slice per event with
+    // one work item per angle); the volume and shapes whose window does not fit take the generic kernel.
     P.kernel = 1;
-    if (P.compound && opt->kernel != 1) {
+    if (opt->kernel != 1) {
         ulm::RingApertureDesc desc[2];
         for (int a = 0; a < 2; ++a) {
             const Aperture &A = P.ap[a];
@@ -557,8 +557,6 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         if (ok) P.kernel = 2;
         else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
         if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
-    } else if (opt->kernel == 2) {
-        return fail(ULM_RCA_EUNSUPPORTED, "the ring kernel covers compound = 1 only");
     }
     for (auto &c : P.ev) for (auto &b : c) for (auto &e : b) CUDA_TRY(cudaEventCreate(&e));
     CUDA_TRY(cudaDeviceSynchronize());
@@ -619,7 +617,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         if (P.kernel == 2) {
             ulm::RingLaunch L{};
             L.iq = P.iq.as<unsigned char>(); L.l_row = P.l_row; L.n_rx_max = P.n_rx_max; L.n_events = P.nv_events;
-            L.out = outp; L.out_frame_stride = P.out_per_frame; L.n_frames = nb;
+            L.out = outp; L.out_frame_stride = P.out_per_frame; L.n_frames = nb; L.per_angle = P.compound ? 0 : 1;
             L.fcfs = (float)(P.fc / P.fs); L.two_f = (float)(2.0 * P.f_number);
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];

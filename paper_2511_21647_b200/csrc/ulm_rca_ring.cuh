@@ -54,6 +54,8 @@ struct RingLaunch {
     float2 *out;
     long long out_frame_stride;
     int n_frames;
+    int per_angle;           // 1: compound = 0 -- a work item is one transmit angle of a tile, the output is one slice
+                             // per event [event][lat][ax] (out_base = first slice of the aperture)
     float fcfs;
     float two_f;
     RingApertureArgs ap[2];
@@ -145,7 +147,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     }
     __syncthreads();
 
-    const int tiles_all = P.ap[0].n_tiles + P.ap[1].n_tiles;
+    // work items of a frame group: (aperture, tile) -- with per_angle (aperture, angle, tile)
+    const int items0 = P.ap[0].n_tiles * (P.per_angle ? P.ap[0].n_tx : 1);
+    const int tiles_all = items0 + P.ap[1].n_tiles * (P.per_angle ? P.ap[1].n_tx : 1);
     // ring position of the next stage (identical sequence in producer and consumers): slot and phase parity are
     // carried along instead of dividing a stage counter by the run-time ring depth
     uint32_t slot = 0, phase = 0;
@@ -157,10 +161,14 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
             const int g = w / tiles_all;
             int tt = w - g * tiles_all;
-            const int a = tt >= P.ap[0].n_tiles ? 1 : 0;
-            if (a) tt -= P.ap[0].n_tiles;
-            const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
-            const int e0 = ULM_AP(e0);
+            const int a = tt >= items0 ? 1 : 0;
+            if (a) tt -= items0;
+            const int n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+            const int n_tiles_a = ULM_AP(n_tiles);
+            const int k0 = P.per_angle ? tt / n_tiles_a : 0;              // first angle of the item
+            const int n_tx = P.per_angle ? 1 : ULM_AP(n_tx);              // angles of the item
+            tt -= (P.per_angle ? k0 : 0) * n_tiles_a;
+            const int e0 = ULM_AP(e0) + k0;
             const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx, *wj = ULM_AP(wj) + (size_t)tt * n_rx;
             const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
             const int n_st = n_rx * n_tx;
@@ -170,7 +178,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 const int my = sb + lane;
                 int my_s0 = 0, my_w = 0;
                 if (my < n_st) {
-                    my_s0 = __ldg(n0 + (my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
+                    my_s0 = __ldg(n0 + (k0 + my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
                     my_w = __ldg(wj + my / n_tx);
                 }
                 const int cnt = min(32, n_st - sb);
@@ -205,9 +213,13 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
         const int g = w / tiles_all;
         int tt = w - g * tiles_all;
-        const int a = tt >= P.ap[0].n_tiles ? 1 : 0;
-        if (a) tt -= P.ap[0].n_tiles;
+        const int a = tt >= items0 ? 1 : 0;
+        if (a) tt -= items0;
         const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+        const int n_tiles_a = ULM_AP(n_tiles);
+        const int k0 = P.per_angle ? tt / n_tiles_a : 0;                     // angles [k0, k1) of the item
+        const int k1 = P.per_angle ? k0 + 1 : n_tx;
+        tt -= (P.per_angle ? k0 : 0) * n_tiles_a;
         const int pos0 = tt * kRingConsumers;
         const int iz0 = (pos0 / n_lat) * PX;                                // first row of the tile
         const int n_pos = n_lat * ((n_ax + PX - 1) / PX);
@@ -283,7 +295,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     }
                 }
             }
-            for (int k = 0; k < n_tx; ++k) {
+            for (int k = k0; k < k1; ++k) {
                 // the table row of the first pixel does not depend on the ring: fetched before the barrier wait
                 const uint32_t tk = tab_addr + (uint32_t)(k * rows_cap) * 8u;
                 unsigned long long tbn = lds64(tk + tab_off[0]);
@@ -360,7 +372,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         }
         // projection write: one float2 per pixel and frame
         if (active) {
-            const long long out_base = ULM_AP(out_base);
+            const long long out_base = ULM_AP(out_base) + (P.per_angle ? (long long)k0 * n_lat * n_ax : 0);
 #pragma unroll
             for (int m = 0; m < PX; ++m) {
                 const int iz = strip * PX + m;

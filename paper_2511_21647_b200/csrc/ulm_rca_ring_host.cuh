@@ -160,7 +160,7 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     L.stage_stride = ring_stage_stride(cfg.window, F, D32);
     L.n_stages = ring_stages(cfg.window, F, D32);
     L.n_groups = (L.n_frames + F - 1) / F;
-    L.n_work = L.n_groups * (L.ap[0].n_tiles + L.ap[1].n_tiles);
+    L.n_work = L.n_groups * (L.ap[0].n_tiles * (L.per_angle ? L.ap[0].n_tx : 1) + L.ap[1].n_tiles * (L.per_angle ? L.ap[1].n_tx : 1));
     if (L.n_work == 0) return 0;
     static bool attr_set = false;
     if (!attr_set) {

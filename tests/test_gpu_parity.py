@@ -143,10 +143,20 @@ def test_small_variants(torch_cuda, kernel, case):
     assert info["precision"] == (2 if case in ("iq", "rf_full") else 1)
 
 
-def test_per_angle_slices(torch_cuda):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_per_angle_slices(torch_cuda, kernel):
+    """compound = 0: one slice per transmit event (the paper's S_k), through the generic kernel and
+    through the ring kernel (one work item per angle and tile)."""
     cfg = small(compound=0)
     ch = synth.random_channel(cfg, 2, seed=5, amplitude=6000)
-    check_noise(torch_cuda, cfg, ch)
+    _, _, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel))
+    assert info["kernel"] == (1 if kernel == 1 else 2)
+    # 13 frames (a full 12-frame group + 1), f-number mask and window, a single-aperture plan
+    w = np.hanning(cfg.n_cols + 2)[1:-1].tolist() + np.hanning(cfg.n_rows + 2)[1:-1].tolist()
+    cfg13 = small(compound=0, n_frames=13, f_number=1.5, elem_window=tuple(w))
+    check_noise(torch_cuda, cfg13, synth.random_channel(cfg13, 13, seed=6, amplitude=6000), plan_extra=dict(kernel=kernel))
+    cfg1 = small(compound=0, col_tx_angles=(), t0=(0.2e-6, -0.1e-6, 0.05e-6))
+    check_noise(torch_cuda, cfg1, synth.random_channel(cfg1, 3, seed=7, amplitude=6000), plan_extra=dict(kernel=kernel))
     # and the slices add up to the compounded images (full entries: the ring and the generic kernel differ by fp32
     # rounding only; with compact entries a delay that differs in the last fp32 bit can round the fp16 weight the
     # other way, so the two kernels agree to the format bound, not to 1e-5)
@@ -154,7 +164,7 @@ def test_per_angle_slices(torch_cuda):
     kr = len(cfg.row_tx_angles)
     for precision, bound in [(2, 1e-5), (1, NOISE_TOL_COMPACT)]:
         kw = rounded_kwargs(cfg)
-        gpu, _ = run_gpu(torch_cuda, kw, ch, dict(precision=precision))
+        gpu, _ = run_gpu(torch_cuda, kw, ch, dict(precision=precision, kernel=kernel))
         gpu1, info1 = run_gpu(torch_cuda, rounded_kwargs(cfg.with_(compound=1)), ch, dict(precision=precision))
         assert info1["kernel"] == 2
         s = gpu[:, :kr * nxz].reshape(2, kr, nxz).sum(1)
