@@ -155,13 +155,17 @@ def run_ours(args):
     sampler = ClockSampler(local_rank)
     sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     ev0.record(stream)
-    for _ in range(args.steps):
+    for i in range(args.steps):
         plan.beamform(channel, out=out)
+        step_ev[i].record(stream)
     ev1.record(stream)
     barrier()
     clocks = sampler.result()
     ms_total = ev0.elapsed_time(ev1)
+    marks = [ev0] + step_ev
+    per_step = sorted(marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps))
     demod_ms, das_ms = plan.timing(min(args.steps, 64))
     info = plan.info()
     launches = info["launches_last_call"] * args.steps
@@ -216,6 +220,7 @@ def run_ours(args):
                        "l2_policy": "inputs (%.1f GB) larger than L2, no flush" % (channel.numel() * 2 / 1e9),
                        "parallelism": "independent ensembles per GPU, no collective", "plan": info},
             "gather_samples_per_s": world * gathers / (ms_step * 1e-3),
+            "ms_per_step_min": per_step[0], "ms_per_step_median": per_step[len(per_step) // 2],
             "ensemble_ms": ms_step, "acquisition_ms": 1e3 * n_frames / cfg.frame_rate_hz,
             "kernels_ms": {"demod_stage": demod_ms, "das": das_ms},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
