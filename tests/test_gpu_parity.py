@@ -199,6 +199,11 @@ def test_event_folding(torch_cuda, kernel):
         ch = synth.random_channel(cfg, cfg.n_frames, seed=77, amplitude=6000)
         gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel))
         assert info["events_executed"] == n_exec, (over, info)
+    # folded events through batches of max_frames (11 frames in batches of 4)
+    cfg = small(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=None, n_frames=11)
+    ch = synth.random_channel(cfg, 11, seed=79, amplitude=6000)
+    gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(kernel=kernel, max_frames=4))
+    assert info["events_executed"] == 4
     # per-angle output never folds
     cfg = small(grid_xz=gx, grid_yz=gy, row_tx_angles=mirror, t0=None, compound=0)
     ch = synth.random_channel(cfg, cfg.n_frames, seed=78, amplitude=6000)
