@@ -11,6 +11,9 @@
 // is computed once per (pixel, j, k) and reused for the F frames, whose accumulators stay in registers; the angle
 // sum is taken in the same registers, so one float2 per pixel and frame is written at the end and no per-angle
 // image or volume ever reaches HBM.
+// The per-item tables (transmit delay rows of the tile, element coordinates, window offsets) are double-buffered and
+// written by a second warp of the producer group one work item ahead, so the consumer warps never meet at a CTA-wide
+// barrier: each flows from item to item on its own (full/empty mbarriers per table buffer, as for the ring).
 //
 // Pixel mapping: the image is cut into horizontal strips of PX rows; a consumer thread owns the PX
 // vertically adjacent pixels of one (strip, column) position and a tile is 384 consecutive positions, so the
@@ -34,7 +37,7 @@ constexpr int kRingConsumerRegs = 160;                      // setmaxnreg target
 constexpr int kRingProducerRegs = 32;
 constexpr int kRingMaxStages = 8;
 constexpr int kRingMaxRx = 256;                             // receive elements per aperture
-constexpr int kRingMaxTab = 1024;                           // n_tx * tile rows
+constexpr int kRingMaxTab = 512;                            // n_tx * tile rows (per table buffer)
 
 struct RingApertureArgs {
     int e0, n_tx, n_rx, n_lat, n_ax;
@@ -61,7 +64,24 @@ struct RingLaunch {
     RingApertureArgs ap[2];
     // filled by ring_launch:
     int window, stage_stride, n_stages, n_groups, n_work;
+    // Tail splitting: the first n_whole work items (a multiple of the grid size) are processed whole; each of the
+    // remaining n_items - n_whole items -- the last, partially filled round of the persistent grid -- is cut into
+    // split_s slices of the receive elements, work item n_whole + v = (item n_whole + v / split_s, slice v % split_s),
+    // whose partial sums go to `partial` [v][thread][PX][F] and are added in slice order by ring_combine_kernel.
+    int n_items, n_whole, split_s;
+    float2 *partial;
 };
+
+// (item, slice) of work item w; slice = -1: whole item
+__device__ __forceinline__ void ring_work(const RingLaunch &P, int w, int &item, int &slice) {
+    if (w < P.n_whole) { item = w; slice = -1; }
+    else { const int v = w - P.n_whole; item = P.n_whole + v / P.split_s; slice = v - (item - P.n_whole) * P.split_s; }
+}
+// receive elements [jb, je) of a slice
+__device__ __forceinline__ void ring_slice(const RingLaunch &P, int slice, int n_rx, int &jb, int &je) {
+    if (slice < 0) { jb = 0; je = n_rx; }
+    else { jb = (int)((long long)slice * n_rx / P.split_s); je = (int)((long long)(slice + 1) * n_rx / P.split_s); }
+}
 
 // ---- PTX helpers (mbarrier + bulk async copy) --------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -102,9 +122,6 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ void consumer_bar() {
-    asm volatile("bar.sync 1, %0;" ::"n"(kRingConsumers) : "memory");
-}
 __device__ __forceinline__ unsigned long long lds64(uint32_t addr) {
     unsigned long long v;
     asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
@@ -128,20 +145,23 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     unsigned char *p_misc = smem + (size_t)NS * P.stage_stride;
     // [k][row] {frac(U0_k(z_row)) - 0.5, floor(U0_k(z_row)) - floor(U0_k(z_iz0))}: the integer row offset is added
     // to the entry index in integer arithmetic, so the fp32 delay sum carries only the fraction and H
-    float2 *s_tab = reinterpret_cast<float2 *>(p_misc);
-    float *s_ejs = reinterpret_cast<float *>(s_tab + kRingMaxTab);         // [n_rx]
-    float *s_win = s_ejs + kRingMaxRx;
-    float *s_ejm = s_win + kRingMaxRx;
-    float *s_dj = s_ejm + kRingMaxRx;                                      // [n_rx] (float)(dj)
-    int *s_hdr = reinterpret_cast<int *>(s_dj + kRingMaxRx);               // [NS] entry shift of the stage
+    // two buffers of: s_tab [kRingMaxTab] float2, then s_ejs, s_win, s_ejm, s_dj [kRingMaxRx] floats each
+    constexpr int kTabBufBytes = kRingMaxTab * 8 + 4 * kRingMaxRx * 4;
+    int *s_hdr = reinterpret_cast<int *>(p_misc + 2 * kTabBufBytes);       // [NS] entry shift of the stage
     uint64_t *s_full = reinterpret_cast<uint64_t *>(s_hdr + kRingMaxStages);
     uint64_t *s_empty = s_full + kRingMaxStages;
+    uint64_t *t_full = s_empty + kRingMaxStages;                           // [2] table buffer written / released
+    uint64_t *t_empty = t_full + 2;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(smem_u32(&s_full[i]), 1);
             mbar_init(smem_u32(&s_empty[i]), kRingConsumerWarps);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(smem_u32(&t_full[i]), 1);
+            mbar_init(smem_u32(&t_empty[i]), kRingConsumerWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -157,13 +177,63 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     if (warp >= kRingConsumerWarps) {
         // ============ PRODUCER WARP GROUP: gives its registers to the consumers; one warp works ============
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRingProducerRegs));
+        if (warp == kRingConsumerWarps + 1) {
+            // ---- table warp: writes the tables of work item i into buffer i & 1, one item ahead of the consumers
+            uint32_t tbuf = 0, tphase = 0;
+            for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
+                int w, slice;
+                ring_work(P, ww, w, slice);
+                const int g = w / tiles_all;
+                int tt = w - g * tiles_all;
+                const int a = tt >= items0 ? 1 : 0;
+                if (a) tt -= items0;
+                const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+                const int n_tiles_a = ULM_AP(n_tiles);
+                const int k0 = P.per_angle ? tt / n_tiles_a : 0;
+                const int k1 = P.per_angle ? k0 + 1 : n_tx;
+                tt -= (P.per_angle ? k0 : 0) * n_tiles_a;
+                const int pos0 = tt * kRingConsumers;
+                const int iz0 = (pos0 / n_lat) * PX;
+                const int n_pos = n_lat * ((n_ax + PX - 1) / PX);
+                const int last_pos = min(pos0 + kRingConsumers, n_pos) - 1;
+                const int rows = min(n_ax, (last_pos / n_lat + 1) * PX) - iz0;
+                const int rows_cap = kRingMaxTab / n_tx;
+                unsigned char *buf = p_misc + tbuf * kTabBufBytes;
+                float2 *s_tab = reinterpret_cast<float2 *>(buf);
+                float *s_ejs = reinterpret_cast<float *>(buf + kRingMaxTab * 8);
+                float *s_win = s_ejs + kRingMaxRx, *s_ejm = s_win + kRingMaxRx, *s_dj = s_ejm + kRingMaxRx;
+                mbar_wait(smem_u32(&t_empty[tbuf]), tphase ^ 1);      // every consumer warp has left the item that used it
+                const int *n0 = ULM_AP(n0);
+                const float *f0m = ULM_AP(f0m);
+                for (int i = lane; i < (k1 - k0) * rows; i += 32) {
+                    const int k = k0 + i / rows, r = i - (k - k0) * rows;
+                    const int base = k * n_ax + iz0;
+                    s_tab[k * rows_cap + r] = make_float2(__ldg(f0m + base + r), __int_as_float(__ldg(n0 + base + r) - __ldg(n0 + base)));
+                }
+                const float *ejs = ULM_AP(ejs), *win = ULM_AP(win), *ejm = ULM_AP(ejm);
+                const int *dj = ULM_AP(dj) + (size_t)tt * n_rx;
+                for (int i = lane; i < n_rx; i += 32) {
+                    s_ejs[i] = __ldg(ejs + i);
+                    s_dj[i] = (float)__ldg(dj + i);
+                    if (APOD) { s_win[i] = __ldg(win + i); s_ejm[i] = __ldg(ejm + i); }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&t_full[tbuf]));
+                if (++tbuf == 2) { tbuf = 0; tphase ^= 1; }
+            }
+            return;
+        }
         if (warp != kRingConsumerWarps) return;
-        for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
+        for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
+            int w, slice;
+            ring_work(P, ww, w, slice);
             const int g = w / tiles_all;
             int tt = w - g * tiles_all;
             const int a = tt >= items0 ? 1 : 0;
             if (a) tt -= items0;
             const int n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+            int jb, je;
+            ring_slice(P, slice, n_rx, jb, je);
             const int n_tiles_a = ULM_AP(n_tiles);
             const int k0 = P.per_angle ? tt / n_tiles_a : 0;              // first angle of the item
             const int n_tx = P.per_angle ? 1 : ULM_AP(n_tx);              // angles of the item
@@ -171,15 +241,15 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             const int e0 = ULM_AP(e0) + k0;
             const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx, *wj = ULM_AP(wj) + (size_t)tt * n_rx;
             const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
-            const int n_st = n_rx * n_tx;
+            const int n_st = (je - jb) * n_tx;
             const unsigned char *grp = P.iq + (size_t)g * P.n_events * P.n_rx_max * P.l_row * EB;
             for (int sb = 0; sb < n_st; sb += 32) {
                 // each lane fetches the (unclamped) window start of one stage
                 const int my = sb + lane;
                 int my_s0 = 0, my_w = 0;
                 if (my < n_st) {
-                    my_s0 = __ldg(n0 + (k0 + my % n_tx) * n_ax + iz0) + __ldg(dj + my / n_tx);
-                    my_w = __ldg(wj + my / n_tx);
+                    my_s0 = __ldg(n0 + (k0 + my % n_tx) * n_ax + iz0) + __ldg(dj + jb + my / n_tx);
+                    my_w = __ldg(wj + jb + my / n_tx);
                 }
                 const int cnt = min(32, n_st - sb);
                 for (int i = 0; i < cnt; ++i) {
@@ -187,7 +257,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     const int wlen = __shfl_sync(0xffffffffu, my_w, i);
                     if (lane == 0) {
                         const int st = sb + i;
-                        const int j = st / n_tx, k = st - j * n_tx;
+                        const int j = jb + st / n_tx, k = st % n_tx;
                         // compact entries are 8-byte multiples: an even first entry keeps the copy 16-byte aligned
                         // (the window has two spare entries at either end, ring_plan_aperture)
                         const int s0 = max(0, min(s0_raw, P.l_row - wlen)) & (D32 ? ~0 : ~1);
@@ -210,12 +280,17 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRingConsumerRegs));
     const int t = threadIdx.x;
     const float th = kTwoPi * P.fcfs;       // 2 pi fc / fs
-    for (int w = blockIdx.x; w < P.n_work; w += gridDim.x) {
+    uint32_t cbuf = 0, cphase = 0;           // table buffer / phase parity of the next work item
+    for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
+        int w, slice;
+        ring_work(P, ww, w, slice);
         const int g = w / tiles_all;
         int tt = w - g * tiles_all;
         const int a = tt >= items0 ? 1 : 0;
         if (a) tt -= items0;
         const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
+        int jb, je;
+        ring_slice(P, slice, n_rx, jb, je);
         const int n_tiles_a = ULM_AP(n_tiles);
         const int k0 = P.per_angle ? tt / n_tiles_a : 0;                     // angles [k0, k1) of the item
         const int k1 = P.per_angle ? k0 + 1 : n_tx;
@@ -227,24 +302,14 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         const int rows = min(n_ax, (last_pos / n_lat + 1) * PX) - iz0;      // rows the tile touches
         const int rows_cap = kRingMaxTab / n_tx;                             // table row stride (>= rows, host-checked)
 
-        consumer_bar();     // everybody has left the previous work item: the tables may be rewritten
-        {
-            const int *n0 = ULM_AP(n0);
-            const float *f0m = ULM_AP(f0m);
-            for (int i = t; i < n_tx * rows; i += kRingConsumers) {
-                const int k = i / rows, r = i - k * rows;
-                const int base = k * n_ax + iz0;
-                s_tab[k * rows_cap + r] = make_float2(f0m[base + r], __int_as_float(n0[base + r] - n0[base]));
-            }
-            const float *ejs = ULM_AP(ejs), *win = ULM_AP(win), *ejm = ULM_AP(ejm);
-            const int *dj = ULM_AP(dj) + (size_t)tt * n_rx;
-            for (int i = t; i < n_rx; i += kRingConsumers) {
-                s_ejs[i] = ejs[i];
-                s_dj[i] = (float)dj[i];
-                if (APOD) { s_win[i] = win[i]; s_ejm[i] = ejm[i]; }
-            }
-        }
-        consumer_bar();
+        // the tables of this item (written by the table warp, possibly long ago)
+        unsigned char *tb_ = p_misc + cbuf * kTabBufBytes;
+        float2 *s_tab = reinterpret_cast<float2 *>(tb_);
+        float *s_ejs = reinterpret_cast<float *>(tb_ + kRingMaxTab * 8);
+        float *s_win = s_ejs + kRingMaxRx, *s_ejm = s_win + kRingMaxRx, *s_dj = s_ejm + kRingMaxRx;
+        const uint32_t my_tab_empty = smem_u32(&t_empty[cbuf]);
+        mbar_wait(smem_u32(&t_full[cbuf]), cphase);
+        if (++cbuf == 2) { cbuf = 0; cphase ^= 1; }
 
         // this thread's PX vertically adjacent pixels
         int pos = pos0 + t;
@@ -275,7 +340,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
 
         bool ready = false;      // the full barrier of the next stage was already seen complete
-        for (int j = 0; j < n_rx; ++j) {
+        for (int j = jb; j < je; ++j) {
             float Hs[PX], wv[PX];
             {
                 const float dxs = xs - s_ejs[j];
@@ -370,25 +435,87 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 if (lane == 0) mbar_arrive(my_empty);
             }
         }
-        // projection write: one float2 per pixel and frame
-        if (active) {
-            const long long out_base = ULM_AP(out_base) + (P.per_angle ? (long long)k0 * n_lat * n_ax : 0);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(my_tab_empty);      // this warp is done with the item's tables
+        if (slice >= 0) {
+            // partial sums of a slice: [work item - n_whole][thread][PX][F], added in slice order by ring_combine_kernel
+            float2 *dst = P.partial + ((size_t)(ww - P.n_whole) * kRingConsumers + t) * (PX * F);
 #pragma unroll
-            for (int m = 0; m < PX; ++m) {
-                const int iz = strip * PX + m;
-                if (iz >= n_ax) continue;
+            for (int m = 0; m < PX; ++m)
 #pragma unroll
-                for (int f = 0; f < F; ++f) {
-                    const int fr = g * F + f;
+                for (int f = 0; f < F; f += 2) {
                     float r0, r1, i0, i1;
                     unpack_f2(accR2[m][f / 2], r0, r1);
                     unpack_f2(accI2[m][f / 2], i0, i1);
-                    const float re = (f & 1) ? r1 : r0, im = (f & 1) ? i1 : i0;
-                    if (fr < P.n_frames)
-                        P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] = make_float2(re, im);
+                    *reinterpret_cast<float4 *>(dst + m * F + f) = make_float4(r0, i0, r1, i1);
+                }
+        } else if (active) {
+            // projection write: one float2 per pixel and frame; the PX pixels of a thread are contiguous in memory
+            // (axial index fastest), so a whole strip is written as 16-byte stores (pixel pairs) when it is aligned
+            const long long out_base = ULM_AP(out_base) + (P.per_angle ? (long long)k0 * n_lat * n_ax : 0);
+            const int izs = strip * PX;
+            const bool vec = (PX % 2 == 0) && izs + PX <= n_ax &&
+                             (((P.out_frame_stride | out_base | (long long)n_ax) & 1) == 0) &&
+                             ((reinterpret_cast<unsigned long long>(P.out) & 15ull) == 0);
+#pragma unroll
+            for (int f = 0; f < F; ++f) {
+                const int fr = g * F + f;
+                if (fr >= P.n_frames) break;
+                float2 *dst = P.out + (long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + izs;
+                float re[PX], im[PX];
+#pragma unroll
+                for (int m = 0; m < PX; ++m) {
+                    float r0, r1, i0, i1;
+                    unpack_f2(accR2[m][f / 2], r0, r1);
+                    unpack_f2(accI2[m][f / 2], i0, i1);
+                    re[m] = (f & 1) ? r1 : r0;
+                    im[m] = (f & 1) ? i1 : i0;
+                }
+                if (vec) {
+#pragma unroll
+                    for (int m = 0; m < PX; m += 2)
+                        *reinterpret_cast<float4 *>(dst + m) = make_float4(re[m], im[m], re[m + 1], im[m + 1]);
+                } else {
+#pragma unroll
+                    for (int m = 0; m < PX; ++m)
+                        if (izs + m < n_ax) dst[m] = make_float2(re[m], im[m]);
                 }
             }
         }
+    }
+}
+
+// Adds the split_s partial sums of every split work item in slice order (deterministic) and writes the pixels.
+// grid = (split items, PX), block = kRingConsumers.
+template <int F, int PX>
+__global__ void __launch_bounds__(kRingConsumers) ring_combine_kernel(const __grid_constant__ RingLaunch P) {
+    const int w = P.n_whole + blockIdx.x, m = blockIdx.y, t = threadIdx.x;
+    const int items0 = P.ap[0].n_tiles * (P.per_angle ? P.ap[0].n_tx : 1);
+    const int tiles_all = items0 + P.ap[1].n_tiles * (P.per_angle ? P.ap[1].n_tx : 1);
+    const int g = w / tiles_all;
+    int tt = w - g * tiles_all;
+    const int a = tt >= items0 ? 1 : 0;
+    if (a) tt -= items0;
+    const int n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax), n_tiles_a = ULM_AP(n_tiles);
+    const int k0 = P.per_angle ? tt / n_tiles_a : 0;
+    tt -= (P.per_angle ? k0 : 0) * n_tiles_a;
+    const int n_pos = n_lat * ((n_ax + PX - 1) / PX);
+    const int pos = tt * kRingConsumers + t;
+    if (pos >= n_pos) return;
+    const int strip = pos / n_lat, ix = pos - strip * n_lat, iz = strip * PX + m;
+    if (iz >= n_ax) return;
+    const long long out_base = ULM_AP(out_base) + (P.per_angle ? (long long)k0 * n_lat * n_ax : 0);
+    const float2 *src = P.partial + ((size_t)blockIdx.x * P.split_s * kRingConsumers + t) * (PX * F) + m * F;
+    const size_t slice_stride = (size_t)kRingConsumers * PX * F;
+    for (int f = 0; f < F; ++f) {
+        const int fr = g * F + f;
+        if (fr >= P.n_frames) break;
+        float2 acc = src[f];
+        for (int s_ = 1; s_ < P.split_s; ++s_) {
+            const float2 v = src[s_ * slice_stride + f];
+            acc.x += v.x; acc.y += v.y;
+        }
+        P.out[(long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + iz] = acc;
     }
 }
 

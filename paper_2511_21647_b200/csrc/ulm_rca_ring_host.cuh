@@ -12,12 +12,33 @@ namespace ulm {
 
 constexpr int kSmemLimit = 232448;   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 constexpr int kRingPx = 4;           // rows per strip = pixels per consumer thread
-constexpr int kRingMisc = kRingMaxTab * 8 + 4 * kRingMaxRx * 4 + kRingMaxStages * 4 + 2 * kRingMaxStages * 8 + 64;
+// two table buffers (per-item transmit table + 4 per-element arrays), stage headers, ring and table barriers
+constexpr int kRingMisc = 2 * (kRingMaxTab * 8 + 4 * kRingMaxRx * 4) + kRingMaxStages * 4 + 2 * kRingMaxStages * 8 + 4 * 8 + 64;
 
 struct RingConfig {
     int window = 0;      // entries per stage
     int n_sms = 0;
+    // tail splitting (RingLaunch::split_s): partial sums of the split work items, kRingSplitCap sub-items at most
+    float2 *d_partial = nullptr;
+    int partial_cap = 0;
+    ~RingConfig() { if (d_partial) cudaFree(d_partial); }
 };
+
+constexpr int kRingSplitMax = 16;    // slices per split work item at most
+
+// Slices for the r = n_items mod n_sms work items of the last, partially filled round of a grid of n_sms persistent
+// CTAs: s slices each turn that round into ceil(r s / n_sms) rounds of 1/s of the time.  Returns 1 (no split) unless a
+// split saves at least 10 % of a round.
+inline int ring_split_choice(int r, int n_sms, int n_rx, int cap) {
+    if (r <= 0) return 1;
+    int best = 1;
+    double best_cost = 1.0;
+    for (int s = 2; s <= kRingSplitMax && s <= n_rx && (long long)r * s <= cap; ++s) {
+        const double cost = (double)(((long long)r * s + n_sms - 1) / n_sms) / s + 0.01 * s;     // + per-slice overhead
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = s; }
+    }
+    return best_cost <= 0.9 ? best : 1;
+}
 
 struct RingTables {
     int n_tiles = 0;
@@ -152,6 +173,12 @@ inline bool ring_plan(const RingApertureDesc *desc, double pitch, double c, doub
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cfg.window = window;
     cfg.n_sms = sms;
+    cfg.partial_cap = 4 * sms;
+    if (cudaMalloc(&cfg.d_partial, (size_t)cfg.partial_cap * kRingConsumers * kRingPx * 12 * sizeof(float2)) != cudaSuccess) {
+        cudaGetLastError();
+        cfg.d_partial = nullptr;      // no tail splitting
+        cfg.partial_cap = 0;
+    }
     return true;
 }
 
@@ -160,8 +187,16 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     L.stage_stride = ring_stage_stride(cfg.window, F, D32);
     L.n_stages = ring_stages(cfg.window, F, D32);
     L.n_groups = (L.n_frames + F - 1) / F;
-    L.n_work = L.n_groups * (L.ap[0].n_tiles * (L.per_angle ? L.ap[0].n_tx : 1) + L.ap[1].n_tiles * (L.per_angle ? L.ap[1].n_tx : 1));
-    if (L.n_work == 0) return 0;
+    L.n_items = L.n_groups * (L.ap[0].n_tiles * (L.per_angle ? L.ap[0].n_tx : 1) + L.ap[1].n_tiles * (L.per_angle ? L.ap[1].n_tx : 1));
+    if (L.n_items == 0) return 0;
+    // tail splitting: the items of the last, partially filled round are cut into slices of the receive elements
+    const int rem = L.n_items > cfg.n_sms ? L.n_items % cfg.n_sms : 0;
+    int n_rx_min = 1 << 30;
+    for (int a = 0; a < 2; ++a) if (L.ap[a].n_tiles > 0) n_rx_min = std::min(n_rx_min, L.ap[a].n_rx);
+    L.split_s = ring_split_choice(rem, cfg.n_sms, n_rx_min, cfg.partial_cap);
+    L.n_whole = L.split_s > 1 ? L.n_items - rem : L.n_items;
+    L.n_work = L.n_whole + (L.n_items - L.n_whole) * L.split_s;
+    L.partial = cfg.d_partial;
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(das_ring_kernel<F, kRingPx, D32, APOD>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
@@ -169,6 +204,10 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     }
     const int grid = std::min(L.n_work, cfg.n_sms);
     das_ring_kernel<F, kRingPx, D32, APOD><<<grid, kRingThreads, ring_smem_bytes(cfg.window, F, D32), st>>>(L);
+    if (L.split_s > 1) {
+        ring_combine_kernel<F, kRingPx><<<dim3(L.n_items - L.n_whole, kRingPx), kRingConsumers, 0, st>>>(L);
+        return 2;
+    }
     return 1;
 }
 
