@@ -77,10 +77,11 @@ __device__ __forceinline__ void ring_work(const RingLaunch &P, int w, int &item,
     if (w < P.n_whole) { item = w; slice = -1; }
     else { const int v = w - P.n_whole; item = P.n_whole + v / P.split_s; slice = v - (item - P.n_whole) * P.split_s; }
 }
-// receive elements [jb, je) of a slice
-__device__ __forceinline__ void ring_slice(const RingLaunch &P, int slice, int n_rx, int &jb, int &je) {
-    if (slice < 0) { jb = 0; je = n_rx; }
-    else { jb = (int)((long long)slice * n_rx / P.split_s); je = (int)((long long)(slice + 1) * n_rx / P.split_s); }
+// receive elements of a slice: j = jb, jb + js, ... < n_rx (nj of them).  The slices interleave the elements, so each
+// holds the same mix of near and far elements (whose stages differ in bank conflicts and window length)
+__device__ __forceinline__ void ring_slice(const RingLaunch &P, int slice, int n_rx, int &jb, int &js, int &nj) {
+    if (slice < 0) { jb = 0; js = 1; nj = n_rx; }
+    else { jb = slice; js = P.split_s; nj = (n_rx - slice + P.split_s - 1) / P.split_s; }
 }
 
 // ---- PTX helpers (mbarrier + bulk async copy) --------------------------------------------------------
@@ -232,8 +233,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             const int a = tt >= items0 ? 1 : 0;
             if (a) tt -= items0;
             const int n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
-            int jb, je;
-            ring_slice(P, slice, n_rx, jb, je);
+            int jb, js, nj;
+            ring_slice(P, slice, n_rx, jb, js, nj);
             const int n_tiles_a = ULM_AP(n_tiles);
             const int k0 = P.per_angle ? tt / n_tiles_a : 0;              // first angle of the item
             const int n_tx = P.per_angle ? 1 : ULM_AP(n_tx);              // angles of the item
@@ -241,15 +242,15 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             const int e0 = ULM_AP(e0) + k0;
             const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx, *wj = ULM_AP(wj) + (size_t)tt * n_rx;
             const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
-            const int n_st = (je - jb) * n_tx;
+            const int n_st = nj * n_tx;
             const unsigned char *grp = P.iq + (size_t)g * P.n_events * P.n_rx_max * P.l_row * EB;
             for (int sb = 0; sb < n_st; sb += 32) {
                 // each lane fetches the (unclamped) window start of one stage
                 const int my = sb + lane;
                 int my_s0 = 0, my_w = 0;
                 if (my < n_st) {
-                    my_s0 = __ldg(n0 + (k0 + my % n_tx) * n_ax + iz0) + __ldg(dj + jb + my / n_tx);
-                    my_w = __ldg(wj + jb + my / n_tx);
+                    my_s0 = __ldg(n0 + (k0 + my % n_tx) * n_ax + iz0) + __ldg(dj + jb + (my / n_tx) * js);
+                    my_w = __ldg(wj + jb + (my / n_tx) * js);
                 }
                 const int cnt = min(32, n_st - sb);
                 for (int i = 0; i < cnt; ++i) {
@@ -257,7 +258,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     const int wlen = __shfl_sync(0xffffffffu, my_w, i);
                     if (lane == 0) {
                         const int st = sb + i;
-                        const int j = jb + st / n_tx, k = st % n_tx;
+                        const int j = jb + (st / n_tx) * js, k = st % n_tx;
                         // compact entries are 8-byte multiples: an even first entry keeps the copy 16-byte aligned
                         // (the window has two spare entries at either end, ring_plan_aperture)
                         const int s0 = max(0, min(s0_raw, P.l_row - wlen)) & (D32 ? ~0 : ~1);
@@ -289,8 +290,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         const int a = tt >= items0 ? 1 : 0;
         if (a) tt -= items0;
         const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
-        int jb, je;
-        ring_slice(P, slice, n_rx, jb, je);
+        int jb, js, nj;
+        ring_slice(P, slice, n_rx, jb, js, nj);
         const int n_tiles_a = ULM_AP(n_tiles);
         const int k0 = P.per_angle ? tt / n_tiles_a : 0;                     // angles [k0, k1) of the item
         const int k1 = P.per_angle ? k0 + 1 : n_tx;
@@ -340,7 +341,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
 
         bool ready = false;      // the full barrier of the next stage was already seen complete
-        for (int j = jb; j < je; ++j) {
+        for (int j = jb; j < n_rx; j += js) {
             float Hs[PX], wv[PX];
             {
                 const float dxs = xs - s_ejs[j];
