@@ -63,6 +63,7 @@ struct Grid {
 struct TxTables {
     int n_planes = 0;
     DeviceBuf n0, f0m;
+    DeviceBuf tab;      // the same interleaved, {bits of f0m, n0} (volume tables only: das_volume_kernel)
 };
 
 struct Aperture {
@@ -100,6 +101,7 @@ struct ulm_rca_plan {
     int n_lo = 0, l_row = 0;      // IQ scratch origin / entries per row
     int mix_n0 = 0;
     DeviceBuf mixer, iq;
+    DeviceBuf vol_rows;           // one frame of fp32 rows for the single-frame volume kernel (build_volume only)
     size_t iq_bytes = 0;
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
@@ -182,7 +184,7 @@ std::vector<int> fold_partners(const std::vector<double> &angles, const std::vec
 }
 
 cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs,
-                            const std::vector<int> &ks, TxTables &T) {
+                            const std::vector<int> &ks, TxTables &T, bool interleaved = false) {
     const size_t n = refs.size() * ks.size() * A.g.n_ax;
     std::vector<int> n0(n);
     std::vector<float> f0m(n);
@@ -197,6 +199,15 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
             }
     T.n_planes = (int)refs.size();
     cudaError_t e;
+    if (interleaved) {
+        std::vector<int2> tab(n);
+        for (size_t q = 0; q < n; ++q) {
+            int bits;
+            std::memcpy(&bits, &f0m[q], sizeof(bits));
+            tab[q] = make_int2(bits, n0[q]);
+        }
+        if ((e = T.tab.upload(tab)) != cudaSuccess) return e;
+    }
     if ((e = T.n0.upload(n0)) != cudaSuccess) return e;
     return T.f0m.upload(f0m);
 }
@@ -285,6 +296,7 @@ ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTabl
     D.n0 = T.n0.as<int>(); D.f0m = T.f0m.as<float>();
     D.fcfs = (float)(P.fc / P.fs);
     D.n_planes = T.n_planes;
+    D.rows = P.vol_rows.as<float4>(); D.tab = T.tab.as<int2>();
     return D;
 }
 
@@ -309,6 +321,35 @@ void launch_generic(const ulm_rca_plan &P, const ulm::DasParams &D, int n_frames
     if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
     if (group_frames(n_frames) == 12) launch_generic_f<12>(P, D, n_frames, st);
     else launch_generic_f<4>(P, D, n_frames, st);
+}
+
+// Volume batches of at most kVolFrameKernelMax frames go frame by frame through unpack_frame_kernel +
+// das_volume_kernel; larger batches amortise the index arithmetic over the frames of a group in the generic kernel.
+constexpr int kVolFrameKernelMax = 2;
+constexpr int kVolPlanes = 4;      // planes per thread of das_volume_kernel
+
+void launch_unpack(const ulm_rca_plan &P, int n_frames, int f, cudaStream_t st) {
+    const int F = group_frames(n_frames);
+    const long long n = (long long)P.n_events * P.n_rx_max * P.l_row;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    const unsigned char *iq = P.iq.as<unsigned char>() + (size_t)(f / F) * n * ulm::entry_bytes(F, P.d32);
+    float4 *rows = P.vol_rows.as<float4>();
+    if (F == 12) {
+        if (P.d32) ulm::unpack_frame_kernel<12, true><<<blocks, 256, 0, st>>>(iq, rows, n, f % F);
+        else ulm::unpack_frame_kernel<12, false><<<blocks, 256, 0, st>>>(iq, rows, n, f % F);
+    } else {
+        if (P.d32) ulm::unpack_frame_kernel<4, true><<<blocks, 256, 0, st>>>(iq, rows, n, f % F);
+        else ulm::unpack_frame_kernel<4, false><<<blocks, 256, 0, st>>>(iq, rows, n, f % F);
+    }
+    ++P.last_launches;
+}
+
+void launch_volume(const ulm_rca_plan &P, const ulm::DasParams &D, cudaStream_t st) {
+    if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
+    const dim3 grid((D.n_lat * D.n_ax + 127) / 128, (D.n_planes + kVolPlanes - 1) / kVolPlanes);
+    if (P.apod) ulm::das_volume_kernel<kVolPlanes, true><<<grid, 128, 0, st>>>(D);
+    else ulm::das_volume_kernel<kVolPlanes, false><<<grid, 128, 0, st>>>(D);
+    ++P.last_launches;
 }
 
 template <int NT, int ZS, bool IQ, int F, bool D32>
@@ -534,12 +575,13 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         if (P.build_volume) {
             std::vector<int> all(A.n_tx);
             for (int k = 0; k < A.n_tx; ++k) all[k] = k;
-            CUDA_TRY(build_tx_tables(P, A, vol_refs[a], all, A.vol));
+            CUDA_TRY(build_tx_tables(P, A, vol_refs[a], all, A.vol, true));
         }
     }
 
     P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * P.n_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
     CUDA_TRY(cudaMalloc(&P.iq.p, P.iq_bytes));
+    if (P.build_volume) CUDA_TRY(cudaMalloc(&P.vol_rows.p, (size_t)P.n_events * P.n_rx_max * P.l_row * sizeof(float4)));
 
     // kernel choice: the shared-memory ring kernel covers the projections (compounded, or one slice per event with
     // one work item per angle); the volume and shapes whose window does not fit take the generic kernel.
@@ -683,19 +725,24 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out_volume) + (long long)f0 * P.vol_per_frame;
         CUDA_TRY(launch_demod(P, in, nb, false, st));
+        const bool by_frame = nb <= kVolFrameKernelMax;
         // V_RC: lateral = x, planes = y; then V_CR accumulated on top: lateral = y, planes = x
-        for (int a = 0; a < 2; ++a) {
-            const Aperture &A = P.ap[a];
-            ulm::DasParams D = das_params(P, A, A.vol, false);
-            D.out = outp; D.out_frame_stride = P.vol_per_frame; D.out_base = 0;
-            D.s_lat = a == 0 ? (long long)ny * nz : nz;
-            D.s_plane = a == 0 ? nz : (long long)ny * nz;
-            D.s_k = 0; D.per_angle = 0; D.accumulate = a == 1 && P.ap[0].n_tx > 0; D.n_frames = nb;
-            if (A.n_tx == 0) {
-                if (a == 0) CUDA_TRY(cudaMemsetAsync(outp, 0, (size_t)nb * P.vol_per_frame * sizeof(float2), st));
-                continue;
+        for (int f = 0; f < (by_frame ? nb : 1); ++f) {
+            if (by_frame) launch_unpack(P, nb, f, st);
+            for (int a = 0; a < 2; ++a) {
+                const Aperture &A = P.ap[a];
+                ulm::DasParams D = das_params(P, A, A.vol, false);
+                D.out = outp; D.out_frame_stride = P.vol_per_frame; D.out_base = (long long)f * P.vol_per_frame;
+                D.s_lat = a == 0 ? (long long)ny * nz : nz;
+                D.s_plane = a == 0 ? nz : (long long)ny * nz;
+                D.s_k = 0; D.per_angle = 0; D.accumulate = a == 1 && P.ap[0].n_tx > 0; D.n_frames = nb;
+                if (A.n_tx == 0) {
+                    if (a == 0) CUDA_TRY(cudaMemsetAsync(outp + D.out_base, 0, (size_t)(by_frame ? 1 : nb) * P.vol_per_frame * sizeof(float2), st));
+                    continue;
+                }
+                if (by_frame) launch_volume(P, D, st);
+                else launch_generic(P, D, nb, st);
             }
-            launch_generic(P, D, nb, st);
         }
     }
     (void)nx;

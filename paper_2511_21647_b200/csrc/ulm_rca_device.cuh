@@ -487,6 +487,9 @@ struct DasParams {
     long long s_lat, s_plane, s_k;   // strides (float2) of lateral index, plane index, angle index
     int n_planes, per_angle, accumulate;
     int n_frames;                    // frames in this batch
+    // single-frame volume path (unpack_frame_kernel + das_volume_kernel)
+    const float4 *rows;              // [event][rx elem (n_rx_max)][l_row] {mid.re, mid.im, d.re, d.im} of ONE frame, fp32
+    const int2 *tab;                 // [plane][k][iz] {bits of f0m, n0}
 };
 
 // the interpolation weight a' = a - 0.5 of one gather: al (fp32) for full entries; ah = 16 a' rounded to fp16 for
@@ -692,6 +695,107 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             if (P.accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
             *dst = v;
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Single-frame volume path (config 4, the conventional comparator, is ONE frame: the frame groups of the scratch,
+// which let the projection kernels share all index arithmetic between 4 / 12 frames, have nothing to share there).
+// unpack_frame_kernel copies frame f of a group out of the scratch entries into plain fp32 rows
+// {mid.re, mid.im, d.re, d.im} (16 B per sample: one LDG.128 per gather-sample); das_volume_kernel gathers from them.
+// ---------------------------------------------------------------------------------------------------
+template <int F, bool D32>
+__global__ void __launch_bounds__(256) unpack_frame_kernel(const unsigned char *iq, float4 *rows, long long n_entries, int f) {
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n_entries) return;
+    const unsigned char *ep = iq + i * entry_bytes(F, D32);
+    float4 o;
+    if (D32) {
+        const float *mid = reinterpret_cast<const float *>(ep) + 4 * (f >> 1) + (f & 1);
+        const float *d = reinterpret_cast<const float *>(ep + 8 * F) + 4 * (f >> 1) + (f & 1);
+        o = make_float4(mid[0], mid[2], d[0], d[2]);
+    } else {
+        const uint32_t *w = reinterpret_cast<const uint32_t *>(ep + 24 * (f >> 2));
+        const int i4 = f & 3;
+        uint32_t re, im;
+        if (i4 < 2) { re = w[i4]; im = w[2 + i4]; }
+        else { re = w[2 + i4]; im = fp24_gather(w[i4 - 2], w[i4], w[i4 + 2]); }
+        const uint32_t dw = reinterpret_cast<const uint32_t *>(ep + 6 * F)[f];
+        const float2 dd = __half22float2(*reinterpret_cast<const __half2 *>(&dw));
+        // fp24 = the top three bytes of the fp32 value (truncated): the low byte is set to the middle of the cell.
+        // An all-zero value (edge rule) stays exactly zero.
+        const uint32_t rb = re & 0xFFFFFF00u, ib = im & 0xFFFFFF00u;
+        o = make_float4(__uint_as_float(rb ? (rb | 0x80u) : 0u), __uint_as_float(ib ? (ib | 0x80u) : 0u),
+                        dd.x * kAlScale, dd.y * kAlScale);
+    }
+    rows[i] = o;
+}
+
+// One thread = one (lateral, depth) pixel x NP consecutive planes (the y pixels of the volume for the row-transmit
+// events, the x pixels for the column-transmit ones).  The receive excess H(pixel, element) is shared by the planes
+// and the angles; neighbouring planes differ by a fraction of a sample in transmit delay, so their gathers hit the
+// same L1 lines.  Per gather-sample: one broadcast LDG.64 of {f0m, n0}, floor / fraction by the magic constant,
+// E(a) by two MUFU, one LDG.128 of the fp32 entry, 2 FMA for the interpolation, 4 FMA for the complex
+// multiply-accumulate.  grid = (pixel blocks, plane groups).
+template <int NP, bool APOD>
+__global__ void __launch_bounds__(128) das_volume_kernel(DasParams P) {
+    const int npix = P.n_lat * P.n_ax;
+    const int p = blockIdx.x * 128 + threadIdx.x;
+    if (p >= npix) return;
+    const int il = p % P.n_lat, iz = p / P.n_lat;
+    const int plane0 = blockIdx.y * NP;
+    const float xs = P.xs[il], zs = P.zs[iz];
+    const float zs2 = zs * zs;
+    const float th = kTwoPi * P.fcfs, th0 = 0.5f * th;
+    float ar[NP], ai[NP];
+    const int2 *tq[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        ar[q] = ai[q] = 0.f;
+        tq[q] = P.tab + (size_t)min(plane0 + q, P.n_planes - 1) * P.n_tx * P.n_ax + iz;
+    }
+    const size_t ev_stride = (size_t)P.n_rx_max * P.l_row;
+    for (int j = 0; j < P.n_rx; ++j) {
+        const float dxs = xs - P.ejs[j];
+        const float dx2 = dxs * dxs;
+        const float den = sqrtf(dx2 + zs2) + zs;
+        const float H = den > 0.f ? __fdividef(dx2, den) : 0.f;
+        float w = 1.f;
+        if (APOD) {
+            w = P.win[j];
+            if (P.two_f > 0.f) {
+                const float lhs = __fmul_rn(fabsf(__fsub_rn(P.xm[il], P.ejm[j])), P.two_f);
+                if (!(lhs <= P.zm[iz])) w = 0.f;
+            }
+            if (w == 0.f) continue;
+        }
+        const float4 *row = P.rows + ((size_t)P.e0 * P.n_rx_max + j) * P.l_row;
+        for (int k = 0; k < P.n_tx; ++k, row += ev_stride) {
+            const int tk = k * P.n_ax;
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                const int2 t = __ldg(tq[q] + tk);
+                const float upm = __int_as_float(t.x) + H;
+                const float tt = upm + kMagic;
+                const float al = upm - (tt - kMagic);
+                const int idx = t.y + (__float_as_int(tt) - kMagicBits);
+                float s, c;
+                __sincosf(fmaf(th, al, th0), &s, &c);       // E(a), a = al + 0.5 in [0, 1]
+                if (APOD) { s *= w; c *= w; }
+                const float4 e = __ldg(row + idx);
+                const float vr = fmaf(al, e.z, e.x), vi = fmaf(al, e.w, e.y);
+                ar[q] = fmaf(c, vr, ar[q]); ar[q] = fmaf(-s, vi, ar[q]);
+                ai[q] = fmaf(s, vr, ai[q]); ai[q] = fmaf(c, vi, ai[q]);
+            }
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        if (plane0 + q >= P.n_planes) break;
+        float2 *dst = P.out + P.out_base + (long long)il * P.s_lat + (long long)(plane0 + q) * P.s_plane + iz;
+        float2 v = make_float2(ar[q], ai[q]);
+        if (P.accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
+        *dst = v;
     }
 }
 

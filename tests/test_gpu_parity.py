@@ -304,23 +304,26 @@ def test_host_entry_matches_device_entry(torch_cuda):
         np.testing.assert_array_equal(dev, host)
 
 
-def test_volume_small(torch_cuda):
-    """Full 3-D comparator against the oracle's point-outer DAS on a small shared-axial-grid case."""
+@pytest.mark.parametrize("n_frames,precision", [(2, 0), (1, 2), (3, 0), (5, 2)])
+def test_volume_small(torch_cuda, n_frames, precision):
+    """Full 3-D comparator against the oracle's point-outer DAS on a small shared-axial-grid case: batches of one or
+    two frames take unpack_frame_kernel + das_volume_kernel (plane counts 15 / 19 leave a ragged plane group),
+    larger ones the generic kernel; compact and full scratch entries."""
     torch = torch_cuda
     from paper_2511_21647_b200 import Plan
     d = synth.LAMBDA_M / 2
     gx = centred_grid(19, d, 33, 6e-3, d, ref=0.0)
     gy = centred_grid(15, 1.3 * d, 33, 6e-3, d, ref=0.0)
-    cfg = small(grid_xz=gx, grid_yz=gy, n_frames=2, f_number=1.4)
-    ch = synth.random_channel(cfg, 2, seed=41, amplitude=6000)
+    cfg = small(grid_xz=gx, grid_yz=gy, n_frames=n_frames, f_number=1.4)
+    ch = synth.random_channel(cfg, n_frames, seed=41, amplitude=6000)
     kw = rounded_kwargs(cfg)
     p = oracle.OracleParams(**kw)
     xs = kw["grid_xz"][1] + kw["grid_xz"][2] * np.arange(gx[0])
     ys = kw["grid_yz"][1] + kw["grid_yz"][2] * np.arange(gy[0])
     zs = kw["grid_xz"][4] + kw["grid_xz"][5] * np.arange(gx[3])
-    with Plan(**kw, build_volume=True) as plan:
+    with Plan(**kw, build_volume=True, precision=precision) as plan:
         vol = plan.beamform_volume(torch.from_numpy(ch).cuda()).cpu().numpy()
-    for f in range(2):
+    for f in range(n_frames):
         v_rc, v_cr = oracle.volume(p, ch[f], xs, ys, zs)
         assert rel_err(vol[f], v_rc + v_cr) <= TOL
 
