@@ -63,7 +63,8 @@ struct Grid {
 struct TxTables {
     int n_planes = 0;
     DeviceBuf n0, f0m;
-    DeviceBuf tab;      // the same interleaved, {bits of f0m, n0} (volume tables only: das_volume_kernel)
+    DeviceBuf tab;      // the same as {bits of f0m, n0}, [plane][iz][k (kpad)] (volume tables only: das_volume_kernel)
+    int kpad = 0;
 };
 
 struct Aperture {
@@ -199,13 +200,18 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
             }
     T.n_planes = (int)refs.size();
     cudaError_t e;
-    if (interleaved) {
-        std::vector<int2> tab(n);
-        for (size_t q = 0; q < n; ++q) {
-            int bits;
-            std::memcpy(&bits, &f0m[q], sizeof(bits));
-            tab[q] = make_int2(bits, n0[q]);
-        }
+    if (interleaved) {      // [plane][iz][k], k padded to an even count (das_volume_kernel reads two angles per load)
+        const size_t nk = ks.size(), kpad = (nk + 1) / 2 * 2, nz = (size_t)A.g.n_ax;
+        std::vector<int2> tab(refs.size() * nz * kpad, make_int2(0, 0));
+        for (size_t r = 0; r < refs.size(); ++r)
+            for (size_t ki = 0; ki < nk; ++ki)
+                for (size_t iz = 0; iz < nz; ++iz) {
+                    const size_t q = (r * nk + ki) * nz + iz;
+                    int bits;
+                    std::memcpy(&bits, &f0m[q], sizeof(bits));
+                    tab[(r * nz + iz) * kpad + ki] = make_int2(bits, n0[q]);
+                }
+        T.kpad = (int)kpad;
         if ((e = T.tab.upload(tab)) != cudaSuccess) return e;
     }
     if ((e = T.n0.upload(n0)) != cudaSuccess) return e;
@@ -296,7 +302,7 @@ ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTabl
     D.n0 = T.n0.as<int>(); D.f0m = T.f0m.as<float>();
     D.fcfs = (float)(P.fc / P.fs);
     D.n_planes = T.n_planes;
-    D.rows = P.vol_rows.as<float4>(); D.tab = T.tab.as<int2>();
+    D.rows = P.vol_rows.as<float4>(); D.tab = T.tab.as<int2>(); D.tab_kpad = T.kpad;
     return D;
 }
 

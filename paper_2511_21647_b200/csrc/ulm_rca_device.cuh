@@ -489,7 +489,8 @@ struct DasParams {
     int n_frames;                    // frames in this batch
     // single-frame volume path (unpack_frame_kernel + das_volume_kernel)
     const float4 *rows;              // [event][rx elem (n_rx_max)][l_row] {mid.re, mid.im, d.re, d.im} of ONE frame, fp32
-    const int2 *tab;                 // [plane][k][iz] {bits of f0m, n0}
+    const int2 *tab;                 // [plane][iz][k (tab_kpad, even)] {bits of f0m, n0}
+    int tab_kpad;
 };
 
 // the interpolation weight a' = a - 0.5 of one gather: al (fp32) for full entries; ah = 16 a' rounded to fp16 for
@@ -734,7 +735,7 @@ __global__ void __launch_bounds__(256) unpack_frame_kernel(const unsigned char *
 // One thread = one (lateral, depth) pixel x NP consecutive planes (the y pixels of the volume for the row-transmit
 // events, the x pixels for the column-transmit ones).  The receive excess H(pixel, element) is shared by the planes
 // and the angles; neighbouring planes differ by a fraction of a sample in transmit delay, so their gathers hit the
-// same L1 lines.  Per gather-sample: one broadcast LDG.64 of {f0m, n0}, floor / fraction by the magic constant,
+// same L1 lines.  Per gather-sample: half a broadcast LDG.128 of {f0m, n0} x 2 angles, floor / fraction by the magic constant,
 // E(a) by two MUFU, one LDG.128 of the fp32 entry, 2 FMA for the interpolation, 4 FMA for the complex
 // multiply-accumulate.  grid = (pixel blocks, plane groups).
 template <int NP, bool APOD>
@@ -752,9 +753,24 @@ __global__ void __launch_bounds__(128) das_volume_kernel(DasParams P) {
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         ar[q] = ai[q] = 0.f;
-        tq[q] = P.tab + (size_t)min(plane0 + q, P.n_planes - 1) * P.n_tx * P.n_ax + iz;
+        tq[q] = P.tab + ((size_t)min(plane0 + q, P.n_planes - 1) * P.n_ax + iz) * P.tab_kpad;
+        asm("" : "+l"(tq[q]));      // keep it a pointer register pair (address = one IMAD.WIDE per load)
     }
     const size_t ev_stride = (size_t)P.n_rx_max * P.l_row;
+    // one gather-sample of plane q: t = {bits of f0m, n0} of (plane, angle, depth row), row = the (angle, element) row
+    auto term = [&](int tf, int tn, const float4 *row, float H, float w, float &accr, float &acci) {
+        const float upm = __int_as_float(tf) + H;
+        const float tt = upm + kMagic;
+        const float al = upm - (tt - kMagic);
+        const int idx = tn + (__float_as_int(tt) - kMagicBits);
+        float s, c;
+        __sincosf(fmaf(th, al, th0), &s, &c);       // E(a), a = al + 0.5 in [0, 1]
+        if (APOD) { s *= w; c *= w; }
+        const float4 e = __ldg(row + idx);
+        const float vr = fmaf(al, e.z, e.x), vi = fmaf(al, e.w, e.y);
+        accr = fmaf(c, vr, accr); accr = fmaf(-s, vi, accr);
+        acci = fmaf(s, vr, acci); acci = fmaf(c, vi, acci);
+    };
     for (int j = 0; j < P.n_rx; ++j) {
         const float dxs = xs - P.ejs[j];
         const float dx2 = dxs * dxs;
@@ -770,22 +786,23 @@ __global__ void __launch_bounds__(128) das_volume_kernel(DasParams P) {
             if (w == 0.f) continue;
         }
         const float4 *row = P.rows + ((size_t)P.e0 * P.n_rx_max + j) * P.l_row;
-        for (int k = 0; k < P.n_tx; ++k, row += ev_stride) {
-            const int tk = k * P.n_ax;
+        // the table rows are [plane][iz][angle], padded to an even angle count: one LDG.128 serves two angles
+        int k = 0;
+        for (; k + 1 < P.n_tx; k += 2, row += 2 * ev_stride) {
+            const float4 *row1 = row + ev_stride;
+            asm("" : "+l"(row), "+l"(row1));
 #pragma unroll
             for (int q = 0; q < NP; ++q) {
-                const int2 t = __ldg(tq[q] + tk);
-                const float upm = __int_as_float(t.x) + H;
-                const float tt = upm + kMagic;
-                const float al = upm - (tt - kMagic);
-                const int idx = t.y + (__float_as_int(tt) - kMagicBits);
-                float s, c;
-                __sincosf(fmaf(th, al, th0), &s, &c);       // E(a), a = al + 0.5 in [0, 1]
-                if (APOD) { s *= w; c *= w; }
-                const float4 e = __ldg(row + idx);
-                const float vr = fmaf(al, e.z, e.x), vi = fmaf(al, e.w, e.y);
-                ar[q] = fmaf(c, vr, ar[q]); ar[q] = fmaf(-s, vi, ar[q]);
-                ai[q] = fmaf(s, vr, ai[q]); ai[q] = fmaf(c, vi, ai[q]);
+                const int4 t = __ldg(reinterpret_cast<const int4 *>(tq[q] + k));
+                term(t.x, t.y, row, H, w, ar[q], ai[q]);
+                term(t.z, t.w, row1, H, w, ar[q], ai[q]);
+            }
+        }
+        if (k < P.n_tx) {
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                const int2 t = __ldg(tq[q] + k);
+                term(t.x, t.y, row, H, w, ar[q], ai[q]);
             }
         }
     }
