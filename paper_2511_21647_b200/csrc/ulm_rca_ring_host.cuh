@@ -190,7 +190,8 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     L.n_items = L.n_groups * (L.ap[0].n_tiles * (L.per_angle ? L.ap[0].n_tx : 1) + L.ap[1].n_tiles * (L.per_angle ? L.ap[1].n_tx : 1));
     if (L.n_items == 0) return 0;
     // tail splitting: the items of the last, partially filled round are cut into slices of the receive elements
-    const int rem = L.n_items > cfg.n_sms ? L.n_items % cfg.n_sms : 0;
+    // (a call with fewer items than SMs -- a single frame -- is one partially filled round: n_whole = 0)
+    const int rem = L.n_items % cfg.n_sms;
     int n_rx_min = 1 << 30;
     for (int a = 0; a < 2; ++a) if (L.ap[a].n_tiles > 0) n_rx_min = std::min(n_rx_min, L.ap[a].n_rx);
     L.split_s = ring_split_choice(rem, cfg.n_sms, n_rx_min, cfg.partial_cap);

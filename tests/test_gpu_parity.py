@@ -427,7 +427,7 @@ def test_many_frames_cross_group_boundaries(torch_cuda):
     ch = synth.random_channel(cfg, 25, seed=29, amplitude=3000)
     ch = (ch.astype(np.int32) + synth.random_channel(cfg, 25, seed=30, amplitude=3000)).astype(np.int16)
     gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=dict(max_frames=25))
-    assert info["launches_last_call"] == 2
+    assert info["launches_last_call"] in (2, 3)     # 3: fewer work items than SMs, cut into element slices
 
 
 def test_tail_split_of_the_last_round(torch_cuda):
