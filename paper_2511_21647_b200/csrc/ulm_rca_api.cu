@@ -401,6 +401,7 @@ cudaError_t launch_demod(const ulm_rca_plan &P, const int16_t *d_channel, int n_
     D.full_channels = P.cpe == P.n_rows + P.n_cols;
     D.n_lo = P.n_lo; D.l_row = P.l_row;
     D.chunks_per_row = (P.l_row + ulm::kDemodChunk - 1) / ulm::kDemodChunk;
+    D.dc = P.demod;
     const int F = group_frames(n_frames);
     const dim3 blocks((unsigned)D.chunks_per_row, (unsigned)P.n_rx_max, (unsigned)(((n_frames + F - 1) / F) * D.n_events));
     ++P.last_launches;
@@ -529,7 +530,6 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     P.l_row = ((n_hi - P.n_lo + 1) + 7) / 8 * 8;
 
     if (ulm_rca_status s = build_demod(P, opt->demod_taps)) return s;
-    CUDA_TRY(cudaMemcpyToSymbol(ulm::c_demod, &P.demod, sizeof(P.demod)));
     {   // exp(-j 2 pi fc t_n): mixes RF input down; its conjugate rho_n rotates every scratch entry (both input kinds)
         P.mix_n0 = P.n_lo - P.half_len;
         const int n_mix = P.l_row + 2 * P.half_len + 264;

@@ -49,7 +49,8 @@ constexpr int kDemodChunk = 126;             // entries per demodulation CTA (ev
 // difference term, 16 F bytes + 16 bytes of padding that keep the entry an odd multiple of 16 B)
 __host__ __device__ constexpr int entry_bytes(int F, bool D32) { return D32 ? 16 * F + 16 : 10 * F; }
 
-// Demodulation constants (per plan), in constant memory.
+// Demodulation constants (per plan); they travel inside the kernel parameters (constant bank 0: unrolled taps are
+// FFMA constant operands), so plans with different filters can be alive and in flight at the same time.
 struct DemodConst {
     int half_len;            // L
     float gd[kMaxTaps];      // dense taps: gd[t] = 2 h[t - L], t = 0..2L   ({1} for IQ input)
@@ -68,6 +69,7 @@ struct DemodParams {
     int full_channels;       // 1: channels_per_event = n_rows + n_cols
     int n_lo, l_row;         // scratch origin (absolute sample of entry 0) and entries per row
     int chunks_per_row;
+    DemodConst dc;
 };
 
 
@@ -155,7 +157,6 @@ __device__ __forceinline__ void zero_edge_entries(unsigned char *s_out, int eb, 
 // NT = dense tap count 2L+1 (0: run-time L).  Lanes of a half-warp are the frames of one group, so every
 // shared-memory access of step (2) is conflict free (row stride of x = 1 mod 16 float2).
 // ---------------------------------------------------------------------------------------------------
-__constant__ DemodConst c_demod[1];
 
 __host__ __device__ constexpr int demod_threads_per_group(int F) { return F == 12 ? 16 : F; }
 __host__ __device__ inline int demod_xs(int L) { return ((kDemodChunk + 2 + 2 * L) + 14) / 16 * 16 + 1; }
@@ -164,13 +165,13 @@ __host__ __device__ inline int demod_smem_bytes(int F, bool D32, int L) {
 }
 
 template <int NT, int ZS, bool IQ_INPUT, int F, bool D32>
-__global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
+__global__ void __launch_bounds__(256) demod_kernel(const __grid_constant__ DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
     constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
     constexpr int R = 8;                       // entries per thread
     constexpr int TPG = demod_threads_per_group(F);
-    const int L = NT > 0 ? (NT - 1) / 2 : c_demod[0].half_len;
+    const int L = NT > 0 ? (NT - 1) / 2 : P.dc.half_len;
     const int XW = kDemodChunk + 2 + 2 * L;    // mixed samples per frame: iq[0..128] needs x[0 .. 128 + 2L]
     const int XS = demod_xs(L);                // row stride of s_x (float2)
     unsigned char *s_out = s_raw;              // [126][EB] image of the output block
@@ -277,8 +278,8 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
                 for (int q = 0; q <= R; ++q) {
                     const int t = q - u + (NT - 1);
                     if (t >= 0 && t < NT && !(ZS > 0 && t != NT / 2 && ((t - NT / 2) % ZS) == 0)) {
-                        ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
-                        ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
+                        ar[q] = fmaf(P.dc.gd[t], xv.x, ar[q]);
+                        ai[q] = fmaf(P.dc.gd[t], xv.y, ai[q]);
                     }
                 }
             }
@@ -289,8 +290,8 @@ __global__ void __launch_bounds__(256) demod_kernel(DemodParams P) {
                 for (int q = 0; q <= R; ++q) {
                     const int t = q - u + 2 * L;
                     if (t >= 0 && t <= 2 * L) {
-                        ar[q] = fmaf(c_demod[0].gd[t], xv.x, ar[q]);
-                        ai[q] = fmaf(c_demod[0].gd[t], xv.y, ai[q]);
+                        ar[q] = fmaf(P.dc.gd[t], xv.x, ar[q]);
+                        ai[q] = fmaf(P.dc.gd[t], xv.y, ai[q]);
                     }
                 }
             }
@@ -360,7 +361,7 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
 }
 
 template <int F, bool D32>
-__global__ void __launch_bounds__(256, 4) demod_quad_kernel(DemodParams P) {
+__global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constant__ DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
     constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
@@ -449,8 +450,8 @@ __global__ void __launch_bounds__(256, 4) demod_quad_kernel(DemodParams P) {
 #pragma unroll
                 for (int q = 0; q < 9; ++q) {
                     const int t = q - u + 2 * L;                    // tap m = t - L
-                    if (t == L) A[q] = c_demod[0].qd[L] * xv;
-                    else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(c_demod[0].qd[t], xv, B[q]);
+                    if (t == L) A[q] = P.dc.qd[L] * xv;
+                    else if (t >= 0 && t <= 2 * L && ((t - L) & 1)) B[q] = fmaf(P.dc.qd[t], xv, B[q]);
                 }
             }
             demod_quad_emit<F, D32>(A, B, r0, f, s_out);

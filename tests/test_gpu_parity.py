@@ -243,6 +243,32 @@ def test_plan_reuse_and_determinism(torch_cuda):
                 assert np.abs(a - ref17[:n]).max() <= 5e-5 * np.abs(ref17).max()
 
 
+def test_two_live_plans_with_different_filters(torch_cuda):
+    """Plans with different demodulation filters (default 17 taps, 25 taps, fs = 5 fc with 21 taps) are alive at the same
+    time and used in turn, on two streams: each keeps its own constants (they travel in the kernel parameters)."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    cfgs = [small(n_frames=3), small(n_frames=3, demod_taps=25), small(n_frames=3, fs=25e6)]
+    kws = [rounded_kwargs(c) for c in cfgs]
+    chs = [synth.random_channel(c, 3, seed=70 + i, amplitude=6000) for i, c in enumerate(cfgs)]
+    refs = [oracle.beamform(oracle.OracleParams(**kw), ch) for kw, ch in zip(kws, chs)]
+    plans = [Plan(**kw, precision=2) for kw in kws]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    try:
+        d_chs = [torch.from_numpy(ch).cuda() for ch in chs]
+        torch.cuda.synchronize()
+        outs = [None] * len(plans)
+        for rep in range(2):
+            for i in (2, 0, 1):
+                outs[i] = plans[i].beamform(d_chs[i], stream=streams[i % 2])
+        torch.cuda.synchronize()
+        for out, ref in zip(outs, refs):
+            assert_parity(out.cpu().numpy(), ref, tol=NOISE_TOL_FULL)
+    finally:
+        for plan in plans:
+            plan.close()
+
+
 def test_zero_frames_and_bad_buffers(torch_cuda):
     torch = torch_cuda
     from paper_2511_21647_b200 import Plan
