@@ -125,6 +125,8 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geometry,
  *               compound == 1: [frame][ x-z: n_lat*n_ax | y-z: n_lat*n_ax ], axial index fastest
  *               compound == 0: [frame][event][lat][ax]
  * One call in flight per plan (the plan owns the IQ scratch).  n_frames == 0 is a no-op.
+ * A plan belongs to the CUDA device that was current at plan_create; calls made while another device is current
+ * fail with ULM_RCA_EINVAL.  Different plans (any filters, any devices) may be in flight at the same time.
  */
 ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel, int32_t n_frames,
                                 void *d_out, void *cuda_stream);

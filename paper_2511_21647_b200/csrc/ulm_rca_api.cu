@@ -95,6 +95,7 @@ struct ulm_rca_plan {
     double pitch = 0, c = 0, fs = 0, fc = 0, t_start = 0, f_number = 0;
     int input_kind = 0, cpe = 0, n_samples = 0, compound = 1, max_frames = 32, build_volume = 0;
     int n_events = 0, n_rx_max = 0, half_len = 0;
+    int device = 0;               // the CUDA device that was current at plan_create: owns every buffer of the plan
     int nv_events = 0;            // folded events of the projection path (= n_events when nothing folds)
     DeviceBuf ev_fold, ev_id;     // short2 per scratch event row: the (first, second or -1) real events it holds
     bool apod = false;
@@ -426,6 +427,15 @@ size_t host_upload_bytes_per_frame(const ulm_rca_plan &P) {
     return n * (size_t)(s_hi - s_lo) * (P.input_kind == 1 ? 4 : 2);
 }
 
+// the plan's tables and scratch live on the device that was current at plan_create; a call made with another
+// current device would launch there on foreign pointers
+ulm_rca_status check_device(const ulm_rca_plan &P) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != P.device) return fail(ULM_RCA_EINVAL, "plan belongs to CUDA device %d, the current device is %d", P.device, dev);
+    return ULM_RCA_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -480,6 +490,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     ulm_rca_plan *Pp = new (std::nothrow) ulm_rca_plan;
     if (!Pp) return fail(ULM_RCA_ENOMEM, "host allocation failed");
     struct Guard { ulm_rca_plan *p; ~Guard() { delete p; } } guard{Pp};
+    CUDA_TRY(cudaGetDevice(&Pp->device));
     ulm_rca_plan &P = *Pp;
     P.n_rows = geo->n_rows; P.n_cols = geo->n_cols; P.pitch = geo->pitch_m;
     P.c = c_mps; P.fs = fs_hz; P.fc = fc_hz; P.t_start = opt->t_start_s; P.f_number = opt->f_number;
@@ -641,6 +652,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
     if (n_frames == 0) return ULM_RCA_OK;
     if (!d_channel || !d_out) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
     const ulm_rca_plan &P = *plan;
+    if (ulm_rca_status s = check_device(P)) return s;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     size_t ch_bytes = 0;
     ulm_rca_plan_sizes(plan, &ch_bytes, nullptr, nullptr);
@@ -721,6 +733,7 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
     if (n_frames == 0) return ULM_RCA_OK;
     if (!d_channel || !d_out_volume) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
     const ulm_rca_plan &P = *plan;
+    if (ulm_rca_status s = check_device(P)) return s;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     size_t ch_bytes = 0;
     ulm_rca_plan_sizes(plan, &ch_bytes, nullptr, nullptr);
@@ -761,6 +774,7 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
     if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
     if (n_frames == 0) return ULM_RCA_OK;
     if (!h_channel || !h_out) return fail(ULM_RCA_EINVAL, "host pointer is NULL");
+    if (ulm_rca_status s = check_device(*plan)) return s;
     size_t ch_bytes = 0, out_bytes = 0;
     ulm_rca_plan_sizes(plan, &ch_bytes, &out_bytes, nullptr);
     if (plan->h_stage_frames < (size_t)n_frames) {
