@@ -111,6 +111,7 @@ struct ulm_rca_plan {
     bool quad = false;            // fs = 4 fc exactly, default 17 taps, analytic signal from two real filters
     bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
     bool quarter_band = false;    // every fourth demodulation tap except the centre is exactly zero (fs = 8 fc)
+    bool analytic8 = false;       // RF input, fs = 8 fc exactly, 33 taps: analytic signal from two real filters (ga, gb)
     ulm::RingConfig ring{};
     long long out_per_frame = 0, vol_per_frame = 0;
     mutable long long last_launches = 0;
@@ -256,6 +257,26 @@ ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
             D.qd[t] = (m == 0) ? (float)(h[t] / sum) : (m4 == 1 ? (float)(h[t] / sum) : m4 == 3 ? (float)(-h[t] / sum) : 0.f);
         }
     }
+    // analytic variant at fs = 8 fc with the default 33 taps: s[n] = sum_m g[m] rf[n-m] exp(j theta m), theta = pi/4
+    P.analytic8 = false;
+    if (P.input_kind == 0 && L == 16 && P.quarter_band && P.fs == 8.0 * P.fc) {
+        const double oct[8][2] = {{1, 0}, {M_SQRT1_2, M_SQRT1_2}, {0, 1}, {-M_SQRT1_2, M_SQRT1_2},
+                                  {-1, 0}, {-M_SQRT1_2, -M_SQRT1_2}, {0, -1}, {M_SQRT1_2, -M_SQRT1_2}};
+        bool ok = true;
+        for (int t = 0; t <= 2 * L; ++t) {
+            const int m = t - L, m8 = ((m % 8) + 8) % 8, m4 = m8 % 4;
+            const double g = 2.0 * h[t] / sum;
+            D.ga[t] = D.gd[t] == 0.f ? 0.f : (float)(g * oct[m8][0]);
+            D.gb[t] = D.gd[t] == 0.f ? 0.f : (float)(g * oct[m8][1]);
+            // the zero pattern the kernel skips at compile time
+            if (m4 == 0 && m != 0 && (D.ga[t] != 0.f || D.gb[t] != 0.f)) ok = false;
+            if (m4 == 2 && D.ga[t] != 0.f) ok = false;
+            if (m == 0 && D.gb[t] != 0.f) ok = false;
+        }
+        D.rot1[0] = (float)M_SQRT1_2;
+        D.rot1[1] = (float)M_SQRT1_2;
+        P.analytic8 = ok;
+    }
     return ULM_RCA_OK;
 }
 
@@ -359,16 +380,16 @@ void launch_volume(const ulm_rca_plan &P, const ulm::DasParams &D, cudaStream_t 
     ++P.last_launches;
 }
 
-template <int NT, int ZS, bool IQ, int F, bool D32>
+template <int NT, int ZS, bool IQ, int F, bool D32, bool AN = false>
 cudaError_t launch_demod_t(const ulm::DemodParams &D, int L, dim3 blocks, cudaStream_t st) {
     const size_t smem = (size_t)ulm::demod_smem_bytes(F, D32, L);
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, ZS, IQ, F, D32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(ulm::demod_kernel<NT, ZS, IQ, F, D32, AN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     // as in the quadrature kernel: one CTA per scratch row walks its chunks when there are enough rows
     if ((long long)blocks.y * blocks.z >= 2048) blocks.x = 1;
-    ulm::demod_kernel<NT, ZS, IQ, F, D32><<<blocks, 256, smem, st>>>(D);
+    ulm::demod_kernel<NT, ZS, IQ, F, D32, AN><<<blocks, 256, smem, st>>>(D);
     return cudaSuccess;
 }
 
@@ -386,6 +407,7 @@ cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim
     }
     if (L == 8) return P.half_band ? launch_demod_t<17, 2, false, F, D32>(D, L, blocks, st)
                                    : launch_demod_t<17, 0, false, F, D32>(D, L, blocks, st);
+    if (L == 16 && P.analytic8) return launch_demod_t<33, 4, false, F, D32, true>(D, L, blocks, st);
     if (L == 16) return P.quarter_band ? launch_demod_t<33, 4, false, F, D32>(D, L, blocks, st)
                                        : launch_demod_t<33, 0, false, F, D32>(D, L, blocks, st);
     return launch_demod_t<0, 0, false, F, D32>(D, L, blocks, st);

@@ -55,6 +55,10 @@ struct DemodConst {
     int half_len;            // L
     float gd[kMaxTaps];      // dense taps: gd[t] = 2 h[t - L], t = 0..2L   ({1} for IQ input)
     float qd[17];            // quadrature path (fs = 4 fc, L = 8): qd[8] = h[0], qd[t] = h[m] j^(m-1) for odd m = t - 8
+    // analytic path (RF input, fs = 8 fc, 33 taps): two REAL filters ga[t] = gd[t] cos(theta m), gb[t] = gd[t] sin(theta m),
+    // m = t - L, theta = 2 pi fc / fs, give s[n] = iq[n] rho_n = A + jB directly; rot1 = (cos theta, sin theta)
+    float ga[33], gb[33];
+    float rot1[2];
 };
 
 struct DemodParams {
@@ -164,8 +168,13 @@ __host__ __device__ inline int demod_smem_bytes(int F, bool D32, int L) {
     return kDemodSlots * entry_bytes(F, D32) + F * demod_xs(L) * 8;
 }
 
-template <int NT, int ZS, bool IQ_INPUT, int F, bool D32>
+// AN = analytic variant (RF input, NT = 33, ZS = 4, i.e. fs = 8 fc): no mixer; the staging buffer holds the REAL samples
+// and the two real filters ga / gb (17 + 24 non-zero taps: ga[m] = 0 for m = 2 mod 4, both 0 for m = 0 mod 4, m != 0,
+// gb[0] = 0 -- checked on the host) give the analytic signal s[n] = A + jB, so an entry needs one constant rotation
+// B_n = s[n+1] exp(-j theta) instead of two table rotations: 41 real FMAs per output instead of 50 + mixing.
+template <int NT, int ZS, bool IQ_INPUT, int F, bool D32, bool AN = false>
 __global__ void __launch_bounds__(256) demod_kernel(const __grid_constant__ DemodParams P) {
+    static_assert(!AN || (!IQ_INPUT && NT == 33 && ZS == 4), "analytic variant: RF input, 33 taps at fs = 8 fc");
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
     constexpr int OUT_BYTES = kDemodSlots * EB;      // every entry slot a thread can address (a multiple of 128 B)
@@ -231,6 +240,12 @@ __global__ void __launch_bounds__(256) demod_kernel(const __grid_constant__ Demo
             const int n = base - L + i;
             const bool inb = n >= 0 && n < P.n_samples;
             float2 *dst = s_x + (h * FH) * XS + i;
+            if (AN) {
+                float *dr_ = reinterpret_cast<float *>(s_x) + (h * FH) * XS + i;
+#pragma unroll
+                for (int f = 0; f < FH; ++f) dr_[f * XS] = (inb && f <= f_last) ? (float)(ra[rep][f] + rb[rep][f]) : 0.f;
+                continue;
+            }
             float2 m = make_float2(1.f, 0.f);
             if (!IQ_INPUT && inb) m = __ldg(P.mixer + (n - P.mix_n0));
 #pragma unroll
@@ -270,7 +285,22 @@ __global__ void __launch_bounds__(256) demod_kernel(const __grid_constant__ Demo
         float ar[R + 1], ai[R + 1];
 #pragma unroll
         for (int q = 0; q <= R; ++q) ar[q] = ai[q] = 0.f;
-        if (NT > 0) {
+        if (AN) {
+            const float *xr = reinterpret_cast<const float *>(s_x) + f * XS + r0;
+#pragma unroll
+            for (int u = 0; u < R + NT; ++u) {
+                const float xv = xr[u];
+#pragma unroll
+                for (int q = 0; q <= R; ++q) {
+                    const int t = q - u + (NT - 1);
+                    const int m4 = ((t - NT / 2) % 4 + 4) % 4;
+                    if (t >= 0 && t < NT && (m4 != 0 || t == NT / 2)) {
+                        if (m4 != 2) ar[q] = fmaf(P.dc.ga[t], xv, ar[q]);
+                        if (t != NT / 2) ai[q] = fmaf(P.dc.gb[t], xv, ai[q]);
+                    }
+                }
+            }
+        } else if (NT > 0) {
 #pragma unroll
             for (int u = 0; u < R + NT; ++u) {
                 const float2 xv = x[u];
@@ -301,10 +331,19 @@ __global__ void __launch_bounds__(256) demod_kernel(const __grid_constant__ Demo
             const int ent = r0 + q;               // < kDemodSlots: slots past n_ent are written but never copied out
             const float m0r = 0.5f * (ar[q] + ar[q + 1]), m0i = 0.5f * (ai[q] + ai[q + 1]);
             const float d0r = ar[q + 1] - ar[q], d0i = ai[q + 1] - ai[q];
-            // rotate by rho_n = conj(mixer[n]) (one broadcast load per entry: all frames share n)
-            const float2 mx = __ldg(P.mixer + (base + ent - P.mix_n0));
-            const float mr = fmaf(m0r, mx.x, m0i * mx.y), mi = fmaf(m0i, mx.x, -m0r * mx.y);
-            const float dr = fmaf(d0r, mx.x, d0i * mx.y), di = fmaf(d0i, mx.x, -d0r * mx.y);
+            float mr, mi, dr, di;
+            if (AN) {
+                // A_n = s[n] = (ar, ai)[q];  B_n = s[n+1] exp(-j theta)
+                const float c1 = P.dc.rot1[0], s1 = P.dc.rot1[1];
+                const float br = fmaf(ar[q + 1], c1, ai[q + 1] * s1), bi = fmaf(ai[q + 1], c1, -ar[q + 1] * s1);
+                mr = 0.5f * (ar[q] + br); mi = 0.5f * (ai[q] + bi);
+                dr = br - ar[q]; di = bi - ai[q];
+            } else {
+                // rotate by rho_n = conj(mixer[n]) (one broadcast load per entry: all frames share n)
+                const float2 mx = __ldg(P.mixer + (base + ent - P.mix_n0));
+                mr = fmaf(m0r, mx.x, m0i * mx.y); mi = fmaf(m0i, mx.x, -m0r * mx.y);
+                dr = fmaf(d0r, mx.x, d0i * mx.y); di = fmaf(d0i, mx.x, -d0r * mx.y);
+            }
             unsigned char *ep = s_out + ent * EB;
             if (D32) {
                 store_full_entry<F>(ep, f, mr, mi, dr, di);

@@ -104,7 +104,7 @@ def test_config0_full(torch_cuda, kernel):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("case", ["rf", "rf_full", "iq", "iq_bandlimited_compact", "apod", "orth", "fs25", "neg_dlat",
-                                  "taps9", "one_aperture", "t_start_odd"])
+                                  "taps9", "one_aperture", "t_start_odd", "fs40", "fs40_taps25", "fs40_edges"])
 def test_small_variants(torch_cuda, kernel, case):
     extra = {}
     cfg = small()
@@ -133,6 +133,15 @@ def test_small_variants(torch_cuda, kernel, case):
         # fs = 4 fc with fc * t_start NOT a multiple of a quarter cycle: the quadrature pre-pass (analytic signal from
         # two real filters, no mixer) must still apply -- its entries carry the sample's own phase exactly
         cfg = small(t_start=0.937e-6)
+    elif case == "fs40":
+        # fs = 8 fc with the default 33 taps: the analytic pre-pass (two real filters, no mixer), t_start off the grid
+        cfg = small(fs=40e6, n_samples=1400, t_start=0.913e-6)
+    elif case == "fs40_taps25":
+        cfg = small(fs=40e6, n_samples=1400, demod_taps=25)      # same sampling, other tap count: the generic path
+    elif case == "fs40_edges":
+        # records so short that the image runs past both ends: the zero padding of the filter and the edge rule
+        g = small().grid_xz
+        cfg = small(fs=40e6, n_samples=520, t_start=3.2e-6, grid_xz=g[:3] + (70, 2e-3, g[5], g[6]))
     ch = synth.random_channel(cfg, cfg.n_frames, seed=17, amplitude=6000)
     if case == "iq_bandlimited_compact":
         # the compact format is meant for band-limited IQ: smooth the white data along the sample axis
@@ -508,3 +517,68 @@ def test_shape_sweep_ring_kernel(torch_cuda, shape):
     gpu, ref, info = run_pair(torch_cuda, cfg, ch, plan_extra=dict(max_frames=nf, precision=1))
     assert info["kernel"] == 2 and info["precision"] == 1
     assert_parity(gpu, ref, tol=3e-4)
+
+
+def _random_case(rng):
+    """One random small configuration: array, angle sets (symmetric ones fold), grids, frames, apodisation, mode."""
+    d = synth.LAMBDA_M / 2
+    n_rows, n_cols = int(rng.integers(4, 70)), int(rng.integers(4, 70))
+    kr, kc = int(rng.integers(0, 6)), int(rng.integers(0, 6))
+    if kr + kc == 0:
+        kr = 1
+    sym = rng.random() < 0.5
+
+    def angles(k):
+        if sym:
+            return tuple(np.radians(np.linspace(-1, 1, k) * rng.uniform(1, 10) if k > 1 else np.zeros(k)))
+        return tuple(np.radians(rng.uniform(-10, 10, k)))
+
+    volume = rng.random() < 0.25
+    nf = int(rng.choice([1, 2, 3, 5]) if volume else rng.choice([1, 2, 3, 4, 5, 12, 13, 25, 30]))
+    nlx, nly, nax = int(rng.integers(1, 120)), int(rng.integers(1, 120)), int(rng.integers(1, 90))
+    nay = int(rng.integers(1, 90))
+    if volume:
+        nlx, nly, nax = min(nlx, 24), min(nly, 24), min(nax, 30)
+        nay = nax
+    dz, z0 = d * rng.uniform(0.4, 1.5), rng.uniform(3e-3, 8e-3)
+    ref_x, ref_y = (0.0, 0.0) if sym else (rng.uniform(-1e-3, 1e-3), rng.uniform(-1e-3, 1e-3))
+    t0 = None if (sym or rng.random() < 0.5) else tuple(rng.uniform(-0.2e-6, 0.2e-6, kr + kc))
+    cfg = synth.config(0).with_(
+        n_rows=n_rows, n_cols=n_cols, pitch=float(rng.uniform(0.15e-3, 0.35e-3)), n_samples=int(rng.integers(600, 1400)),
+        row_tx_angles=angles(kr), col_tx_angles=angles(kc),
+        grid_xz=centred_grid(nlx, d * rng.uniform(0.3, 1.2), nax, z0, dz, ref=ref_y),
+        grid_yz=centred_grid(nly, d * rng.uniform(0.3, 1.2), nay, z0, dz, ref=ref_x),
+        n_frames=nf, t_start=float(rng.uniform(0, 1e-6)), t0=t0, f_number=float(rng.choice([0.0, 0.0, 1.0, 1.7])),
+        compound=int(rng.random() < 0.7))
+    extra = dict(kernel=int(rng.choice([0, 0, 1])), max_frames=int(rng.choice([nf, max(1, nf // 2), 32])),
+                 build_volume=bool(volume), precision=2)
+    return cfg, nf, extra
+
+
+@pytest.mark.parametrize("block", range(4))
+def test_random_shapes(torch_cuda, block):
+    """Seeded random configurations (40 per block) against the oracle with full-precision entries, where only fp32
+    rounding separates the two (2e-5 on white noise): array sizes, 0..5 angles per aperture (symmetric sets fold),
+    one-pixel to multi-tile grids, 1..30 frames in batches, f-number masks, per-angle output, both DAS kernels, and
+    the volume path on a quarter of the cases."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    for it in range(40):
+        rng = np.random.default_rng(7000 + 40 * block + it)
+        cfg, nf, extra = _random_case(rng)
+        ch = synth.random_channel(cfg, nf, seed=int(rng.integers(1 << 30)), amplitude=5000)
+        kw = rounded_kwargs(cfg)
+        p = oracle.OracleParams(**kw)
+        with Plan(**kw, **extra) as plan:
+            d_ch = torch.from_numpy(ch).cuda()
+            out = plan.beamform(d_ch).cpu().numpy()
+            vol = plan.beamform_volume(d_ch).cpu().numpy() if extra["build_volume"] else None
+        err = rel_err(out, oracle.beamform(p, ch))
+        if vol is not None:
+            gx, gy = kw["grid_xz"], kw["grid_yz"]
+            xs, ys = gx[1] + gx[2] * np.arange(gx[0]), gy[1] + gy[2] * np.arange(gy[0])
+            zs = gx[4] + gx[5] * np.arange(gx[3])
+            for f in range(nf):
+                v_rc, v_cr = oracle.volume(p, ch[f], xs, ys, zs)
+                err = max(err, rel_err(vol[f], v_rc + v_cr))
+        assert err <= NOISE_TOL_FULL, (block, it, err, cfg)
