@@ -247,7 +247,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
 # capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {2: 3.666862e9 + 0.136388e9}     # profiles/r01_v5_ncu.md
+TRAFFIC_BYTES = {2: 3.677742e9 + 0.195292e9}     # profiles/r01_v7_ncu.md (das_ring_kernel<12,4,0,0>, one launch)
 
 
 def run_volume(args):
@@ -293,7 +293,7 @@ def run_volume(args):
         "gather_samples_per_s": gathers / (ms * 1e-3),
         "projection_path_ms_same_frame": ms_proj, "volume_over_projection_time": ms / ms_proj,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None, "kernel": "das_volume_kernel<4,0>"},
+                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": 19.985152e6 + 0.501760e6, "kernel": "das_volume_kernel<4,0>"},
         "gpu_launches": launches * args.steps}))
 
 
