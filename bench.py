@@ -247,7 +247,8 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
 # capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {2: 3.677742e9 + 0.195292e9}     # profiles/r01_v7_ncu.md (das_ring_kernel<12,4,0,0>, one launch)
+TRAFFIC_BYTES = {2: 3.677742e9 + 0.195292e9,      # profiles/r01_v7_ncu.md (das_ring_kernel<12,4,0,0>, one launch)
+                 3: 7.129134e9 + 0.556273e9}      # profiles/r01_v7_cfg3.md
 
 
 def run_volume(args):
