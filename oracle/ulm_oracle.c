@@ -148,14 +148,12 @@ static double complex *demod_frame(const ulm_oracle_params *p, const int16_t *fr
     return iq;
 }
 
-/* boxcar f-number mask.  The in/out decision is taken in fp32 on fp32-rounded
- * coordinates: |lat - lat_elem| * (2 F#) <= z. */
+/* boxcar f-number mask, w_j = [f_number = 0 or |lat - lat_j| <= z / (2 f_number)],
+ * evaluated in fp64 exactly as the definition writes it (the edge is inclusive). */
 static int in_aperture(double f_number, double lat, double lat_elem, double z)
 {
     if (f_number == 0.0) return 1;
-    volatile float d = fabsf((float)lat - (float)lat_elem);
-    volatile float lhs = d * (float)(2.0 * f_number);
-    return lhs <= (float)z;
+    return fabs(lat - lat_elem) <= z / (2.0 * f_number);
 }
 
 /*

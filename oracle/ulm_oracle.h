@@ -10,10 +10,12 @@
  * build, load or call this library.  It shares no code, header, table or constant with the CUDA
  * path under paper_2511_21647_b200/ and neither includes the other.
  *
- * Parity pins (tests/test_oracle_pins.py): P1 impulse closed form, P2 phase convention,
- * P3 demodulation of a pure tone, P4 independently coded 3-D DAS == projection on the reference
- * plane, P5 linearity, P7 point-scatterer peak, P8 symmetries, P9 work count.
- * Parity unpinned: nothing in this file (the Stage-2 shift law, is not implemented).
+ * Parity pins (tests/test_oracle_pins.py): P1 impulse closed form, P2 phase convention and the
+ * f-number mask counted over whole grids against the fp64 inequality (near-edge and on-edge pairs),
+ * P3 demodulation of a pure tone and the FIR taps against literal values and numpy's sinc / hamming,
+ * P4 independently coded 3-D DAS == projection on the reference plane, P5 linearity,
+ * P7 point-scatterer peak, P8 symmetries, P9 work count.
+ * Every decision and every value in this file is fp64.  Parity unpinned: nothing in this file.
  */
 #ifndef ULM_ORACLE_H
 #define ULM_ORACLE_H

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libulm_rca.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--use_fast_math=false", "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
 
 
 def sources():
@@ -30,8 +30,7 @@ def _deps():
 def build(force: bool = False, verbose: bool = False) -> str:
     stale = (not os.path.exists(LIB)) or any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in _deps())
     if force or stale:
-        flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-        cmd = ["nvcc"] + flags + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
               ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-o", LIB] + sources()
         res = subprocess.run(cmd, cwd=HERE, capture_output=True, text=True)
         if verbose or res.returncode:
@@ -41,16 +40,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_probe() -> str:
-    """Compile the stand-alone shared-memory / pipe-rate micro-benchmark (probes/smem_probe.cu)."""
-    out = os.path.join(HERE, "probes", "smem_probe")
-    src = os.path.join(HERE, "probes", "smem_probe.cu")
-    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", out, src], check=True, cwd=HERE)
-    return out
-
-
 if __name__ == "__main__":
-    if "--probe" in sys.argv:
-        print(build_probe())
-    else:
-        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -144,6 +144,57 @@ def test_p2_matched_phase_sums_coherently(f_number):
         assert abs(got) >= np.abs(img).max() * (1 - 1e-9)          # and it is the image maximum
 
 
+def test_p2_f_number_mask_counts_over_a_whole_grid():
+    """w_j = [|lat - lat_j| <= z / (2 F#)], decided in fp64, edge inclusive.  With fc = 0 the
+    rotation is 1 and constant IQ data A makes every term contribute exactly A, so P(lat, z) = A * K * (number of
+    in-mask elements): the oracle's count is compared, over every pixel of both grids, with the inequality written
+    out here.  F# is chosen so that one (pixel, element) pair sits 1e-10 (relative) INSIDE the edge, then 1e-10
+    OUTSIDE: a decision taken in fp32, on rounded coordinates or with the wrong side / strictness miscounts it."""
+    cfg = tiny(t0=None, t_start=0.0)
+    A = 1000
+    ch = np.zeros(cfg.channel_shape, dtype=np.int16)
+    ch[..., 0] = A
+    rng = np.random.default_rng(12)
+    for trial in range(12):
+        row_tx = trial % 2 == 0
+        g = cfg.grid_xz if row_tx else cfg.grid_yz
+        lat, z, _ = grid_axes(g)
+        n_el = cfg.n_cols if row_tx else cfg.n_rows
+        lat_j = elem_pos(np.arange(n_el), n_el, cfg.pitch)
+        il, iz, j = int(rng.integers(g[0])), int(rng.integers(g[3])), int(rng.integers(n_el))
+        dx = abs(lat[il] - lat_j[j])
+        if dx < 1e-5:
+            continue
+        for side in (-1.0, +1.0):
+            f_number = z[iz] / (2.0 * dx) * (1.0 + side * 1e-10)     # side < 0: the pair is just inside
+            p = params(cfg, fc=0.0, f_number=f_number)
+            out = oracle.beamform(p, ch)[0]
+            for rt, img in zip((True, False), split_projections(p, out)):
+                gg = cfg.grid_xz if rt else cfg.grid_yz
+                la, zz, _ = grid_axes(gg)
+                ne = cfg.n_cols if rt else cfg.n_rows
+                lj = elem_pos(np.arange(ne), ne, cfg.pitch)
+                K = len(cfg.row_tx_angles if rt else cfg.col_tx_angles)
+                inside = np.abs(la[:, None, None] - lj[None, None, :]) <= zz[None, :, None] / (2.0 * f_number)
+                count = inside.sum(-1)
+                np.testing.assert_allclose(img, A * K * count, rtol=0, atol=1e-9)
+                if rt == row_tx:
+                    assert bool(inside[il, iz, j]) == (side < 0)
+    # the edge itself is inclusive: power-of-two coordinates make |lat - lat_j| = z / (2 F#) exact
+    g2 = (9, -4 * 2.0 ** -12, 2.0 ** -12, 8, 2.0 ** -7, 2.0 ** -12, 0.0)
+    cfg2 = tiny(t0=None, t_start=0.0, pitch=2.0 ** -12, grid_xz=g2, grid_yz=g2, n_rows=9, n_cols=9)
+    ch2 = np.zeros(cfg2.channel_shape, dtype=np.int16)
+    ch2[..., 0] = A
+    p2 = params(cfg2, fc=0.0, f_number=4.0)
+    img = split_projections(p2, oracle.beamform(p2, ch2)[0])[0]
+    la, zz, _ = grid_axes(g2)
+    lj = elem_pos(np.arange(9), 9, cfg2.pitch)
+    inside = np.abs(la[:, None, None] - lj[None, None, :]) <= zz[None, :, None] / 8.0
+    on_edge = np.abs(la[:, None, None] - lj[None, None, :]) == zz[None, :, None] / 8.0
+    assert on_edge.sum() >= 4                                        # the case really has pairs on the edge
+    np.testing.assert_allclose(img, A * len(cfg2.row_tx_angles) * inside.sum(-1), rtol=0, atol=1e-9)
+
+
 # ---------------------------------------------------------------------------------------------
 # P3  demodulation of a pure tone at fc
 # ---------------------------------------------------------------------------------------------
@@ -177,6 +228,30 @@ def test_p3_fir_is_symmetric_lowpass_with_unit_dc_gain():
     p33 = params(tiny(input_kind=0, fs=40e6))
     assert len(oracle.fir_taps(p33)) == 33
     assert len(oracle.fir_taps(params(cfg, demod_taps=9))) == 9
+
+
+# the 17 taps at fs = 4 fc, m = 0..8 (h[-m] = h[m]), written out: Hamming-windowed sinc(m/2), normalised to sum 1
+# (SURVEY 8(c) step 0).  A Hann (0.5/0.5) or Blackman window, a sinc of the wrong argument or a missing
+# normalisation changes the 3rd digit of several of them.
+H17_HALF = [0.5008702925771573, 0.3076987787367444, 0.0, -0.07610584574867356, 0.0, 0.023211101786365082, 0.0,
+            -0.005239181063014528, 0.0]
+
+
+def test_p3_fir_taps_literal_and_library_cross_check():
+    """ulm_oracle_fir against numbers stated here and against numpy's own sinc / hamming (a library routine, not the
+    oracle's code): 17 taps (fs = 4 fc), 33 taps (fs = 8 fc), 21 taps (fs = 5 fc), and explicit tap counts."""
+    cfg = tiny(input_kind=0)
+    h = oracle.fir_taps(params(cfg))
+    np.testing.assert_allclose(h[8:], H17_HALF, rtol=0, atol=1e-15)
+    np.testing.assert_allclose(h[:9][::-1], H17_HALF, rtol=0, atol=1e-15)
+    for fs, fc, taps, L in [(20e6, 5e6, 0, 8), (40e6, 5e6, 0, 16), (25e6, 5e6, 0, 10), (20e6, 5e6, 9, 4),
+                            (40e6, 5.21e6, 25, 12), (20e6, 5.21e6, 0, 8)]:
+        hh = oracle.fir_taps(params(tiny(input_kind=0, fs=fs), fc=fc, demod_taps=taps))
+        m = np.arange(-L, L + 1)
+        ref = np.sinc(2.0 * fc * m / fs) * np.hamming(2 * L + 1)
+        ref /= ref.sum()
+        assert len(hh) == 2 * L + 1
+        np.testing.assert_allclose(hh, ref, rtol=0, atol=1e-15)
 
 
 def test_p3_impulse_response_and_zero_padding():
