@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- projection-beamformed frames/s on the 300-frame ensemble (BASELINE.json config 2).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2|3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2|3|4]
 
 One "step" = one pass of the whole hot path (demodulation/staging pre-pass + DAS gather/compound +
 projection write) over one 300-frame ensemble that is already resident in HBM.  Prints ONE JSON line
-(contract in DESIGN.md "Measurement").  N > 1: one process per GPU (torchrun), every rank beamforms its
-own ensemble (frames/ensembles are independent: no data-path collective), value = all frames / max time.
+(contract in DESIGN.md "Measurement").  N > 1: one process per GPU, every rank beamforms its own ensemble
+(frames/ensembles are independent: no data-path collective), value = all frames / max time; when the script is
+started without a launcher (WORLD_SIZE unset) it starts the N ranks itself through torch.distributed.run and fails
+if fewer than N GPUs are visible.
 `--impl reference` times the fp64 CPU oracle (oracle/) on the host cores instead.
 """
 from __future__ import annotations
@@ -74,6 +76,23 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "samples": len(self.samples), "reasons": sorted(self.reasons)}
 
 
+def measured_traffic(config_index: int, precision: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, read from the summary of the
+    `ncu --set full` capture under profiles/ (profiles/r02_traffic.json; its .md names the commands).  None when no
+    capture of that (config, precision) exists."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as fh:
+            rec = json.load(fh)["das_ring_kernel"]["cfg%d_precision%d" % (config_index, precision)]
+        return float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
+    except Exception:
+        return None
+
+
+DTYPE_OF_PRECISION = {1: "f32 accumulate; staged IQ: fp24 mid + fp16 difference, fp16 weight (precision=1, compact-fast)",
+                      2: "f32 (staged IQ, interpolation and accumulation all fp32; precision=2)",
+                      3: "f32 accumulate; staged IQ: fp24 mid + fp16 difference, two-term fp16 weight (precision=3, compact)"}
+
+
 def whole_job(frames_per_rank: int, world: int, ms_local: float, all_reduce_max=None):
     """Whole-job throughput for independent per-rank ensembles: every rank beamforms frames_per_rank frames,
     the job takes the MAX over ranks of the device time (no data-path collective).  all_reduce_max(x) -> max over
@@ -111,15 +130,70 @@ def make_ensemble(cfg, torch, device):
 
 
 def oracle_frames_per_s(cfg, host_frames, n_frames):
-    """Time the fp64 oracle, as it stands, on n_frames frames (demodulation + both projections)."""
+    """Time the fp64 oracle, as it stands, on n_frames frames (demodulation + both projections).  Also returns its
+    output for each distinct host frame it saw ({index into host_frames: complex128 frame})."""
     import oracle
     p = oracle.OracleParams(**rounded_kwargs(cfg))
-    reps = [host_frames[i % host_frames.shape[0]] for i in range(n_frames)]
+    outs = {}
     t0 = time.perf_counter()
-    for fr in reps:
-        oracle.beamform(p, fr[None])
+    for i in range(n_frames):
+        d = i % host_frames.shape[0]
+        outs[d] = oracle.beamform(p, host_frames[d][None])[0]
     dt = time.perf_counter() - t0
-    return n_frames / dt, dt, oracle.threads()
+    return n_frames / dt, dt, oracle.threads(), outs
+
+
+def time_arm(torch, plan, channel, out, steps, warmup, barrier, local_rank, sample_clocks=False):
+    """W untimed + K timed whole-ensemble calls of ulm_rca_beamform on torch's current stream, CUDA events on that
+    stream, barrier + synchronize on both sides.  Returns a dict of timings."""
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        plan.beamform(channel, out=out)
+    barrier()
+    sampler = ClockSampler(local_rank) if sample_clocks else None
+    if sampler:
+        sampler.start()
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    marks[0].record(stream)
+    for i in range(steps):
+        plan.beamform(channel, out=out)
+        marks[i + 1].record(stream)
+    barrier()
+    clocks = sampler.result() if sampler else None
+    per_step = sorted(marks[i].elapsed_time(marks[i + 1]) for i in range(steps))
+    demod_ms, das_ms = plan.timing(min(steps, 64))
+    info = plan.info()
+    return {"ms_step": marks[0].elapsed_time(marks[steps]) / steps, "per_step": per_step, "demod_ms": demod_ms,
+            "das_ms": das_ms, "info": info, "launches": info["launches_last_call"] * steps, "clocks": clocks}
+
+
+def das_roofline(cfg, args, arm, gathers, fp32_probe, world_ms=None):
+    """ALU roofline of the DAS kernel: achieved = 18 flop x EXECUTED gather-samples / the
+    kernel's mean duration (CUDA events the library records on the launching stream); peak = derived FP32 peak,
+    with the in-run FFMA probe beside it."""
+    info = arm["info"]
+    n_events = len(cfg.row_tx_angles) + len(cfg.col_tx_angles)
+    fold = info["events_executed"] / float(n_events)
+    gathers_exec = gathers * fold
+    achieved = FLOP_PER_GATHER * gathers_exec / (arm["das_ms"] * 1e-3) / 1e12
+    achieved_def = FLOP_PER_GATHER * gathers / (arm["das_ms"] * 1e-3) / 1e12
+    ms_step = world_ms if world_ms is not None else arm["ms_step"]
+    # the kernel's own shared-memory floor: bytes of scratch entries gathered per executed term at 128 B/clk/SM
+    smem_floor_ms = gathers_exec * info["scratch_bytes_per_sample"] / (148 * 128 * 1.965e9) * 1e3
+    return {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved / NOMINAL_FP32_TFLOPS,
+            "peak_measured": fp32_probe, "frac_of_measured": (achieved / fp32_probe) if fp32_probe else None,
+            "traffic": measured_traffic(args.config, info["precision"]) if not args.per_angle else None,
+            "kernel": ("das_ring_kernel<12,4,%s,0,%s>" % ("1" if info["precision"] == 2 else "0", "1" if info["precision"] == 3 else "0"))
+            if info["kernel"] == 2 else "das_generic_kernel",
+            "precision": info["precision"], "kernel_ms": arm["das_ms"], "prepass_ms": arm["demod_ms"],
+            "flop_per_gather_sample": FLOP_PER_GATHER, "gather_samples_per_launch": gathers_exec,
+            "gather_samples_of_the_definition": gathers, "events_executed_per_frame": info["events_executed"],
+            "events_per_frame": n_events, "frac_on_definition_count": achieved_def / NOMINAL_FP32_TFLOPS,
+            "peak_source": "derived: 148 SM x 128 lanes x 2 x 1965 MHz (DESIGN.md section 8); peak_measured = the "
+                           "library's register-only FFMA probe run in this process",
+            "whole_step_frac": FLOP_PER_GATHER * gathers_exec / (ms_step * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
+            "smem_floor_ms": smem_floor_ms, "frac_of_smem_floor": smem_floor_ms / arm["das_ms"]}
 
 
 def run_ours(args):
@@ -130,6 +204,9 @@ def run_ours(args):
     rank, local_rank, world = dist_env()
     if world > 1:
         dist.init_process_group("nccl")
+    if torch.cuda.device_count() <= local_rank:
+        sys.stderr.write("bench.py: rank %d needs cuda:%d but only %d device(s) are visible\n" % (rank, local_rank, torch.cuda.device_count()))
+        sys.exit(2)
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
     build.build()
@@ -139,36 +216,23 @@ def run_ours(args):
     n_frames = cfg.n_frames
     channel, host_frames, distinct = make_ensemble(cfg, torch, device)
     gathers = cfg.gather_samples_per_frame() * n_frames
-
-    plan = Plan(**rounded_kwargs(cfg), max_frames=n_frames)
-    out = torch.empty((n_frames, plan.out_complex_per_frame), dtype=torch.complex64, device=device)
-    stream = torch.cuda.current_stream()
+    warmup = max(args.warmup, 3)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        plan.beamform(channel, out=out)
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    step_ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ev0.record(stream)
-    for i in range(args.steps):
-        plan.beamform(channel, out=out)
-        step_ev[i].record(stream)
-    ev1.record(stream)
-    barrier()
-    clocks = sampler.result()
-    ms_total = ev0.elapsed_time(ev1)
-    marks = [ev0] + step_ev
-    per_step = sorted(marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps))
-    demod_ms, das_ms = plan.timing(min(args.steps, 64))
-    info = plan.info()
-    launches = info["launches_last_call"] * args.steps
+    def all_max(x):
+        v = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        return float(v[0])
+
+    plan = Plan(**rounded_kwargs(cfg), max_frames=n_frames, precision=args.precision)
+    out = torch.empty((n_frames, plan.out_complex_per_frame), dtype=torch.complex64, device=device)
+    arm = time_arm(torch, plan, channel, out, args.steps, warmup, barrier, local_rank, sample_clocks=True)
+    info = arm["info"]
+    got_default = out[:len(distinct)].cpu().numpy()
 
     # end to end through the C-ABI host entry: pinned host buffers, H2D + kernels + D2H inside the timed region
     h_in = torch.empty(channel.shape, dtype=torch.int16, pin_memory=True)
@@ -180,75 +244,82 @@ def run_ours(args):
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         plan.beamform_host(h_in.numpy(), out=h_out.numpy())
-    e2e_s = time.perf_counter() - t0
-    e2e_ms = torch.tensor([e2e_s * 1e3 / e2e_steps, ms_total / args.steps], dtype=torch.float64, device=device)
+    e2e_ms_step = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    ms_step = arm["ms_step"]
     if world > 1:
-        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
-    e2e_ms_step, ms_step = float(e2e_ms[0]), float(e2e_ms[1])
+        e2e_ms_step, ms_step = all_max(e2e_ms_step), all_max(ms_step)
+    plan.close()
+    del h_in, h_out
+
+    # the other scratch formats on the same workload (rank 0 of a single-GPU run only): the driver-run record shows
+    # the precision / speed trade next to the default arm
+    arms = {}
+    if rank == 0 and world == 1 and not args.no_arms and not args.per_angle:
+        for prec in (1, 2, 3):
+            if prec == info["precision"]:
+                continue
+            with Plan(**rounded_kwargs(cfg), max_frames=n_frames, precision=prec) as p2:
+                a = time_arm(torch, p2, channel, out, max(3, min(args.steps, 6)), 3, barrier, local_rank)
+                a["got"] = out[:len(distinct)].cpu().numpy()
+                arms[prec] = a
 
     fp32_probe = fp32_peak_tflops() if rank == 0 else None
-    cpu = None
+    cpu, parity = None, {}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        fps1, dt1, cores = oracle_frames_per_s(cfg, host_frames, 1)
-        n_more = int(np.clip(round(12.0 / max(dt1, 1e-3)), 1, 24))
-        fps, dt, cores = oracle_frames_per_s(cfg, host_frames, n_more)
+        fps1, dt1, cores, _ = oracle_frames_per_s(cfg, host_frames, 1)
+        n_more = int(np.clip(round(12.0 / max(dt1, 1e-3)), len(distinct), 24))
+        fps, dt, cores, refs = oracle_frames_per_s(cfg, host_frames, n_more)
         cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle",
                "sample": "%d frames of the %s workload (demodulation + both projections), %.1f s" % (n_more, cfg.name, dt)}
-    plan.close()
+
+        def worst(got):
+            return max(float(np.abs(got[d] - refs[d]).max() / np.abs(refs[d]).max()) for d in refs)
+
+        parity[info["precision"]] = worst(got_default)
+        for prec, a in arms.items():
+            parity[prec] = worst(a["got"])
 
     if rank == 0:
-        # Roofline accounting: `gathers` = the pixel x element x angle terms of the definition;
-        # the kernel executes fewer when transmit events fold (mirror angles about a centred reference slice are
-        # added in the pre-pass and beamformed once).  The roofline fraction is taken on the EXECUTED terms -- the
-        # conservative count; the unfolded (definition) count is reported beside it.
-        n_events = len(cfg.row_tx_angles) + len(cfg.col_tx_angles)
-        fold = info["events_executed"] / float(n_events)
-        gathers_exec = gathers * fold
-        achieved = FLOP_PER_GATHER * gathers_exec / (das_ms * 1e-3) / 1e12
-        achieved_def = FLOP_PER_GATHER * gathers / (das_ms * 1e-3) / 1e12
+        roof = das_roofline(cfg, args, arm, gathers, fp32_probe, world_ms=ms_step)
+        roof["parity_max_rel_err_vs_oracle"] = parity.get(info["precision"])
         line = {
             "metric": "projection-beamformed frames/s (300-frame ensemble)" + (", one slice per transmit event (compound = 0)" if args.per_angle else ""),
-            "value": whole_job(n_frames, world, ms_step)[0],
-            "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "value": world * n_frames / (ms_step * 1e-3),
+            "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic: frames %s of the seeded moving scene rendered by synth/ (CPU echo "
+            "dtype": DTYPE_OF_PRECISION[info["precision"]],
+            "data": "synthetic: frames %s of the seeded moving scene rendered by synth/ (CPU echo "
             "simulator), tiled over the ensemble" % (list(distinct),),
             "config": {"workload": "BASELINE.json configs[%d] (%s): 128+128 RCA, 11+11 angles, %d frames, %dx%d px "
                        "per projection, %d samples @ %.0f MHz" % (args.config, cfg.name, n_frames, cfg.grid_xz[0],
                                                                    cfg.grid_xz[3], cfg.n_samples, cfg.fs / 1e6),
                        "frames": n_frames, "channel_bytes": int(channel.numel() * 2),
                        "l2_policy": "inputs (%.1f GB) larger than L2, no flush" % (channel.numel() * 2 / 1e9),
-                       "parallelism": "independent ensembles per GPU, no collective", "plan": info},
+                       "parallelism": "independent ensembles per GPU, no collective",
+                       "precision_requested": args.precision, "plan": info},
             "gather_samples_per_s": world * gathers / (ms_step * 1e-3),
-            "ms_per_step_min": per_step[0], "ms_per_step_median": per_step[len(per_step) // 2],
+            "ms_per_step_min": arm["per_step"][0], "ms_per_step_median": arm["per_step"][len(arm["per_step"]) // 2],
             "ensemble_ms": ms_step, "acquisition_ms": 1e3 * n_frames / cfg.frame_rate_hz,
-            "kernels_ms": {"demod_stage": demod_ms, "das": das_ms},
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": TRAFFIC_BYTES.get(args.config),
-                         "kernel": "das_ring_kernel<12,4,%s,0>" % ("1" if info["precision"] == 2 else "0") if info["kernel"] == 2 else "das_generic_kernel",
-                         "flop_per_gather_sample": FLOP_PER_GATHER, "gather_samples_per_launch": gathers_exec,
-                         "gather_samples_of_the_definition": gathers, "events_executed_per_frame": info["events_executed"],
-                         "events_per_frame": n_events, "frac_on_definition_count": achieved_def / NOMINAL_FP32_TFLOPS,
-                         "peak_source": "derived: 148 SM x 128 lanes x 2 x 1965 MHz (DESIGN.md); FFMA probe measured "
-                                        "%.1f TFLOP/s on this box" % fp32_probe,
-                         "whole_step_frac": FLOP_PER_GATHER * gathers_exec / (ms_step * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS},
-            "roofline_prepass": prepass_roofline(cfg, info, n_frames, demod_ms),
-            "cpu_baseline": cpu, "clocks": clocks,
+            "kernels_ms": {"demod_stage": arm["demod_ms"], "das": arm["das_ms"]},
+            "roofline": roof,
+            "roofline_prepass": prepass_roofline(cfg, info, n_frames, arm["demod_ms"]),
+            "cpu_baseline": cpu, "clocks": arm["clocks"],
             "e2e": {"value": world * n_frames / (e2e_ms_step * 1e-3), "unit": "frames/s",
                     "h2d_bytes_per_step": int(info["host_upload_bytes_per_frame"]) * n_frames,
                     "host_buffer_bytes": int(channel.numel() * 2), "d2h_bytes_per_step": int(out.numel() * 8),
                     "ms_per_step": e2e_ms_step, "steps": e2e_steps},
-            "gpu_launches": int(launches),
+            "gpu_launches": int(arm["launches"]),
         }
+        names = {1: "roofline_compact_fast", 2: "roofline_full", 3: "roofline_compact"}
+        for prec, a in arms.items():
+            r = das_roofline(cfg, args, a, gathers, fp32_probe)
+            r["parity_max_rel_err_vs_oracle"] = parity.get(prec)
+            r["frames_per_s"] = n_frames / (a["ms_step"] * 1e-3)
+            r["steps"] = len(a["per_step"])
+            line[names[prec]] = r
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the ncu --set full
-# capture summarised under profiles/ (None until captured for that config)
-TRAFFIC_BYTES = {2: 3.677742e9 + 0.195292e9,      # profiles/r01_v7_ncu.md (das_ring_kernel<12,4,0,0>, one launch)
-                 3: 7.129134e9 + 0.556273e9}      # profiles/r01_v7_cfg3.md
 
 
 def run_volume(args):
@@ -289,7 +360,8 @@ def run_volume(args):
     print(json.dumps({
         "metric": "full-3D DAS volumes/s (config 4, conventional comparator)", "value": 1e3 / ms, "unit": "volumes/s",
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic: config 1 frame rendered by synth/",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 (fp32 rows unpacked from the staged IQ entries, fp32 weight)",
+        "data": "synthetic: config 1 frame rendered by synth/",
         "config": {"workload": "BASELINE.json configs[4]: 180x180x164 voxels, 11+11 angles, 128+128 RCA, 1 frame"},
         "gather_samples_per_s": gathers / (ms * 1e-3),
         "projection_path_ms_same_frame": ms_proj, "volume_over_projection_time": ms / ms_proj,
@@ -334,6 +406,52 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def launch_ranks(args):
+    """`--gpus N` without a launcher (WORLD_SIZE unset): start the N ranks through torch.distributed.run -- the
+    command the driver uses -- and pass their output and exit code through.  Fails (exit 2) when fewer than N GPUs are
+    visible instead of silently running one."""
+    import subprocess
+    if not args.selftest_launch:
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.stderr.write("bench.py: --gpus %d but only %d CUDA device(s) are visible\n" % (args.gpus, have))
+            return 2
+    port = 29500 + (os.getpid() * 7) % 2000
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")        # the rank / topology lines show that N ranks really formed
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd, env=env).returncode
+
+
+def run_selftest_launch(args):
+    """CPU stand-in for the multi-rank run (tests/test_multirank_cpu.py): the same launch path and rank bookkeeping
+    as run_ours -- process group (gloo), barrier, max over ranks, rank 0 prints ONE line -- with a sleep for the
+    kernels.  Hidden flag; never a bench value."""
+    import torch
+    import torch.distributed as dist
+    rank, _, world = dist_env()
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    ms_local = 10.0 * (rank + 1)
+    time.sleep(ms_local * 1e-3)
+
+    def all_max(x):
+        v = torch.tensor([x], dtype=torch.float64)
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        return float(v[0])
+
+    fps, ms = whole_job(300, world, ms_local, all_max)
+    if world > 1:
+        dist.barrier()
+    if rank == 0:
+        print(json.dumps({"selftest": True, "n_gpus": world, "value": fps, "ms_per_step": ms, "unit": "frames/s"}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -341,20 +459,28 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
+    ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
+    ap.add_argument("--no-arms", action="store_true", help="skip the other scratch formats (roofline_full, ...)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-frames", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-angle", action="store_true",
                     help="compound = 0: one slice per transmit event (the paper's S_k) instead of the compounded "
                          "projections -- a secondary figure, not the BASELINE metric")
+    ap.add_argument("--selftest-launch", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
-    if args.steps < 1:
-        ap.error("--steps must be >= 1")
+    if args.steps < 1 or args.gpus < 1:
+        ap.error("--steps and --gpus must be >= 1")
     _, _, world = dist_env()
-    if world != max(1, args.gpus):
-        if world == 1 and args.gpus > 1:
-            sys.stderr.write("bench.py: --gpus %d needs torchrun with --nproc-per-node %d; running 1 GPU\n" % (args.gpus, args.gpus))
-    if args.impl == "reference":
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1 and not (args.impl == "reference"):
+        sys.exit(launch_ranks(args))
+    if world != args.gpus and args.impl != "reference":
+        sys.stderr.write("bench.py: --gpus %d but the launcher started %d rank(s)\n" % (args.gpus, world))
+        sys.exit(2)
+    if args.selftest_launch:
+        run_selftest_launch(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.config == 4:
         run_volume(args)

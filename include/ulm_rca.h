@@ -86,13 +86,23 @@ typedef struct {
     int32_t kernel;             /* 0 = auto (ring kernel where the shape fits); 1 = generic gather kernel;
                                    2 = shared-memory ring kernel or ULM_RCA_EUNSUPPORTED                 */
     int32_t precision;          /* format of the staged IQ scratch entries (mid = (a+b)/2, d = b-a of two
-                                   neighbouring samples): 1 = compact, 10 bytes per (sample, frame): mid with
-                                   17 significant bits, d and the interpolation weight in fp16 (error
-                                   <= ~2^-12 |d| per term: within 1e-4 of the image maximum on echo data,
-                                   meant for band-limited input), 2 = full (fp32 throughout, 16 bytes),
-                                   0 = auto: compact for RF input (the library's own low-pass band-limits
-                                   it), full for IQ input (spectrum unknown)                            */
-    int32_t reserved[4];        /* must be 0                                                           */
+                                   neighbouring samples) and of the interpolation v = mid + a' d, a' in [-1/2, 1/2]:
+                                   2 = full: fp32 throughout, 16 bytes per (sample, frame); nothing but fp32 rounding.
+                                   3 = compact, 10 bytes: mid with 17 significant bits, d in fp16 (relative 2^-11,
+                                       i.e. <= 2^-12 |d| per term), the weight a' carried as TWO fp16 terms
+                                       (22 bits): holds max|err| <= 1e-4 max|image| on any int16 RF input, white
+                                       noise included (the library's low-pass bounds |d| / |iq|).
+                                   1 = compact-fast (opt-in): as 3 but a' rounded to ONE fp16 (another 2^-12 |d| per
+                                       term, ~10 % faster DAS): within 1e-4 on band-limited echo data (|d| ~ 0.3 |iq|;
+                                       1.1e-5 .. 1.4e-5 measured on the five BASELINE configs) but up to ~1.5e-4 on
+                                       white noise -- select it only for echo-like input.
+                                   0 = auto = 3 for RF input, 2 for IQ input (spectrum unknown).
+                                   With the compact formats the low mantissa byte of a stored mid value is a byte of
+                                   another frame of the same 4-frame chunk, so the result of frame f depends, by
+                                   < 2^-16 relative per term (zero-mean), on which frames share its chunk.       */
+    int32_t no_timing;          /* 1 = ulm_rca_beamform records no CUDA events around its kernels (and
+                                   ulm_rca_plan_timing is unavailable); 0 = three cudaEventRecord per batch   */
+    int32_t reserved[3];        /* must be 0                                                           */
 } ulm_rca_options;
 
 /*
@@ -142,11 +152,12 @@ ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_c
 
 /* Host convenience (this is the end-to-end call bench.py times as "e2e"): copies n_frames of HOST
  * channel data to an internal device buffer, beamforms, copies the images back to HOST memory and
- * synchronises.  The work is cut into up to 8 chunks of whole 12-frame groups and pipelined on two internal
- * streams (upload of chunk i+1 overlaps the kernels and the download of chunk i); only what the method reads is
- * uploaded (the receive aperture of every event, the touched sample range); pass pinned host memory
- * for the overlap to take place.  Allocates device staging and the streams on first use (freed by
- * plan_destroy).  One call in flight per plan. */
+ * synchronises.  The work is cut into chunks of 24 frames (12 for calls of fewer than 48 frames) and pipelined on two
+ * internal streams through two device staging slots of one chunk each (upload of chunk i+1 overlaps the kernels and
+ * the download of chunk i); only what the method reads is uploaded (the receive aperture of every event, the
+ * touched sample range); pass pinned host memory for the overlap to take place.  Allocates the staging slots and
+ * the streams on first use (freed by plan_destroy).  On any failure both streams are drained before the call
+ * returns, so the caller's buffers are no longer in use.  One call in flight per plan. */
 ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, int32_t n_frames,
                                      void *h_out);
 

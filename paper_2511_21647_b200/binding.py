@@ -45,7 +45,7 @@ class Options(C.Structure):
                 ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
                 ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
                 ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
-                ("precision", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("precision", C.c_int32), ("no_timing", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 def library_path() -> str:
@@ -122,7 +122,8 @@ class Plan:
                  n_samples: int, input_kind: int = 0, channels_per_event: Optional[int] = None,
                  t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
                  elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
-                 max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0):
+                 max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0,
+                 no_timing: bool = False):
         lib = load()
         self._h = C.c_void_p()
         geo = Geometry(n_rows, n_cols, pitch)
@@ -136,7 +137,7 @@ class Plan:
             raise ValueError("elem_window must have n_cols + n_rows entries")
         opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
                       float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
-                      1 if build_volume else 0, int(kernel), int(precision))
+                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0)
         gx, gy = Grid(*grid_xz), Grid(*grid_yz)
         _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
                                        float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),
@@ -148,6 +149,8 @@ class Plan:
         self.volume_shape = (grid_xz[0], grid_yz[0], grid_xz[3])
         self.grid_xz, self.grid_yz = tuple(grid_xz), tuple(grid_yz)
         self.n_row_tx, self.n_col_tx = len(row_tx_angles), len(col_tx_angles)
+        import torch
+        self.device_index = torch.cuda.current_device()      # the plan belongs to the device current at creation
 
     # -- lifetime -------------------------------------------------------------------------------------
     def close(self):
@@ -189,21 +192,33 @@ class Plan:
         s = stream if stream is not None else torch.cuda.current_stream()
         return C.c_void_p(s.cuda_stream)
 
-    def beamform(self, channel, out=None, stream=None):
-        """channel: torch int16 CUDA tensor [frame][event][channel][sample] (+[2] for IQ input).
-        Returns a torch complex64 CUDA tensor [frame][out_complex_per_frame]; asynchronous on `stream`."""
+    def _check_channel(self, channel) -> int:
         import torch
         if not (channel.is_cuda and channel.dtype == torch.int16 and channel.is_contiguous()):
             raise ValueError("channel must be a contiguous int16 CUDA tensor")
+        if channel.device.index != self.device_index:
+            raise ValueError("channel lives on cuda:%d, the plan on cuda:%d" % (channel.device.index, self.device_index))
         n_frames = int(channel.shape[0])
         if n_frames and channel.numel() * 2 != n_frames * self.channel_bytes_per_frame:
             raise ValueError("channel has %d bytes per frame, plan expects %d" %
                              (channel.numel() * 2 // n_frames, self.channel_bytes_per_frame))
+        return n_frames
+
+    def _check_out(self, out, numel: int):
+        import torch
+        if not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and out.numel() == numel
+                and out.device.index == self.device_index):
+            raise ValueError("out must be a contiguous complex64 CUDA tensor of the plan's size on the plan's device")
+
+    def beamform(self, channel, out=None, stream=None):
+        """channel: torch int16 CUDA tensor [frame][event][channel][sample] (+[2] for IQ input).
+        Returns a torch complex64 CUDA tensor [frame][out_complex_per_frame]; asynchronous on `stream`."""
+        import torch
+        n_frames = self._check_channel(channel)
         if out is None:
             out = torch.empty((n_frames, self.out_complex_per_frame), dtype=torch.complex64, device=channel.device)
-        elif not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous()
-                  and out.numel() == n_frames * self.out_complex_per_frame):
-            raise ValueError("out must be a contiguous complex64 CUDA tensor of the plan's size")
+        else:
+            self._check_out(out, n_frames * self.out_complex_per_frame)
         _check(load().ulm_rca_beamform(self._h, C.c_void_p(channel.data_ptr()), n_frames,
                                        C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
         return out
@@ -211,11 +226,11 @@ class Plan:
     def beamform_volume(self, channel, out=None, stream=None):
         """Full 3-D DAS comparator: returns complex64 [frame][x][y][z]."""
         import torch
-        if not (channel.is_cuda and channel.dtype == torch.int16 and channel.is_contiguous()):
-            raise ValueError("channel must be a contiguous int16 CUDA tensor")
-        n_frames = int(channel.shape[0])
+        n_frames = self._check_channel(channel)
         if out is None:
             out = torch.empty((n_frames,) + self.volume_shape, dtype=torch.complex64, device=channel.device)
+        else:
+            self._check_out(out, n_frames * self.volume_bytes_per_frame // 8)
         _check(load().ulm_rca_beamform_volume(self._h, C.c_void_p(channel.data_ptr()), n_frames,
                                               C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
         return out

@@ -108,6 +108,7 @@ struct ulm_rca_plan {
     ulm::DemodConst demod{};
     int kernel = 1;               // 1 generic, 2 ring
     bool d32 = false;             // full (fp32) difference term in the scratch
+    bool w2 = false;              // compact entries, interpolation weight carried as two fp16 terms (precision = 3)
     bool quad = false;            // fs = 4 fc exactly, default 17 taps, analytic signal from two real filters
     bool half_band = false;       // every even demodulation tap except the centre is exactly zero (fs = 4 fc)
     bool quarter_band = false;    // every fourth demodulation tap except the centre is exactly zero (fs = 8 fc)
@@ -116,11 +117,13 @@ struct ulm_rca_plan {
     long long out_per_frame = 0, vol_per_frame = 0;
     mutable long long last_launches = 0;
     // host-convenience staging
+    // (two slots of h_stage_frames frames each: the upload of chunk i + 1 overlaps the kernels / download of chunk i)
     DeviceBuf h_stage_in, h_stage_out;
     size_t h_stage_frames = 0;
     cudaStream_t h_copy = nullptr, h_compute = nullptr;     // created on the first host call
-    static constexpr int kHostChunks = 8;
-    cudaEvent_t h_in_done[kHostChunks] = {};
+    static constexpr int kHostSlots = 2;
+    cudaEvent_t h_in_done[kHostSlots] = {}, h_slot_free[kHostSlots] = {};
+    bool timing = true;           // record CUDA events around the kernels (options.no_timing = 0)
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -130,6 +133,7 @@ struct ulm_rca_plan {
     ~ulm_rca_plan() {
         for (auto &c : ev) for (auto &b : c) for (auto &e : b) if (e) cudaEventDestroy(e);
         for (auto &e : h_in_done) if (e) cudaEventDestroy(e);
+        for (auto &e : h_slot_free) if (e) cudaEventDestroy(e);
         if (h_copy) cudaStreamDestroy(h_copy);
         if (h_compute) cudaStreamDestroy(h_compute);
     }
@@ -338,6 +342,9 @@ void launch_generic_f(const ulm_rca_plan &P, const ulm::DasParams &D, int n_fram
     if (P.d32) {
         if (P.apod) ulm::das_generic_kernel<F, true, true><<<grid, 128, 0, st>>>(D);
         else ulm::das_generic_kernel<F, true, false><<<grid, 128, 0, st>>>(D);
+    } else if (P.w2) {
+        if (P.apod) ulm::das_generic_kernel<F, false, true, true><<<grid, 128, 0, st>>>(D);
+        else ulm::das_generic_kernel<F, false, false, true><<<grid, 128, 0, st>>>(D);
     } else {
         if (P.apod) ulm::das_generic_kernel<F, false, true><<<grid, 128, 0, st>>>(D);
         else ulm::das_generic_kernel<F, false, false><<<grid, 128, 0, st>>>(D);
@@ -482,8 +489,9 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
     if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
-    for (int i = 0; i < 4; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
-    if (opt->precision < 0 || opt->precision > 2) return fail(ULM_RCA_EINVAL, "precision must be 0, 1 or 2");
+    for (int i = 0; i < 3; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->no_timing != 0 && opt->no_timing != 1) return fail(ULM_RCA_EINVAL, "no_timing must be 0 or 1");
+    if (opt->precision < 0 || opt->precision > 3) return fail(ULM_RCA_EINVAL, "precision must be 0, 1, 2 or 3");
     if (opt->input_kind != 0 && opt->input_kind != 1) return fail(ULM_RCA_EINVAL, "input_kind must be 0 or 1");
     if (opt->n_samples < 2) return fail(ULM_RCA_EINVAL, "n_samples must be >= 2");
     if (!std::isfinite(opt->t_start_s) || !std::isfinite(opt->f_number) || opt->f_number < 0)
@@ -521,10 +529,14 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if ((long long)((P.max_frames + 3) / 4) * (n_row_tx + n_col_tx) > 65535)
         return fail(ULM_RCA_EUNSUPPORTED, "max_frames x events too large for one batch: lower max_frames");
     P.build_volume = opt->build_volume;
+    P.timing = opt->no_timing == 0;
     P.n_events = n_row_tx + n_col_tx;
     P.n_rx_max = std::max(P.n_rows, P.n_cols);
     P.apod = opt->f_number > 0 || opt->elem_window != nullptr;
+    // auto: RF input (band-limited by the library's own low-pass) -> compact entries with the exact weight;
+    // IQ input (spectrum unknown) -> full entries
     P.d32 = opt->precision == 2 || (opt->precision == 0 && opt->input_kind == 1);
+    P.w2 = !P.d32 && opt->precision != 1;
 
     for (int a = 0; a < 2; ++a) {
         Aperture &A = P.ap[a];
@@ -618,7 +630,10 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         }
     }
 
-    P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * P.n_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
+    // one scratch row block per event the plan will fill: the folded events of the projection path, or every real
+    // event when the volume comparator (which never folds) is prepared as well
+    const int scratch_events = P.build_volume ? P.n_events : P.nv_events;
+    P.iq_bytes = (size_t)((P.max_frames + 11) / 12) * scratch_events * P.n_rx_max * P.l_row * ulm::entry_bytes(12, P.d32);
     CUDA_TRY(cudaMalloc(&P.iq.p, P.iq_bytes));
     if (P.build_volume) CUDA_TRY(cudaMalloc(&P.vol_rows.p, (size_t)P.n_events * P.n_rx_max * P.l_row * sizeof(float4)));
 
@@ -635,11 +650,13 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         const char *why = nullptr;
         const bool ok = ulm::ring_plan(desc, P.pitch, P.c, P.fs, P.t_start, P.l_row, P.ring, P.ap[0].ring,
                                        P.ap[1].ring, &why);
-        if (ok) P.kernel = 2;
-        else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
+        if (ok) {
+            P.kernel = 2;
+            CUDA_TRY(ulm::ring_set_attributes());       // per-device function attribute, set on the plan's device
+        } else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
         if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
     }
-    for (auto &c : P.ev) for (auto &b : c) for (auto &e : b) CUDA_TRY(cudaEventCreate(&e));
+    if (P.timing) for (auto &c : P.ev) for (auto &b : c) for (auto &e : b) CUDA_TRY(cudaEventCreate(&e));
     CUDA_TRY(cudaDeviceSynchronize());
     guard.p = nullptr;
     *out = Pp;
@@ -661,7 +678,7 @@ ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n
                               ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
                               ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
                               ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
-                              ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : 1, ulm::entry_bytes(12, d32) / 12,
+                              ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : (plan->w2 ? 3 : 1), ulm::entry_bytes(12, d32) / 12,
                               (int64_t)host_upload_bytes_per_frame(*plan), plan->nv_events};
     for (int i = 0; i < n && i < 16; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
@@ -686,10 +703,10 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
         const int nb = std::min(P.max_frames, n_frames - f0);
         const int16_t *in = reinterpret_cast<const int16_t *>(static_cast<const char *>(d_channel) + (size_t)f0 * ch_bytes);
         float2 *outp = static_cast<float2 *>(d_out) + (long long)f0 * P.out_per_frame;
-        const int tb = P.timed_batches[slot] < ulm_rca_plan::kTimedBatches ? P.timed_batches[slot] : -1;
-        if (tb >= 0) cudaEventRecord(P.ev[slot][tb][0], st);
+        const int tb = (P.timing && P.timed_batches[slot] < ulm_rca_plan::kTimedBatches) ? P.timed_batches[slot] : -1;
+        if (tb >= 0) CUDA_TRY(cudaEventRecord(P.ev[slot][tb][0], st));
         CUDA_TRY(launch_demod(P, in, nb, true, st));
-        if (tb >= 0) cudaEventRecord(P.ev[slot][tb][1], st);
+        if (tb >= 0) CUDA_TRY(cudaEventRecord(P.ev[slot][tb][1], st));
         for (int a = 0; a < 2; ++a) {     // an aperture without transmit events: its image is all zeros
             const Aperture &A = P.ap[a];
             if (A.n_tx == 0 && P.compound)
@@ -710,7 +727,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
                 R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
                 R.out_base = A.out_base;
             }
-            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, group_frames(nb), P.d32, P.apod, st);
+            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, group_frames(nb), P.d32, P.w2, P.apod, st);
         } else {
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];
@@ -721,7 +738,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
                 launch_generic(P, D, nb, st);
             }
         }
-        if (tb >= 0) { cudaEventRecord(P.ev[slot][tb][2], st); P.timed_batches[slot] = tb + 1; }
+        if (tb >= 0) { CUDA_TRY(cudaEventRecord(P.ev[slot][tb][2], st)); P.timed_batches[slot] = tb + 1; }
     }
     CUDA_TRY(cudaGetLastError());
     return ULM_RCA_OK;
@@ -729,6 +746,7 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
 
 ulm_rca_status ulm_rca_plan_timing(const ulm_rca_plan *plan, int32_t n_calls, double *demod_ms, double *das_ms) {
     if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->timing) return fail(ULM_RCA_EUNSUPPORTED, "plan was created with no_timing = 1");
     if (n_calls < 1 || n_calls > ulm_rca_plan::kTimedCalls || n_calls > plan->n_calls)
         return fail(ULM_RCA_EINVAL, "n_calls must be 1..min(64, calls made)");
     double d = 0, g = 0;
@@ -799,57 +817,74 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
     if (ulm_rca_status s = check_device(*plan)) return s;
     size_t ch_bytes = 0, out_bytes = 0;
     ulm_rca_plan_sizes(plan, &ch_bytes, &out_bytes, nullptr);
-    if (plan->h_stage_frames < (size_t)n_frames) {
+    // pipeline over chunks of whole 12-frame groups through two staging slots: the upload of chunk i + 1 overlaps the
+    // kernels and the download of chunk i (the host buffers should be pinned for the copies to be asynchronous)
+    constexpr int kSlots = ulm_rca_plan::kHostSlots;
+    const int chunk = n_frames >= 48 ? 24 : 12;
+    if (plan->h_stage_frames < (size_t)chunk) {
         if (plan->h_stage_in.p) { cudaFree(plan->h_stage_in.p); plan->h_stage_in.p = nullptr; }
         if (plan->h_stage_out.p) { cudaFree(plan->h_stage_out.p); plan->h_stage_out.p = nullptr; }
         plan->h_stage_frames = 0;
-        CUDA_TRY(cudaMalloc(&plan->h_stage_in.p, ch_bytes * n_frames));
-        CUDA_TRY(cudaMalloc(&plan->h_stage_out.p, out_bytes * n_frames));
-        plan->h_stage_frames = n_frames;
+        CUDA_TRY(cudaMalloc(&plan->h_stage_in.p, ch_bytes * chunk * kSlots));
+        CUDA_TRY(cudaMalloc(&plan->h_stage_out.p, out_bytes * chunk * kSlots));
+        plan->h_stage_frames = chunk;
     }
     if (!plan->h_copy) {
         CUDA_TRY(cudaStreamCreateWithFlags(&plan->h_copy, cudaStreamNonBlocking));
         CUDA_TRY(cudaStreamCreateWithFlags(&plan->h_compute, cudaStreamNonBlocking));
         for (auto &e : plan->h_in_done) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        for (auto &e : plan->h_slot_free) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    // pipeline over chunks of frames (whole frame groups of 12): the upload of chunk i + 1 overlaps the kernels
-    // and the download of chunk i (the host buffers should be pinned for the copies to be asynchronous)
-    int chunk = (n_frames + ulm_rca_plan::kHostChunks - 1) / ulm_rca_plan::kHostChunks;
-    chunk = std::max(12, (chunk + 11) / 12 * 12);
     const char *h_in = static_cast<const char *>(h_channel);
     char *h_o = static_cast<char *>(h_out);
-    char *d_in = plan->h_stage_in.as<char>(), *d_o = plan->h_stage_out.as<char>();
     const int eb = plan->input_kind == 1 ? 4 : 2;
     int s_lo = 0, s_hi = 0;
     host_sample_range(*plan, s_lo, s_hi);
+    // a failure inside the loop must not return while copies still read / write the caller's buffers
+    auto drain = [&](ulm_rca_status s) {
+        cudaStreamSynchronize(plan->h_copy);
+        cudaStreamSynchronize(plan->h_compute);
+        return s;
+    };
+#define HOST_TRY(expr)                                                                                     \
+    do {                                                                                                   \
+        cudaError_t e_ = (expr);                                                                           \
+        if (e_ != cudaSuccess)                                                                             \
+            return drain(fail(e_ == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "%s: %s", #expr, \
+                              cudaGetErrorString(e_)));                                                    \
+    } while (0)
     int i = 0;
     for (int f0 = 0; f0 < n_frames; f0 += chunk, ++i) {
         const int nb = std::min(chunk, n_frames - f0);
+        const int slot = i % kSlots;
+        char *d_in = plan->h_stage_in.as<char>() + (size_t)slot * chunk * ch_bytes;
+        char *d_o = plan->h_stage_out.as<char>() + (size_t)slot * chunk * out_bytes;
+        // the slot is free once the kernels and the download of the chunk that used it last have finished
+        if (i >= kSlots) HOST_TRY(cudaStreamWaitEvent(plan->h_copy, plan->h_slot_free[slot], 0));
         // upload only what the pre-pass reads: the receive aperture of every event, touched sample range
-        for (int f = f0; f < f0 + nb; ++f)
+        for (int f = 0; f < nb; ++f)
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = plan->ap[a];
                 if (A.n_tx == 0) continue;
                 cudaMemcpy3DParms cp = {};
                 const size_t row_pitch = (size_t)plan->n_samples * eb;
-                cp.srcPtr = make_cudaPitchedPtr(const_cast<char *>(h_in) + (size_t)f * ch_bytes, row_pitch, row_pitch, plan->cpe);
+                cp.srcPtr = make_cudaPitchedPtr(const_cast<char *>(h_in) + (size_t)(f0 + f) * ch_bytes, row_pitch, row_pitch, plan->cpe);
                 cp.dstPtr = make_cudaPitchedPtr(d_in + (size_t)f * ch_bytes, row_pitch, row_pitch, plan->cpe);
                 const size_t c0 = (a == 0 && plan->cpe == plan->n_rows + plan->n_cols) ? plan->n_rows : 0;
                 cp.srcPos = make_cudaPos((size_t)s_lo * eb, c0, A.e0);
                 cp.dstPos = cp.srcPos;
                 cp.extent = make_cudaExtent((size_t)(s_hi - s_lo) * eb, A.n_rx, A.n_tx);
                 cp.kind = cudaMemcpyHostToDevice;
-                CUDA_TRY(cudaMemcpy3DAsync(&cp, plan->h_copy));
+                HOST_TRY(cudaMemcpy3DAsync(&cp, plan->h_copy));
             }
-        CUDA_TRY(cudaEventRecord(plan->h_in_done[i], plan->h_copy));
-        CUDA_TRY(cudaStreamWaitEvent(plan->h_compute, plan->h_in_done[i], 0));
-        if (ulm_rca_status s = ulm_rca_beamform(plan, d_in + (size_t)f0 * ch_bytes, nb, d_o + (size_t)f0 * out_bytes,
-                                                plan->h_compute))
-            return s;
-        CUDA_TRY(cudaMemcpyAsync(h_o + (size_t)f0 * out_bytes, d_o + (size_t)f0 * out_bytes, out_bytes * nb,
-                                 cudaMemcpyDeviceToHost, plan->h_compute));
+        HOST_TRY(cudaEventRecord(plan->h_in_done[slot], plan->h_copy));
+        HOST_TRY(cudaStreamWaitEvent(plan->h_compute, plan->h_in_done[slot], 0));
+        if (ulm_rca_status s = ulm_rca_beamform(plan, d_in, nb, d_o, plan->h_compute)) return drain(s);
+        HOST_TRY(cudaMemcpyAsync(h_o + (size_t)f0 * out_bytes, d_o, out_bytes * nb, cudaMemcpyDeviceToHost, plan->h_compute));
+        HOST_TRY(cudaEventRecord(plan->h_slot_free[slot], plan->h_compute));
     }
-    CUDA_TRY(cudaStreamSynchronize(plan->h_compute));
+    HOST_TRY(cudaStreamSynchronize(plan->h_compute));
+#undef HOST_TRY
     return ULM_RCA_OK;
 }
 

@@ -537,14 +537,24 @@ struct DasParams {
 // compact entries, whose difference term is stored / 16 in fp16 -- there the whole interpolation
 // v = mid + (16 a') (d / 16) is ONE mixed-precision FMA per component (FHFMA: fp16 x fp16 product exact, fp32 addend,
 // one rounding), so the only errors are the fp16 roundings of the two factors
+// W2 ("exact-weight" compact entries, precision = 3): 16 a' = ah + al2 with al2 = fp16(16 a' - ah), so the weight is
+// carried with 22 significant bits and the interpolation is two FHFMAs per component, v = ah d + (al2 d + mid): the
+// only format error left is the fp16 rounding of the stored difference term.
 struct Alpha {
     float al;
-    unsigned short ah;
+    unsigned short ah, ah2;
 };
+__device__ __forceinline__ float h2f_bits(unsigned short h) {
+    float r;
+    asm("cvt.f32.f16 %0, %1;" : "=f"(r) : "h"(h));
+    return r;
+}
+template <bool W2 = false>
 __device__ __forceinline__ Alpha make_alpha(float al) {
     Alpha a;
     a.al = al;
     a.ah = f2h_bits(kAlScale * al);
+    a.ah2 = W2 ? f2h_bits(fmaf(kAlScale, al, -h2f_bits(a.ah))) : (unsigned short)0;
     return a;
 }
 
@@ -572,6 +582,7 @@ __device__ __forceinline__ uint32_t fp24_gather(uint32_t w0, uint32_t w1, uint32
 // of the four frames (difference term / 16).
 // Scalar version (generic kernel): v = mid + ah * d (one FHFMA per component), acc += (c + j s) v.
 // nv = number of valid frames among the four.
+template <bool W2 = false>
 __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t (&dd)[4], const Alpha &A, float c,
                                           float s, float *accr, float *acci, int nv = 4) {
     const uint32_t re[4] = {w[0], w[1], w[4], w[5]};
@@ -581,8 +592,10 @@ __device__ __forceinline__ void chunk_mac(const uint32_t (&w)[6], const uint32_t
         if (i >= nv) break;
         unsigned short dr, di;
         split_h2(dd[i], dr, di);
-        const float vr = fhfma(A.ah, dr, __uint_as_float(re[i]));
-        const float vi = fhfma(A.ah, di, __uint_as_float(im[i]));
+        float mr = __uint_as_float(re[i]), mi = __uint_as_float(im[i]);
+        if (W2) { mr = fhfma(A.ah2, dr, mr); mi = fhfma(A.ah2, di, mi); }
+        const float vr = fhfma(A.ah, dr, mr);
+        const float vi = fhfma(A.ah, di, mi);
         accr[i] = fmaf(c, vr, accr[i]); accr[i] = fmaf(-s, vi, accr[i]);
         acci[i] = fmaf(s, vr, acci[i]); acci[i] = fmaf(c, vi, acci[i]);
     }
@@ -597,10 +610,17 @@ __device__ __forceinline__ void split_u2(unsigned long long v, uint32_t &lo, uin
 // one FHFMA per component and frame, the complex multiply-accumulate of a frame pair runs as FFMA2 on
 // (frame 2p, frame 2p+1) register pairs; aR / aI are pairs of real / imaginary accumulators; CC = (c, c), SS = (s, s),
 // NS = (-s, -s).  Each half is an ordinary round-to-nearest fp32 FMA, so the results are bit-identical to chunk_mac.
+template <bool W2 = false>
 __device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long long m23, unsigned long long m45,
                                            unsigned long long da, unsigned long long db, unsigned short ah,
-                                           unsigned long long CC, unsigned long long SS, unsigned long long NS,
-                                           unsigned long long *aR, unsigned long long *aI) {
+                                           unsigned short ah2, unsigned long long CC, unsigned long long SS,
+                                           unsigned long long NS, unsigned long long *aR, unsigned long long *aI) {
+    // interpolation of one component: mid + (ah + ah2) d, the small residual term first
+    auto lerp = [&](unsigned short d, uint32_t mid) {
+        float m = __uint_as_float(mid);
+        if (W2) m = fhfma(ah2, d, m);
+        return fhfma(ah, d, m);
+    };
     uint32_t w0, w1, w2, w3, w4, w5, d0, d1, d2, d3;
     split_u2(m01, w0, w1); split_u2(m23, w2, w3); split_u2(m45, w4, w5);
     split_u2(da, d0, d1); split_u2(db, d2, d3);
@@ -608,17 +628,16 @@ __device__ __forceinline__ void chunk_mac2(unsigned long long m01, unsigned long
     {
         split_h2(d0, r0, i0);
         split_h2(d1, r1, i1);
-        const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w0)), fhfma(ah, r1, __uint_as_float(w1)));
-        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(w2)), fhfma(ah, i1, __uint_as_float(w3)));
+        const unsigned long long VR = pack_f2(lerp(r0, w0), lerp(r1, w1));
+        const unsigned long long VI = pack_f2(lerp(i0, w2), lerp(i1, w3));
         aR[0] = ffma2(CC, VR, aR[0]); aR[0] = ffma2(NS, VI, aR[0]);
         aI[0] = ffma2(SS, VR, aI[0]); aI[0] = ffma2(CC, VI, aI[0]);
     }
     {
         split_h2(d2, r0, i0);
         split_h2(d3, r1, i1);
-        const unsigned long long VR = pack_f2(fhfma(ah, r0, __uint_as_float(w4)), fhfma(ah, r1, __uint_as_float(w5)));
-        const unsigned long long VI = pack_f2(fhfma(ah, i0, __uint_as_float(fp24_gather(w0, w2, w4))),
-                                              fhfma(ah, i1, __uint_as_float(fp24_gather(w1, w3, w5))));
+        const unsigned long long VR = pack_f2(lerp(r0, w4), lerp(r1, w5));
+        const unsigned long long VI = pack_f2(lerp(i0, fp24_gather(w0, w2, w4)), lerp(i1, fp24_gather(w1, w3, w5)));
         aR[1] = ffma2(CC, VR, aR[1]); aR[1] = ffma2(NS, VI, aR[1]);
         aI[1] = ffma2(SS, VR, aI[1]); aI[1] = ffma2(CC, VI, aI[1]);
     }
@@ -639,7 +658,7 @@ __device__ __forceinline__ void pair_mac2_full(const uint4 &m, const uint4 &d, u
 // interpolate-and-accumulate of F frames from one entry in global memory (generic kernel):
 // v = mid + a' d  (a' in fp32; compact: d converted from fp16),  acc += (c + j s) v.
 // Full entries are read as 16-byte units, compact entries (8-byte aligned) as 8-byte units.
-template <int F, bool D32>
+template <int F, bool D32, bool W2 = false>
 __device__ __forceinline__ void entry_mac(const unsigned char *ent, const Alpha &A, float c, float s, float *accr,
                                           float *acci, int nv = F) {
     if (D32) {
@@ -667,7 +686,7 @@ __device__ __forceinline__ void entry_mac(const unsigned char *ent, const Alpha 
             const uint2 da = __ldg(e2 + (6 * F) / 8 + 2 * q), db = __ldg(e2 + (6 * F) / 8 + 2 * q + 1);
             const uint32_t w[6] = {a.x, a.y, b.x, b.y, cc.x, cc.y};
             const uint32_t dd[4] = {da.x, da.y, db.x, db.y};
-            chunk_mac(w, dd, A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
+            chunk_mac<W2>(w, dd, A, c, s, accr + 4 * q, acci + 4 * q, nv - 4 * q);
         }
     }
 }
@@ -677,7 +696,7 @@ __device__ __forceinline__ void entry_mac(const unsigned char *ent, const Alpha 
 // IQ scratch through L1/L2.  Serves per-angle slices (compound = 0), the 3-D comparator (config 4) and any
 // shape the shared-memory ring kernel does not cover.  grid = (pixel blocks, frame groups, plane * angle groups).
 // ---------------------------------------------------------------------------------------------------
-template <int F, bool D32, bool APOD>
+template <int F, bool D32, bool APOD, bool W2 = false>
 __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
     const int npix = P.n_lat * P.n_ax;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -722,7 +741,7 @@ __global__ void __launch_bounds__(128) das_generic_kernel(DasParams P) {
             __sincosf(fmaf(kTwoPi * P.fcfs, al, 0.5f * kTwoPi * P.fcfs), &s, &c);     // E(a), a = al + 0.5 in [0, 1]
             if (APOD) { s *= w; c *= w; }
             const unsigned char *ent = P.iq + ((grow + (size_t)(P.e0 + k) * P.n_rx_max + j) * P.l_row + idx) * entry_bytes(F, D32);
-            entry_mac<F, D32>(ent, make_alpha(al), c, s, accr, acci, nv);
+            entry_mac<F, D32, W2>(ent, make_alpha<W2>(al), c, s, accr, acci, nv);
         }
     }
     const long long o = P.out_base + (long long)il * P.s_lat + (long long)plane * P.s_plane +

@@ -138,7 +138,7 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 // run-time index would copy the whole struct to local memory)
 #define ULM_AP(field) (a ? P.ap[1].field : P.ap[0].field)
 
-template <int F, int PX, bool D32, bool APOD>
+template <int F, int PX, bool D32, bool APOD, bool W2 = false>
 __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_constant__ RingLaunch P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int EB = entry_bytes(F, D32);
@@ -384,7 +384,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     const float al = upm - (tt_ - kMagic);
                     PixCtx x;
                     x.addr = (uint32_t)(__float_as_int(tt_) + (int)ioff + hdr) * EB + cbase;
-                    x.A = make_alpha(al);
+                    x.A = make_alpha<W2>(al);
                     // E(a) = exp(j 2 pi (fc/fs) a), a = al + 0.5 in [0, 1]: the whole phase rotation of this gather
                     __sincosf(fmaf(th, al, 0.5f * th), &x.s, &x.c);
                     if (APOD) { x.c *= wv[m]; x.s *= wv[m]; }
@@ -427,7 +427,7 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                             b[3] = lds64(a1 + 6u * F + 16u * q1); b[4] = lds64(a1 + 6u * F + 16u * q1 + 8u);
                         }
                         const unsigned long long *b = buf[st & 1];
-                        chunk_mac2(b[0], b[1], b[2], b[3], b[4], cur.A.ah, pack_f2(cur.c, cur.c),
+                        chunk_mac2<W2>(b[0], b[1], b[2], b[3], b[4], cur.A.ah, cur.A.ah2, pack_f2(cur.c, cur.c),
                                    pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
                         if (q == NQ - 1) cur = nxt;
                     }

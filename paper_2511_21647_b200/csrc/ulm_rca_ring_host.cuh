@@ -182,7 +182,7 @@ inline bool ring_plan(const RingApertureDesc *desc, double pitch, double c, doub
     return true;
 }
 
-template <int F, bool D32, bool APOD>
+template <int F, bool D32, bool APOD, bool W2>
 inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) {
     L.stage_stride = ring_stage_stride(cfg.window, F, D32);
     L.n_stages = ring_stages(cfg.window, F, D32);
@@ -198,13 +198,8 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     L.n_whole = L.split_s > 1 ? L.n_items - rem : L.n_items;
     L.n_work = L.n_whole + (L.n_items - L.n_whole) * L.split_s;
     L.partial = cfg.d_partial;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(das_ring_kernel<F, kRingPx, D32, APOD>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
-        attr_set = true;
-    }
     const int grid = std::min(L.n_work, cfg.n_sms);
-    das_ring_kernel<F, kRingPx, D32, APOD><<<grid, kRingThreads, ring_smem_bytes(cfg.window, F, D32), st>>>(L);
+    das_ring_kernel<F, kRingPx, D32, APOD, W2><<<grid, kRingThreads, ring_smem_bytes(cfg.window, F, D32), st>>>(L);
     if (L.split_s > 1) {
         ring_combine_kernel<F, kRingPx><<<dim3(L.n_items - L.n_whole, kRingPx), kRingConsumers, 0, st>>>(L);
         return 2;
@@ -212,14 +207,37 @@ inline int ring_launch_t(const RingConfig &cfg, RingLaunch &L, cudaStream_t st) 
     return 1;
 }
 
-template <int F, bool D32>
-inline int ring_launch_a(const RingConfig &cfg, RingLaunch &L, bool apod, cudaStream_t st) {
-    return apod ? ring_launch_t<F, D32, true>(cfg, L, st) : ring_launch_t<F, D32, false>(cfg, L, st);
+// The opt-in to 227 KB of dynamic shared memory is a per-device function attribute: ulm_rca_plan_create calls this on
+// the plan's device for every instantiation a launch can select (no process-wide "already set" flag).
+template <int F, bool D32, bool APOD, bool W2 = false>
+inline cudaError_t ring_set_attr_one() {
+    return cudaFuncSetAttribute(das_ring_kernel<F, kRingPx, D32, APOD, W2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemLimit);
+}
+inline cudaError_t ring_set_attributes() {
+    cudaError_t e;
+    if ((e = ring_set_attr_one<12, false, false>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<12, false, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<12, true, false>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<12, true, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<4, false, false>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<4, false, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<4, true, false>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<4, true, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<12, false, false, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<12, false, true, true>()) != cudaSuccess) return e;
+    if ((e = ring_set_attr_one<4, false, false, true>()) != cudaSuccess) return e;
+    return ring_set_attr_one<4, false, true, true>();
 }
 
-// returns the number of kernels launched; F = frames per group of the scratch (4 or 12), d32 = full entries
+template <int F, bool D32, bool W2>
+inline int ring_launch_a(const RingConfig &cfg, RingLaunch &L, bool apod, cudaStream_t st) {
+    return apod ? ring_launch_t<F, D32, true, W2>(cfg, L, st) : ring_launch_t<F, D32, false, W2>(cfg, L, st);
+}
+
+// returns the number of kernels launched; F = frames per group of the scratch (4 or 12), d32 = full entries,
+// w2 = compact entries with the two-term interpolation weight
 inline int ring_launch(const RingConfig &cfg, const RingTables &tab0, const RingTables &tab1, const RingLaunch &Lin,
-                       int F, bool d32, bool apod, cudaStream_t st) {
+                       int F, bool d32, bool w2, bool apod, cudaStream_t st) {
     RingLaunch L = Lin;
     const RingTables *tabs[2] = {&tab0, &tab1};
     for (int a = 0; a < 2; ++a) {
@@ -228,8 +246,10 @@ inline int ring_launch(const RingConfig &cfg, const RingTables &tab0, const Ring
         L.ap[a].n_tiles = L.ap[a].n_tx > 0 ? tabs[a]->n_tiles : 0;
     }
     L.window = cfg.window;
-    if (F == 12) return d32 ? ring_launch_a<12, true>(cfg, L, apod, st) : ring_launch_a<12, false>(cfg, L, apod, st);
-    return d32 ? ring_launch_a<4, true>(cfg, L, apod, st) : ring_launch_a<4, false>(cfg, L, apod, st);
+    if (F == 12) return d32 ? ring_launch_a<12, true, false>(cfg, L, apod, st)
+                            : (w2 ? ring_launch_a<12, false, true>(cfg, L, apod, st) : ring_launch_a<12, false, false>(cfg, L, apod, st));
+    return d32 ? ring_launch_a<4, true, false>(cfg, L, apod, st)
+               : (w2 ? ring_launch_a<4, false, true>(cfg, L, apod, st) : ring_launch_a<4, false, false>(cfg, L, apod, st));
 }
 
 }  // namespace ulm

@@ -60,3 +60,29 @@ def test_reference_arm_other_ranks_exit_without_work():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
                         "--warmup", "0", "--gpus", "2"], env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_flag_without_a_launcher_starts_the_ranks_itself():
+    """`python bench.py --gpus 2` with WORLD_SIZE unset goes through bench.launch_ranks (torch.distributed.run,
+    2 ranks) and prints ONE line with n_gpus = 2; the CPU stand-in uses gloo and a sleep for the kernels."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-launch"], env=env,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    rec = json.loads(lines[0])
+    assert rec["n_gpus"] == 2 and rec["ms_per_step"] == pytest.approx(20.0)
+    assert rec["value"] == pytest.approx(2 * 300 / 20e-3)
+
+
+def test_gpus_flag_fails_loudly_when_the_devices_are_missing():
+    """No silent 1-GPU run: asking for more GPUs than are visible exits non-zero and prints no JSON line."""
+    import torch
+    if torch.cuda.device_count() >= 2:
+        pytest.skip("two CUDA devices are present")
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"], env=env,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "{" not in r.stdout
