@@ -1,4 +1,5 @@
-"""fp64 CPU oracle of the RCA Stage-1 projection beamformer -- TEST INFRASTRUCTURE.
+"""fp64 CPU oracle of the RCA projection beamformer (Stage 1: ulm_oracle.c; Stage 2 + sum-projection: stage2.py)
+-- TEST INFRASTRUCTURE.
 
 Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
 ``--impl reference`` legs may import this package (see oracle/ulm_oracle.h).  It imports nothing
@@ -14,3 +15,4 @@ from .oracle import (  # noqa: F401
     threads,
     volume,
 )
+from . import stage2  # noqa: F401,E402
