@@ -322,6 +322,111 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+
+def run_stage2(args):
+    """NEXT-1: Stage-2 extrapolation + compounding over 2K + P = 8 sum-projection (PAPER.md:45, 79, 93,
+    117) on the per-event slices of a 300-frame ensemble of config 2's shape: 22 slices of 180 x 164 px per frame ->
+    23 + 23 projected planes per frame.  One step = ulm_rca_stage2_project over the whole ensemble, slices resident in
+    HBM (1.56 GB in, 3.26 GB out: larger than L2)."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build, fp32_peak_tflops
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(2).with_(compound=0)
+    n_frames, block = cfg.n_frames, 8
+    kw = rounded_kwargs(cfg)
+    per_frame = len(cfg.row_tx_angles) * cfg.grid_xz[0] * cfg.grid_xz[3] + len(cfg.col_tx_angles) * cfg.grid_yz[0] * cfg.grid_yz[3]
+    n_distinct = 3
+    distinct = synth.random_complex((n_distinct, per_frame), 21, amplitude=50.0)
+    idx = torch.arange(n_frames, device="cuda") % n_distinct
+    slices = torch.from_numpy(distinct).cuda()[idx].contiguous()
+    warmup = max(args.warmup, 3)
+    with Plan(**kw, stage2_block=block, max_frames=n_frames) as plan:
+        out = plan.stage2_project(slices)
+        for _ in range(warmup):
+            plan.stage2_project(slices, out=out)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        stream = torch.cuda.current_stream()
+        marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        gs_ms = pj_ms = 0.0
+        marks[0].record(stream)
+        for i in range(args.steps):
+            plan.stage2_project(slices, out=out)
+            marks[i + 1].record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        ms = marks[0].elapsed_time(marks[args.steps]) / args.steps
+        gs_ms, pj_ms = plan.stage2_timing()
+        info = plan.info()
+        n_g = (plan.n_planes_xz, plan.n_planes_yz)
+        got = out[:n_distinct].cpu().numpy()
+        # end to end: pinned host slices -> device -> planes -> pinned host
+        h_in = torch.empty(slices.shape, dtype=torch.complex64, pin_memory=True)
+        h_in.copy_(slices)
+        h_out = torch.empty(out.shape, dtype=torch.complex64, pin_memory=True)
+        d_in = torch.empty_like(slices)
+        t0 = time.perf_counter()
+        for _ in range(2):
+            d_in.copy_(h_in, non_blocking=True)
+            plan.stage2_project(d_in, out=out)
+            h_out.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / 2
+    fp32_probe = fp32_peak_tflops()
+    # work: definition = every (voxel, event) term: linear interpolation (6 flop) + carrier rotation-accumulate (8) +
+    # block sum (2); executed = complex multiply-adds of the factored form (DESIGN.md 11), 8 flop each
+    nx, ny, nz = cfg.grid_xz[0], cfg.grid_yz[0], cfg.grid_xz[3]
+    kr, kc = len(cfg.row_tx_angles), len(cfg.col_tx_angles)
+    terms_def = float(nx) * ny * nz * (kr + kc) * 2 * n_frames          # each voxel term feeds both plane stacks
+    cmac = float(n_frames) * nz * (n_g[0] * nx * (kr * info["stage2_taps"] + kc * 2) + n_g[1] * ny * (kc * info["stage2_taps"] + kr * 2))
+    flop_exec, flop_def = 8.0 * cmac, 16.0 * terms_def
+    byts = float(slices.numel() + out.numel()) * 8
+    peak_hbm, hbm_src = hbm_peak()
+    t_alu, t_hbm = flop_exec / (NOMINAL_FP32_TFLOPS * 1e12) * 1e3, byts / (peak_hbm * 1e9) * 1e3
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        from oracle import stage2
+        p = oracle.OracleParams(**kw)
+        t0 = time.perf_counter()
+        ref = stage2.stage2_planes(p, distinct[:2].astype(np.complex128), block)
+        dt = time.perf_counter() - t0
+        parity = max(float(np.abs(got[i] - ref[i]).max() / np.abs(ref[i]).max()) for i in range(2))
+        cpu = {"value": 2 / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
+               "sample": "2 frames of the same slices (oracle/stage2.py, numpy fp64, single thread), %.1f s" % dt,
+               "parity_max_rel_err_vs_oracle": parity}
+    print(json.dumps({
+        "metric": "Stage-2 + compounding + P=8 sum-projected frames/s (300-frame ensemble)", "value": n_frames / (ms * 1e-3),
+        "unit": "frames/s", "n_gpus": 1, "steps": args.steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 complex (taps built in fp64 on the host)",
+        "data": "synthetic: 3 seeded random complex slice sets (synth.random_complex) tiled over 300 frames",
+        "config": {"workload": "SURVEY 8(f) NEXT-1 on BASELINE configs[2] shapes: 300 frames x 22 slices of %dx%d px -> %d+%d "
+                               "planes (P = %d)" % (nx, nz, n_g[0], n_g[1], block),
+                   "l2_policy": "inputs + outputs (%.1f GB) larger than L2, no flush" % (byts / 1e9), "plan": info},
+        "kernels_ms": {"groupsum": gs_ms, "project": pj_ms},
+        "roofline": {"bound": "alu", "achieved": flop_exec / (pj_ms * 1e-3) / 1e12, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
+                     "frac": flop_exec / (pj_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS, "peak_measured": fp32_probe,
+                     "frac_of_measured": flop_exec / (pj_ms * 1e-3) / 1e12 / fp32_probe, "traffic": None,
+                     "kernel": "stage2_project_kernel<%d>" % info["stage2_taps"], "kernel_ms": pj_ms,
+                     "executed_complex_macs": cmac, "flop_executed": flop_exec, "flop_of_the_definition": flop_def,
+                     "frac_on_definition_count": flop_def / (pj_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
+                     "alu_bound_ms": t_alu, "hbm_bound_ms": t_hbm, "algorithmic_bytes": byts,
+                     "hbm_frac_whole_step": byts / (ms * 1e-3) / 1e9 / peak_hbm, "hbm_peak_source": hbm_src},
+        "cpu_baseline": cpu, "clocks": clocks,
+        "e2e": {"value": n_frames / (e2e_ms * 1e-3), "unit": "frames/s", "h2d_bytes_per_step": int(slices.numel() * 8),
+                "d2h_bytes_per_step": int(out.numel() * 8), "ms_per_step": e2e_ms, "steps": 2},
+        "gpu_launches": int(info["launches_last_call"]) * args.steps}))
+
+
 def run_volume(args):
     """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
     180 x 180 x 164 volume by unpack_frame_kernel + das_volume_kernel (one frame); reported as volumes/s next to the
@@ -459,6 +564,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
+    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2"],
+                    help="beamform = the BASELINE metric (Stage 1); stage2 = SURVEY 8(f) NEXT-1 on config 2's shapes")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
                     help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
     ap.add_argument("--no-arms", action="store_true", help="skip the other scratch formats (roofline_full, ...)")
@@ -482,6 +589,8 @@ def main():
         run_selftest_launch(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.workload == "stage2":
+        run_stage2(args)
     elif args.config == 4:
         run_volume(args)
     else:

@@ -102,7 +102,9 @@ typedef struct {
                                    < 2^-16 relative per term (zero-mean), on which frames share its chunk.       */
     int32_t no_timing;          /* 1 = ulm_rca_beamform records no CUDA events around its kernels (and
                                    ulm_rca_plan_timing is unavailable); 0 = three cudaEventRecord per batch   */
-    int32_t reserved[3];        /* must be 0                                                           */
+    int32_t stage2_block;       /* P > 0: also prepare ulm_rca_stage2_project with sub-blocks of P x P voxel columns
+                                   (P = 8; needs identical axial grids); 0 = not prepared           */
+    int32_t reserved[2];        /* must be 0                                                           */
 } ulm_rca_options;
 
 /*
@@ -173,7 +175,9 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [11] tiles per projection (y-z)   [12] precision in use (1 compact / 2 full)
  *   [13] scratch bytes per (sample, frame)   [14] bytes per frame ulm_rca_beamform_host uploads
  *   [15] transmit events beamformed per frame by ulm_rca_beamform after folding (see below; = n_row_tx + n_col_tx
- *        when nothing folds) */
+ *        when nothing folds)
+ *   [16] Stage 2: depth taps per (event, group) FIR executed by the kernel (0 = Stage 2 not prepared)
+ *   [17] Stage 2: columns of the shared-memory slice tile (24 depths + halo) */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this
@@ -185,6 +189,39 @@ ulm_rca_status ulm_rca_plan_timing(const ulm_rca_plan *plan, int32_t n_calls, do
 /* FP32 FMA throughput probe used for the roofline denominator: runs a register-only FFMA loop on every
  * SM on cuda_stream, synchronises, and returns the measured TFLOP/s (2 flop per FMA) in *tflops. */
 ulm_rca_status ulm_rca_fp32_peak(double *tflops, void *cuda_stream);
+
+/*
+ * Stage 2 of the two-stage beamformer fused with the coherent compounding over all 2K transmissions and the sub-block
+ * sum-projection ("the full volume V_k is reconstructed from [the slice] by extrapolating along the
+ * transmit direction ... the compounded volume V is obtained by coherently summing all V_k-RC and V_k-CR";
+ * the volume is divided into P x P x N sub-blocks that are "sum-projected along lateral (x) and
+ * elevational (y) directions, resulting in projected planes V_p-m (m = 1 .. N/P x 2)"; P = 8).  The paper
+ * prints no formula; the reading implemented is DESIGN.md section 11 (= oracle/stage2.py):
+ *   voxel (lat, w, z_i) of event k, w = coordinate along the event's transmit direction, ref = the slice's position:
+ *     tau0_k(z) = t0_k + (z cos th_k + ref sin th_k)/c + z/c,   B_k(lat, i) = S_k(lat, i) exp(-j 2 pi fc tau0_k(z_i)),
+ *     q = i + (w - ref) tan(th_k/2) / dz,  n = floor(q),  b = q - n,  B_k = 0 outside the axial grid,
+ *     V_k(lat, w, z_i) = [(1-b) B_k(lat, n) + b B_k(lat, n+1)] exp(+j 2 pi fc (tau0_k(z_i) + (w - ref) sin th_k / c)),
+ *   V = sum of V_k over all row-tx (lat = x, w = y) and column-tx (lat = y, w = x) events on x = grid_xz lateral,
+ *   y = grid_yz lateral, z = the common axial grid;  XZ_m(x, z) = sum over the m-th group of P consecutive y of V,
+ *   YZ_m(y, z) = sum over the m-th group of P consecutive x of V (a last, shorter group is kept).
+ * The volume is never formed (the group sums are complex FIRs along z with host-built taps).
+ *   d_slices : complex fp32 [frame][event][lat][ax] -- exactly the compound == 0 output layout of ulm_rca_beamform
+ *              (the paper filters these slices before Stage 2; any such array may be passed), device memory
+ *   d_planes : complex fp32 [frame][ XZ: ceil(n_y/P) planes of n_x*n_ax | YZ: ceil(n_x/P) planes of n_y*n_ax ], axial
+ *              index fastest, device memory
+ * Needs options.stage2_block = P at plan_create (any `compound`); enqueues two kernels per batch of max_frames frames
+ * on cuda_stream and returns without synchronising; never allocates; one call in flight per plan.
+ */
+ulm_rca_status ulm_rca_stage2_project(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames,
+                                      void *d_planes, void *cuda_stream);
+
+/* Byte sizes per frame of the two buffers of ulm_rca_stage2_project and the plane counts (any pointer may be NULL). */
+ulm_rca_status ulm_rca_stage2_sizes(const ulm_rca_plan *plan, size_t *slices_bytes_per_frame,
+                                    size_t *planes_bytes_per_frame, int32_t *n_planes_xz, int32_t *n_planes_yz);
+
+/* Device time of the two kernels of the LAST batch of the last ulm_rca_stage2_project call (group sums, projection),
+ * from CUDA events recorded on the caller's stream; waits for them.  Unavailable with options.no_timing. */
+ulm_rca_status ulm_rca_stage2_timing(const ulm_rca_plan *plan, double *groupsum_ms, double *project_ms);
 
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets

@@ -21,6 +21,7 @@ _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
            "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
+           "ulm_rca_stage2_project", "ulm_rca_stage2_sizes", "ulm_rca_stage2_timing",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -45,7 +46,7 @@ class Options(C.Structure):
                 ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
                 ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
                 ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
-                ("precision", C.c_int32), ("no_timing", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("precision", C.c_int32), ("no_timing", C.c_int32), ("stage2_block", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
 def library_path() -> str:
@@ -78,6 +79,12 @@ def load() -> C.CDLL:
     lib.ulm_rca_plan_info.argtypes = [vp, C.POINTER(C.c_int64), i32]
     lib.ulm_rca_plan_timing.restype = C.c_int
     lib.ulm_rca_plan_timing.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.ulm_rca_stage2_project.restype = C.c_int
+    lib.ulm_rca_stage2_project.argtypes = [vp, vp, i32, vp, vp]
+    lib.ulm_rca_stage2_sizes.restype = C.c_int
+    lib.ulm_rca_stage2_sizes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(i32), C.POINTER(i32)]
+    lib.ulm_rca_stage2_timing.restype = C.c_int
+    lib.ulm_rca_stage2_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_ring_probe.restype = C.c_int
@@ -108,7 +115,8 @@ def _farr(v):
 
 
 INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
-             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame", "events_executed"]
+             "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame", "events_executed",
+             "stage2_taps", "stage2_tile_cols"]
 
 
 class Plan:
@@ -123,7 +131,7 @@ class Plan:
                  t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
                  elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
                  max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0,
-                 no_timing: bool = False):
+                 no_timing: bool = False, stage2_block: int = 0):
         lib = load()
         self._h = C.c_void_p()
         geo = Geometry(n_rows, n_cols, pitch)
@@ -137,7 +145,7 @@ class Plan:
             raise ValueError("elem_window must have n_cols + n_rows entries")
         opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
                       float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
-                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0)
+                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0, int(stage2_block))
         gx, gy = Grid(*grid_xz), Grid(*grid_yz)
         _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
                                        float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),
@@ -151,6 +159,12 @@ class Plan:
         self.n_row_tx, self.n_col_tx = len(row_tx_angles), len(col_tx_angles)
         import torch
         self.device_index = torch.cuda.current_device()      # the plan belongs to the device current at creation
+        self.stage2_block = int(stage2_block)
+        if self.stage2_block:
+            sb, pb, nxz, nyz = C.c_size_t(), C.c_size_t(), C.c_int32(), C.c_int32()
+            _check(lib.ulm_rca_stage2_sizes(self._h, C.byref(sb), C.byref(pb), C.byref(nxz), C.byref(nyz)))
+            self.slices_bytes_per_frame, self.planes_bytes_per_frame = sb.value, pb.value
+            self.n_planes_xz, self.n_planes_yz = nxz.value, nyz.value
 
     # -- lifetime -------------------------------------------------------------------------------------
     def close(self):
@@ -234,6 +248,33 @@ class Plan:
         _check(load().ulm_rca_beamform_volume(self._h, C.c_void_p(channel.data_ptr()), n_frames,
                                               C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
         return out
+
+    def stage2_project(self, slices, out=None, stream=None):
+        """Stage 2 + compounding + P-block sum-projection (ulm_rca_stage2_project).  slices: complex64 CUDA tensor
+        [frame][compound = 0 output of beamform()]; returns complex64 [frame][planes_bytes_per_frame / 8]."""
+        import torch
+        if not self.stage2_block:
+            raise ValueError("the plan was created without stage2_block")
+        if not (slices.is_cuda and slices.dtype == torch.complex64 and slices.is_contiguous()
+                and slices.device.index == self.device_index):
+            raise ValueError("slices must be a contiguous complex64 CUDA tensor on the plan's device")
+        n_frames = int(slices.shape[0])
+        if n_frames and slices.numel() * 8 != n_frames * self.slices_bytes_per_frame:
+            raise ValueError("slices have %d bytes per frame, plan expects %d" %
+                             (slices.numel() * 8 // n_frames, self.slices_bytes_per_frame))
+        if out is None:
+            out = torch.empty((n_frames, self.planes_bytes_per_frame // 8), dtype=torch.complex64, device=slices.device)
+        else:
+            self._check_out(out, n_frames * self.planes_bytes_per_frame // 8)
+        _check(load().ulm_rca_stage2_project(self._h, C.c_void_p(slices.data_ptr()), n_frames,
+                                             C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
+        return out
+
+    def stage2_timing(self) -> tuple:
+        """(groupsum_ms, project_ms) of the last batch of the last stage2_project() call."""
+        a, b = C.c_double(), C.c_double()
+        _check(load().ulm_rca_stage2_timing(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def beamform_host(self, channel: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
         """Host-buffer entry (H2D + beamform + D2H + synchronise inside the library)."""

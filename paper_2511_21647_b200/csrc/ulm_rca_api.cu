@@ -15,6 +15,7 @@
 
 #include "ulm_rca_device.cuh"
 #include "ulm_rca_ring_host.cuh"
+#include "ulm_rca_stage2_host.cuh"
 
 namespace {
 
@@ -124,6 +125,7 @@ struct ulm_rca_plan {
     static constexpr int kHostSlots = 2;
     cudaEvent_t h_in_done[kHostSlots] = {}, h_slot_free[kHostSlots] = {};
     bool timing = true;           // record CUDA events around the kernels (options.no_timing = 0)
+    ulm::Stage2Plan s2;           // Stage 2 + sum-projection tables (options.stage2_block > 0)
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -489,7 +491,10 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
     if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
-    for (int i = 0; i < 3; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    for (int i = 0; i < 2; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->stage2_block < 0 || opt->stage2_block > 4096) return fail(ULM_RCA_EINVAL, "stage2_block must be 0 .. 4096");
+    if (opt->stage2_block && (grid_xz->n_ax != grid_yz->n_ax || grid_xz->z0_m != grid_yz->z0_m || grid_xz->dz_m != grid_yz->dz_m))
+        return fail(ULM_RCA_EINVAL, "stage2_block needs identical axial grids");
     if (opt->no_timing != 0 && opt->no_timing != 1) return fail(ULM_RCA_EINVAL, "no_timing must be 0 or 1");
     if (opt->precision < 0 || opt->precision > 3) return fail(ULM_RCA_EINVAL, "precision must be 0, 1, 2 or 3");
     if (opt->input_kind != 0 && opt->input_kind != 1) return fail(ULM_RCA_EINVAL, "input_kind must be 0 or 1");
@@ -657,6 +662,19 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
         if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
     }
     if (P.timing) for (auto &c : P.ev) for (auto &b : c) for (auto &e : b) CUDA_TRY(cudaEventCreate(&e));
+    if (opt->stage2_block > 0) {
+        ulm::Stage2Axis ax[2];
+        for (int a = 0; a < 2; ++a) {
+            ax[a].n_lat = P.ap[a].g.n_lat; ax[a].lat0 = P.ap[a].g.lat0; ax[a].dlat = P.ap[a].g.dlat; ax[a].ref = P.ap[a].g.ref;
+            ax[a].angles = P.ap[a].angles;
+        }
+        if (const char *why = ulm::stage2_build(P.s2, ax, P.ap[0].g.n_ax, P.ap[0].g.dz, P.c, P.fc, opt->stage2_block,
+                                                 P.max_frames, P.timing)) {
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "stage 2: %s: %s", why, cudaGetErrorString(e));
+            return fail(ULM_RCA_EUNSUPPORTED, "stage 2: %s", why);
+        }
+    }
     CUDA_TRY(cudaDeviceSynchronize());
     guard.p = nullptr;
     *out = Pp;
@@ -674,13 +692,14 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *ch, size_t *
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n) {
     if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
     const bool ring = plan->kernel == 2, d32 = plan->d32;
-    const int64_t vals[16] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
+    const int64_t vals[18] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
                               ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
                               ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
                               ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
                               ring ? plan->ap[1].ring.n_tiles : 0, d32 ? 2 : (plan->w2 ? 3 : 1), ulm::entry_bytes(12, d32) / 12,
-                              (int64_t)host_upload_bytes_per_frame(*plan), plan->nv_events};
-    for (int i = 0; i < n && i < 16; ++i) v[i] = vals[i];
+                              (int64_t)host_upload_bytes_per_frame(*plan), plan->nv_events,
+                              plan->s2.ready ? plan->s2.nt : 0, plan->s2.ready ? plan->s2.ncol : 0};
+    for (int i = 0; i < n && i < 18; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
 }
 
@@ -885,6 +904,49 @@ ulm_rca_status ulm_rca_beamform_host(ulm_rca_plan *plan, const void *h_channel, 
     }
     HOST_TRY(cudaStreamSynchronize(plan->h_compute));
 #undef HOST_TRY
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_stage2_sizes(const ulm_rca_plan *plan, size_t *slices_bytes_per_frame, size_t *planes_bytes_per_frame,
+                                    int32_t *n_planes_xz, int32_t *n_planes_yz) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->s2.ready) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without stage2_block");
+    if (slices_bytes_per_frame) *slices_bytes_per_frame = (size_t)plan->s2.slices_per_frame * sizeof(float2);
+    if (planes_bytes_per_frame) *planes_bytes_per_frame = (size_t)plan->s2.planes_per_frame * sizeof(float2);
+    if (n_planes_xz) *n_planes_xz = plan->s2.n_g[0];
+    if (n_planes_yz) *n_planes_yz = plan->s2.n_g[1];
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_stage2_project(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames, void *d_planes,
+                                      void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->s2.ready) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without stage2_block");
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!d_slices || !d_planes) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
+    if (ulm_rca_status s = check_device(*plan)) return s;
+    const ulm::Stage2Plan &S = plan->s2;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int launches = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += S.max_frames) {
+        const int nb = std::min(S.max_frames, n_frames - f0);
+        CUDA_TRY(ulm::stage2_launch(S, static_cast<const float2 *>(d_slices) + (long long)f0 * S.slices_per_frame, nb,
+                                    static_cast<float2 *>(d_planes) + (long long)f0 * S.planes_per_frame, st, &launches));
+    }
+    plan->last_launches = launches;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_stage2_timing(const ulm_rca_plan *plan, double *groupsum_ms, double *project_ms) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->s2.ready || !plan->s2.ev[0]) return fail(ULM_RCA_EUNSUPPORTED, "no Stage-2 timing events on this plan");
+    float a = 0, b = 0;
+    CUDA_TRY(cudaEventSynchronize(plan->s2.ev[2]));
+    CUDA_TRY(cudaEventElapsedTime(&a, plan->s2.ev[0], plan->s2.ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(&b, plan->s2.ev[1], plan->s2.ev[2]));
+    if (groupsum_ms) *groupsum_ms = a;
+    if (project_ms) *project_ms = b;
     return ULM_RCA_OK;
 }
 

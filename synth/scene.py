@@ -163,3 +163,10 @@ def random_channel(cfg: RcaConfig, n_frames: int, seed: int, amplitude: int = 20
     if cfg.input_kind == 1:
         shape = shape + (2,)
     return rng.integers(-amplitude, amplitude + 1, size=shape, dtype=np.int16)
+
+
+def random_complex(shape, seed: int, amplitude: float = 1.0) -> np.ndarray:
+    """Seeded complex64 array (normal real and imaginary parts): stand-in for beamformed slices / images where a test
+    of a later pipeline stage needs an input that does not come from either beamformer."""
+    rng = _rng(seed, 11)
+    return (amplitude * (rng.standard_normal(shape) + 1j * rng.standard_normal(shape))).astype(np.complex64)
