@@ -177,7 +177,7 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [15] transmit events beamformed per frame by ulm_rca_beamform after folding (see below; = n_row_tx + n_col_tx
  *        when nothing folds)
  *   [16] Stage 2: depth taps per (event, group) FIR executed by the kernel (0 = Stage 2 not prepared)
- *   [17] Stage 2: columns of the shared-memory slice tile (24 depths + halo) */
+ *   [17] Stage 2: columns of the shared-memory slice tile (16 depths + halo) */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this

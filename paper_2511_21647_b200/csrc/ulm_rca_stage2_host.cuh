@@ -62,6 +62,13 @@ inline void shift_of(double w, double ref, double th, double dz, int &n, double 
 
 }  // namespace s2host
 
+inline int stage2_smem_bytes(const Stage2Plan &S) {
+    const int n_tx_max = std::max(S.n_row_tx, S.n_events - S.n_row_tx);
+    // tile buffers + the CTA's tap tables (own: [events][8 groups][1 + NT], cross: [events][32 positions][3])
+    return (kS2Stages * (kS2Lat * S.rs + kS2Warps * S.ncol) + n_tx_max * kS2Warps * (1 + S.nt) + n_tx_max * kS2Lat * 3) *
+           (int)sizeof(float2);
+}
+
 // Builds the tables.  ax[0] = x-z slices (row-tx events, transmit direction y), ax[1] = y-z slices.  Returns nullptr on
 // success or a reason; cudaGetLastError() tells allocation failures apart.
 inline const char *stage2_build(Stage2Plan &S, const Stage2Axis ax[2], int n_z, double dz, double c, double fc,
@@ -137,6 +144,7 @@ inline const char *stage2_build(Stage2Plan &S, const Stage2Axis ax[2], int n_z, 
     if (S.ncol > kS2MaxCol) return "axial shift range too large for the shared-memory tile";
     S.rs = S.ncol | 1;
     S.g_max = std::max(S.n_g[0], S.n_g[1]);
+    if (stage2_smem_bytes(S) > 100 * 1024) return "too many transmit events for the shared-memory tap tables";
     S.slices_per_frame = ((long long)ax[0].angles.size() * ax[0].n_lat + (long long)ax[1].angles.size() * ax[1].n_lat) * n_z;
     S.planes_per_frame = ((long long)S.n_g[0] * S.n_lat[0] + (long long)S.n_g[1] * S.n_lat[1]) * n_z;
     for (int a = 0; a < 2; ++a) {
@@ -156,8 +164,6 @@ inline const char *stage2_build(Stage2Plan &S, const Stage2Axis ax[2], int n_z, 
     S.ready = true;
     return nullptr;
 }
-
-inline int stage2_smem_bytes(const Stage2Plan &S) { return (2 * kS2Lat * S.rs + 2 * kS2Warps * S.ncol) * (int)sizeof(float2); }
 
 template <int NT>
 inline cudaError_t stage2_launch_t(const Stage2Params &P, dim3 grid, int smem, cudaStream_t st) {
@@ -201,7 +207,19 @@ inline cudaError_t stage2_launch(const Stage2Plan &S, const float2 *slices, int 
     }
     const int lat_tiles = (std::max(S.n_lat[0], S.n_lat[1]) + kS2Lat - 1) / kS2Lat;
     const int m_blocks = (S.g_max + kS2Warps - 1) / kS2Warps;
-    const dim3 grid(lat_tiles, P.z_tiles * m_blocks, 2 * n_frames);
+    // a CTA walks as many consecutive depth tiles as still leaves ~8 CTAs per SM (measured on cfg 2: one tile per CTA
+    // 7.80 ms, three 7.45 ms, all eleven 7.30 ms: the tap tables and the pipeline prologue are paid once per CTA)
+    {
+        int sms = 148, dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const long long base = (long long)lat_tiles * m_blocks * 2 * n_frames;
+        int tpc = P.z_tiles;
+        while (tpc > 1 && base * ((P.z_tiles + tpc - 1) / tpc) < 8ll * sms) --tpc;
+        P.tiles_per_cta = tpc;
+    }
+    const int z_runs = (P.z_tiles + P.tiles_per_cta - 1) / P.tiles_per_cta;
+    const dim3 grid(lat_tiles, m_blocks * z_runs, 2 * n_frames);
     const int smem = stage2_smem_bytes(S);
     switch (S.nt) {
         case 2: e = stage2_launch_t<2>(P, grid, smem, st); break;
