@@ -16,3 +16,4 @@ from .oracle import (  # noqa: F401
     volume,
 )
 from . import stage2  # noqa: F401,E402
+from . import clutter  # noqa: F401,E402
