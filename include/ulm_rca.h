@@ -104,7 +104,9 @@ typedef struct {
                                    ulm_rca_plan_timing is unavailable); 0 = three cudaEventRecord per batch   */
     int32_t stage2_block;       /* P > 0: also prepare ulm_rca_stage2_project with sub-blocks of P x P voxel columns
                                    (P = 8; needs identical axial grids); 0 = not prepared           */
-    int32_t reserved[2];        /* must be 0                                                           */
+    int32_t clutter_frames;     /* n_t > 0: also prepare ulm_rca_clutter_filter for ensembles of up to n_t frames
+                                   (32 .. 320; sizes the bf16 operand planes: ~8 bytes per slice value); 0 = not    */
+    int32_t reserved[1];        /* must be 0                                                           */
 } ulm_rca_options;
 
 /*
@@ -222,6 +224,33 @@ ulm_rca_status ulm_rca_stage2_sizes(const ulm_rca_plan *plan, size_t *slices_byt
 /* Device time of the two kernels of the LAST batch of the last ulm_rca_stage2_project call (group sums, projection),
  * from CUDA events recorded on the caller's stream; waits for them.  Unavailable with options.no_timing. */
 ulm_rca_status ulm_rca_stage2_timing(const ulm_rca_plan *plan, double *groupsum_ms, double *project_ms);
+
+/*
+ * Eigen-based clutter filter on the Stage-1 slice stacks ("parallelly computing the covariance matrix C
+ * in C^{n_t x n_t} of I, performing a lightweight eigenvalue decomposition of C, and parallelly projecting to recover
+ * blood flow signals", "applied ... immediately on 2D slices S_k-RC/CR obtained from Stage 1").  Reading (DESIGN.md
+ * section 12 = oracle/clutter.py), per transmit event e with X[f][p] = slice value of pixel p in frame f:
+ *   C[i][j] = sum_p conj(X[i][p]) X[j][p];   U_c = the clutter_rank eigenvectors of the largest eigenvalues of C;
+ *   X_f[f][p] = X[f][p] - sum_m conj(U_c[f][m]) t_m[p],  t_m[p] = sum_f U_c[f][m] X[f][p]      (I_f = I (1 - U_c U_c^H)).
+ * The paper gives no rule for the number of clutter components: clutter_rank (0 .. 24) is an argument.
+ * C is formed on the tensor cores from bf16 (hi, lo) splits of the slices (three tcgen05.mma products per term, fp32
+ * accumulation: relative error of C ~1e-5); the clutter subspace by 32 blocked orthogonal iterations on 32 vectors + a
+ * Rayleigh-Ritz step, which is exact (to fp32) when lambda_{rank} is well separated from lambda_33 -- the tissue /
+ * blood separation the filter is used for; for a flat spectrum the subspace, hence the result, is not determined.
+ *   d_slices   : complex fp32 [frame][event][lat][ax] (compound == 0 layout), n_frames = n_t frames, device memory
+ *   d_filtered : same layout and size; may be the same pointer as d_slices (in place)
+ *   d_eigenvalues : NULL, or float [n_events][32]: the 32 largest eigenvalues of every C_e, descending
+ *   d_covariance  : NULL, or complex fp32 [n_events][n_t][n_t]: the covariance matrices
+ * Needs options.clutter_frames >= n_frames >= 32.  Enqueues five kernels on cuda_stream, never synchronises; one call in
+ * flight per plan.
+ */
+ulm_rca_status ulm_rca_clutter_filter(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames,
+                                      int32_t clutter_rank, void *d_filtered, void *d_eigenvalues, void *d_covariance,
+                                      void *cuda_stream);
+
+/* Device time of the last ulm_rca_clutter_filter call: ms4[0] bf16 split, [1] Gram (tcgen05) + assembly, [2] eigen-
+ * subspace, [3] projection.  Waits for the events.  Unavailable with options.no_timing. */
+ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms4);
 
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets

@@ -22,6 +22,7 @@ _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
            "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
            "ulm_rca_stage2_project", "ulm_rca_stage2_sizes", "ulm_rca_stage2_timing",
+           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -46,7 +47,7 @@ class Options(C.Structure):
                 ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
                 ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
                 ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
-                ("precision", C.c_int32), ("no_timing", C.c_int32), ("stage2_block", C.c_int32), ("reserved", C.c_int32 * 2)]
+                ("precision", C.c_int32), ("no_timing", C.c_int32), ("stage2_block", C.c_int32), ("clutter_frames", C.c_int32), ("reserved", C.c_int32 * 1)]
 
 
 def library_path() -> str:
@@ -85,6 +86,10 @@ def load() -> C.CDLL:
     lib.ulm_rca_stage2_sizes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), C.POINTER(i32), C.POINTER(i32)]
     lib.ulm_rca_stage2_timing.restype = C.c_int
     lib.ulm_rca_stage2_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.ulm_rca_clutter_filter.restype = C.c_int
+    lib.ulm_rca_clutter_filter.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp]
+    lib.ulm_rca_clutter_timing.restype = C.c_int
+    lib.ulm_rca_clutter_timing.argtypes = [vp, C.POINTER(C.c_double)]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_ring_probe.restype = C.c_int
@@ -131,7 +136,7 @@ class Plan:
                  t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
                  elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
                  max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0,
-                 no_timing: bool = False, stage2_block: int = 0):
+                 no_timing: bool = False, stage2_block: int = 0, clutter_frames: int = 0):
         lib = load()
         self._h = C.c_void_p()
         geo = Geometry(n_rows, n_cols, pitch)
@@ -145,7 +150,7 @@ class Plan:
             raise ValueError("elem_window must have n_cols + n_rows entries")
         opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
                       float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
-                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0, int(stage2_block))
+                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0, int(stage2_block), int(clutter_frames))
         gx, gy = Grid(*grid_xz), Grid(*grid_yz)
         _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
                                        float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),
@@ -159,6 +164,9 @@ class Plan:
         self.n_row_tx, self.n_col_tx = len(row_tx_angles), len(col_tx_angles)
         import torch
         self.device_index = torch.cuda.current_device()      # the plan belongs to the device current at creation
+        self.clutter_frames = int(clutter_frames)
+        self.n_events = len(row_tx_angles) + len(col_tx_angles)
+        self.slices_complex_per_frame = (len(row_tx_angles) * grid_xz[0] * grid_xz[3] + len(col_tx_angles) * grid_yz[0] * grid_yz[3])
         self.stage2_block = int(stage2_block)
         if self.stage2_block:
             sb, pb, nxz, nyz = C.c_size_t(), C.c_size_t(), C.c_int32(), C.c_int32()
@@ -269,6 +277,38 @@ class Plan:
         _check(load().ulm_rca_stage2_project(self._h, C.c_void_p(slices.data_ptr()), n_frames,
                                              C.c_void_p(out.data_ptr()), self._stream_ptr(stream)))
         return out
+
+    def clutter_filter(self, slices, rank: int, out=None, want_eigenvalues: bool = False, want_covariance: bool = False,
+                       stream=None):
+        """Eigen-based clutter filter (ulm_rca_clutter_filter) on complex64 CUDA slices [frame][compound = 0 output].
+        Returns the filtered slices, or (filtered, eigenvalues [n_events][32], covariance [n_events][n_t][n_t]) with the
+        requested extras (None where not requested)."""
+        import torch
+        if not self.clutter_frames:
+            raise ValueError("the plan was created without clutter_frames")
+        if not (slices.is_cuda and slices.dtype == torch.complex64 and slices.is_contiguous()
+                and slices.device.index == self.device_index and slices.dim() == 2
+                and slices.shape[1] == self.slices_complex_per_frame):
+            raise ValueError("slices must be a contiguous complex64 CUDA tensor [frame][%d] on the plan's device" % self.slices_complex_per_frame)
+        n_t = int(slices.shape[0])
+        if out is None:
+            out = torch.empty_like(slices)
+        else:
+            self._check_out(out, slices.numel())
+        lam = torch.empty((self.n_events, 32), dtype=torch.float32, device=slices.device) if want_eigenvalues else None
+        cov = torch.empty((self.n_events, n_t, n_t), dtype=torch.complex64, device=slices.device) if want_covariance else None
+        _check(load().ulm_rca_clutter_filter(self._h, C.c_void_p(slices.data_ptr()), n_t, int(rank), C.c_void_p(out.data_ptr()),
+                                             C.c_void_p(lam.data_ptr()) if lam is not None else None,
+                                             C.c_void_p(cov.data_ptr()) if cov is not None else None, self._stream_ptr(stream)))
+        if want_eigenvalues or want_covariance:
+            return out, lam, cov
+        return out
+
+    def clutter_timing(self) -> tuple:
+        """(split_ms, gram_ms, eig_ms, project_ms) of the last clutter_filter() call."""
+        v = (C.c_double * 4)()
+        _check(load().ulm_rca_clutter_timing(self._h, v))
+        return tuple(float(x) for x in v)
 
     def stage2_timing(self) -> tuple:
         """(groupsum_ms, project_ms) of the last batch of the last stage2_project() call."""

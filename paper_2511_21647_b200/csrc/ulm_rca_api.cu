@@ -16,6 +16,7 @@
 #include "ulm_rca_device.cuh"
 #include "ulm_rca_ring_host.cuh"
 #include "ulm_rca_stage2_host.cuh"
+#include "ulm_rca_clutter_host.cuh"
 
 namespace {
 
@@ -126,6 +127,7 @@ struct ulm_rca_plan {
     cudaEvent_t h_in_done[kHostSlots] = {}, h_slot_free[kHostSlots] = {};
     bool timing = true;           // record CUDA events around the kernels (options.no_timing = 0)
     ulm::Stage2Plan s2;           // Stage 2 + sum-projection tables (options.stage2_block > 0)
+    mutable ulm::ClutterPlan cf;  // clutter filter scratch (options.clutter_frames > 0)
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -491,7 +493,9 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
     if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
-    for (int i = 0; i < 2; ++i) if (opt->reserved[i]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->reserved[0]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->clutter_frames != 0 && (opt->clutter_frames < ulm::kCfB || opt->clutter_frames > ulm::kCfMaxFrames))
+        return fail(ULM_RCA_EINVAL, "clutter_frames must be 0 or %d .. %d", ulm::kCfB, ulm::kCfMaxFrames);
     if (opt->stage2_block < 0 || opt->stage2_block > 4096) return fail(ULM_RCA_EINVAL, "stage2_block must be 0 .. 4096");
     if (opt->stage2_block && (grid_xz->n_ax != grid_yz->n_ax || grid_xz->z0_m != grid_yz->z0_m || grid_xz->dz_m != grid_yz->dz_m))
         return fail(ULM_RCA_EINVAL, "stage2_block needs identical axial grids");
@@ -673,6 +677,22 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
             const cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "stage 2: %s: %s", why, cudaGetErrorString(e));
             return fail(ULM_RCA_EUNSUPPORTED, "stage 2: %s", why);
+        }
+    }
+    if (opt->clutter_frames > 0) {
+        std::vector<long long> off;
+        std::vector<int> npix;
+        long long o = 0;
+        for (int a = 0; a < 2; ++a)
+            for (int k = 0; k < P.ap[a].n_tx; ++k) {
+                off.push_back(o);
+                npix.push_back(P.ap[a].g.n_lat * P.ap[a].g.n_ax);
+                o += (long long)P.ap[a].g.n_lat * P.ap[a].g.n_ax;
+            }
+        if (const char *why = ulm::clutter_build(P.cf, off, npix, o, opt->clutter_frames, P.timing)) {
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "clutter filter: %s: %s", why, cudaGetErrorString(e));
+            return fail(ULM_RCA_EUNSUPPORTED, "clutter filter: %s", why);
         }
     }
     CUDA_TRY(cudaDeviceSynchronize());
@@ -947,6 +967,37 @@ ulm_rca_status ulm_rca_stage2_timing(const ulm_rca_plan *plan, double *groupsum_
     CUDA_TRY(cudaEventElapsedTime(&b, plan->s2.ev[1], plan->s2.ev[2]));
     if (groupsum_ms) *groupsum_ms = a;
     if (project_ms) *project_ms = b;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_clutter_filter(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames, int32_t clutter_rank,
+                                      void *d_filtered, void *d_eigenvalues, void *d_covariance, void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->cf.ready) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without clutter_frames");
+    if (n_frames < ulm::kCfB || n_frames > plan->cf.max_t)
+        return fail(ULM_RCA_EINVAL, "n_frames must be %d .. clutter_frames (%d)", ulm::kCfB, plan->cf.max_t);
+    if (clutter_rank < 0 || clutter_rank > ulm::kCfMaxRank) return fail(ULM_RCA_EINVAL, "clutter_rank must be 0 .. %d", ulm::kCfMaxRank);
+    if (!d_slices || !d_filtered) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
+    if (ulm_rca_status s = check_device(*plan)) return s;
+    int launches = 0;
+    const char *why = nullptr;
+    const cudaError_t e = ulm::clutter_launch(plan->cf, static_cast<const float2 *>(d_slices), n_frames, clutter_rank,
+                                              static_cast<float2 *>(d_filtered), static_cast<float *>(d_eigenvalues),
+                                              static_cast<float2 *>(d_covariance), (cudaStream_t)cuda_stream, &launches, &why);
+    if (e != cudaSuccess) return fail(why ? ULM_RCA_EUNSUPPORTED : ULM_RCA_ECUDA, "clutter filter: %s", why ? why : cudaGetErrorString(e));
+    plan->last_launches = launches;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms4) {
+    if (!plan || !ms4) return fail(ULM_RCA_EINVAL, "plan / ms4 is NULL");
+    if (!plan->cf.ready || !plan->cf.ev[0]) return fail(ULM_RCA_EUNSUPPORTED, "no clutter-filter timing events on this plan");
+    CUDA_TRY(cudaEventSynchronize(plan->cf.ev[4]));
+    for (int i = 0; i < 4; ++i) {
+        float v = 0;
+        CUDA_TRY(cudaEventElapsedTime(&v, plan->cf.ev[i], plan->cf.ev[i + 1]));
+        ms4[i] = v;
+    }
     return ULM_RCA_OK;
 }
 

@@ -170,3 +170,25 @@ def random_complex(shape, seed: int, amplitude: float = 1.0) -> np.ndarray:
     of a later pipeline stage needs an input that does not come from either beamformer."""
     rng = _rng(seed, 11)
     return (amplitude * (rng.standard_normal(shape) + 1j * rng.standard_normal(shape))).astype(np.complex64)
+
+
+def clutter_ensemble(n_t: int, n_pix_per_event, seed: int, tissue_rank: int = 3, tissue_gain_db: float = 30.0,
+                     bubble_density: float = 0.01, noise: float = 0.05) -> np.ndarray:
+    """Seeded complex64 slice stacks [n_t][sum of n_pix_per_event] shaped like clutter-dominated Stage-1 output (stand-in
+    for the in-vivo slices of PAPER.md:53-59, which are not available): per event, `tissue_rank` strong components
+    (smooth slow-time profile x fixed spatial speckle, tissue_gain_db above the bubbles, decaying 6 dB per component),
+    sparse unit-amplitude "bubble" samples that change from frame to frame, and white noise."""
+    rng = _rng(seed, 13)
+    f = np.arange(n_t)[:, None]
+    blocks = []
+    for n in n_pix_per_event:
+        x = noise * (rng.standard_normal((n_t, n)) + 1j * rng.standard_normal((n_t, n)))
+        hit = rng.random((n_t, n)) < bubble_density
+        x = x + hit * np.exp(2j * np.pi * rng.random((n_t, n)))
+        for m in range(tissue_rank):
+            gain = 10.0 ** ((tissue_gain_db - 6.0 * m) / 20.0)
+            drift = np.exp(2j * np.pi * (0.3 * (m + 1) * np.sin(2 * np.pi * (m + 1) * f / (2.5 * n_t) + rng.random()) + rng.random()))
+            speckle = (rng.standard_normal(n) + 1j * rng.standard_normal(n)) / np.sqrt(2.0)
+            x = x + gain * drift * speckle[None, :]
+        blocks.append(x)
+    return np.concatenate(blocks, axis=1).astype(np.complex64)
