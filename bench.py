@@ -427,6 +427,91 @@ def run_stage2(args):
         "gpu_launches": int(info["launches_last_call"]) * args.steps}))
 
 
+def run_clutter(args):
+    """NEXT-2: eigen-based clutter filter on the per-event slice stacks of a 300-frame
+    ensemble of config 2's shape: 22 stacks of 300 x 29 520 complex values; one step = ulm_rca_clutter_filter (bf16 split,
+    tcgen05 Gram kernel, assembly, eigen-subspace, projection), slices resident in HBM (1.56 GB > L2)."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(2).with_(compound=0)
+    n_t, rank = cfg.n_frames, 4
+    kw = rounded_kwargs(cfg)
+    n_pix = [cfg.grid_xz[0] * cfg.grid_xz[3]] * len(cfg.row_tx_angles) + [cfg.grid_yz[0] * cfg.grid_yz[3]] * len(cfg.col_tx_angles)
+    x = synth.clutter_ensemble(n_t, n_pix, seed=22, tissue_rank=rank)
+    d_x = torch.from_numpy(x).cuda()
+    warmup = max(args.warmup, 3)
+    with Plan(**kw, clutter_frames=n_t) as plan:
+        out = plan.clutter_filter(d_x, rank)
+        for _ in range(warmup):
+            plan.clutter_filter(d_x, rank, out=out)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        stream = torch.cuda.current_stream()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            plan.clutter_filter(d_x, rank, out=out)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        k_ms = dict(zip(("split", "gram", "assemble", "eig", "project"), plan.clutter_timing()))
+        info = plan.info()
+        h_in = torch.empty(d_x.shape, dtype=torch.complex64, pin_memory=True)
+        h_in.copy_(d_x)
+        h_out = torch.empty(d_x.shape, dtype=torch.complex64, pin_memory=True)
+        d_in = torch.empty_like(d_x)
+        t0 = time.perf_counter()
+        for _ in range(2):
+            d_in.copy_(h_in, non_blocking=True)
+            plan.clutter_filter(d_in, rank, out=out)
+            h_out.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / 2
+        got = out[:, :n_pix[0]].cpu().numpy()
+    # tensor-core roofline of the Gram kernel: algorithmic = 8 flop per complex multiply-add of C = I^H I (full, not the
+    # Hermitian half); executed = the bf16 x 3 real products over the upper-triangular 128 x 128 tiles of the padded Gram
+    n_ev = len(n_pix)
+    flop_alg = 8.0 * n_t * n_t * float(sum(n_pix))
+    nr = 2 * ((n_t + 63) // 64 * 64)
+    tiles = (nr // 128) * (nr // 128 + 1) // 2
+    flop_exec = 3 * 2.0 * tiles * 128 * 128 * ((max(n_pix) + 63) // 64 * 64) * n_ev
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peak, src = float(json.load(fh)["bf16_tflops"]), "MEASURED_PEAKS.json bf16_tflops (burst: the kernel is timed alone by CUDA events)"
+    except Exception:
+        peak, src = 1590.0, "fallback 1.59 PFLOP/s (B200_PROFILING.md)"
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import clutter
+        t0 = time.perf_counter()
+        ref, lam, _ = clutter.clutter_filter_stack(x[:, :n_pix[0]].astype(np.complex128), rank)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_t / (dt * n_ev), "unit": "frames/s", "cores": int(os.cpu_count() or 1), "kind": "oracle",
+               "sample": "1 of the %d slice stacks (oracle/clutter.py, numpy fp64 + LAPACK threads), %.1f s; scaled to %d stacks" % (n_ev, dt, n_ev),
+               "parity_max_err_over_max_input": float(np.abs(got - ref).max() / np.abs(x).max())}
+    print(json.dumps({
+        "metric": "clutter-filtered frames/s (300-frame ensemble, 22 slice stacks)", "value": n_t / (ms * 1e-3), "unit": "frames/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16 x 3 split operands, fp32 accumulate (covariance); fp32 (eigen-subspace, projection)",
+        "data": "synthetic: synth.clutter_ensemble (rank-4 tissue 30 dB above sparse bubbles + noise), seed 22",
+        "config": {"workload": "SURVEY 8(f) NEXT-2 on BASELINE configs[2] shapes: 22 stacks of 300 frames x 29520 px, clutter rank 4",
+                   "l2_policy": "inputs (%.2f GB) larger than L2, no flush" % (d_x.numel() * 8 / 1e9), "plan": info},
+        "kernels_ms": k_ms,
+        "roofline": {"bound": "tensor", "achieved": flop_alg / (k_ms["gram"] * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                     "frac": flop_alg / (k_ms["gram"] * 1e-3) / 1e12 / peak, "traffic": None, "kernel": "clutter_gram_kernel",
+                     "kernel_ms": k_ms["gram"], "flop_algorithmic": flop_alg, "flop_executed": flop_exec,
+                     "achieved_executed": flop_exec / (k_ms["gram"] * 1e-3) / 1e12,
+                     "frac_executed": flop_exec / (k_ms["gram"] * 1e-3) / 1e12 / peak, "peak_source": src},
+        "cpu_baseline": cpu, "clocks": clocks,
+        "e2e": {"value": n_t / (e2e_ms * 1e-3), "unit": "frames/s", "h2d_bytes_per_step": int(d_x.numel() * 8),
+                "d2h_bytes_per_step": int(d_x.numel() * 8), "ms_per_step": e2e_ms, "steps": 2},
+        "gpu_launches": int(info["launches_last_call"]) * args.steps}))
+
+
 def run_volume(args):
     """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
     180 x 180 x 164 volume by unpack_frame_kernel + das_volume_kernel (one frame); reported as volumes/s next to the
@@ -564,7 +649,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
-    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2"],
+    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter"],
                     help="beamform = the BASELINE metric (Stage 1); stage2 = SURVEY 8(f) NEXT-1 on config 2's shapes")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
                     help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
@@ -591,6 +676,8 @@ def main():
         run_reference(args)
     elif args.workload == "stage2":
         run_stage2(args)
+    elif args.workload == "clutter":
+        run_clutter(args)
     elif args.config == 4:
         run_volume(args)
     else:

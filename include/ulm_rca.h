@@ -234,7 +234,8 @@ ulm_rca_status ulm_rca_stage2_timing(const ulm_rca_plan *plan, double *groupsum_
  *   X_f[f][p] = X[f][p] - sum_m conj(U_c[f][m]) t_m[p],  t_m[p] = sum_f U_c[f][m] X[f][p]      (I_f = I (1 - U_c U_c^H)).
  * The paper gives no rule for the number of clutter components: clutter_rank (0 .. 24) is an argument.
  * C is formed on the tensor cores from bf16 (hi, lo) splits of the slices (three tcgen05.mma products per term, fp32
- * accumulation: relative error of C ~1e-5); the clutter subspace by 32 blocked orthogonal iterations on 32 vectors + a
+ * accumulation: relative error of C ~1e-5); the clutter subspace by blocked orthogonal iteration on 32 vectors (at most
+ * 24 steps; it stops three steps after the leading clutter_rank eigenvalue estimates have settled to 1e-6) + a
  * Rayleigh-Ritz step, which is exact (to fp32) when lambda_{rank} is well separated from lambda_33 -- the tissue /
  * blood separation the filter is used for; for a flat spectrum the subspace, hence the result, is not determined.
  *   d_slices   : complex fp32 [frame][event][lat][ax] (compound == 0 layout), n_frames = n_t frames, device memory
@@ -248,9 +249,9 @@ ulm_rca_status ulm_rca_clutter_filter(const ulm_rca_plan *plan, const void *d_sl
                                       int32_t clutter_rank, void *d_filtered, void *d_eigenvalues, void *d_covariance,
                                       void *cuda_stream);
 
-/* Device time of the last ulm_rca_clutter_filter call: ms4[0] bf16 split, [1] Gram (tcgen05) + assembly, [2] eigen-
- * subspace, [3] projection.  Waits for the events.  Unavailable with options.no_timing. */
-ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms4);
+/* Device time of the five kernels of the last ulm_rca_clutter_filter call: ms5[0] bf16 split, [1] Gram (tcgen05),
+ * [2] assembly of C, [3] eigen-subspace, [4] projection.  Waits for the events.  Unavailable with options.no_timing. */
+ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms5);
 
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets

@@ -305,8 +305,8 @@ class Plan:
         return out
 
     def clutter_timing(self) -> tuple:
-        """(split_ms, gram_ms, eig_ms, project_ms) of the last clutter_filter() call."""
-        v = (C.c_double * 4)()
+        """(split_ms, gram_ms, assemble_ms, eig_ms, project_ms) of the last clutter_filter() call."""
+        v = (C.c_double * 5)()
         _check(load().ulm_rca_clutter_timing(self._h, v))
         return tuple(float(x) for x in v)
 

@@ -990,13 +990,14 @@ ulm_rca_status ulm_rca_clutter_filter(const ulm_rca_plan *plan, const void *d_sl
 }
 
 ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms4) {
-    if (!plan || !ms4) return fail(ULM_RCA_EINVAL, "plan / ms4 is NULL");
+    double *ms5 = ms4;
+    if (!plan || !ms5) return fail(ULM_RCA_EINVAL, "plan / ms5 is NULL");
     if (!plan->cf.ready || !plan->cf.ev[0]) return fail(ULM_RCA_EUNSUPPORTED, "no clutter-filter timing events on this plan");
-    CUDA_TRY(cudaEventSynchronize(plan->cf.ev[4]));
-    for (int i = 0; i < 4; ++i) {
+    CUDA_TRY(cudaEventSynchronize(plan->cf.ev[5]));
+    for (int i = 0; i < 5; ++i) {
         float v = 0;
         CUDA_TRY(cudaEventElapsedTime(&v, plan->cf.ev[i], plan->cf.ev[i + 1]));
-        ms4[i] = v;
+        ms5[i] = v;
     }
     return ULM_RCA_OK;
 }

@@ -262,16 +262,17 @@ __global__ void __launch_bounds__(256) clutter_assemble_kernel(const __grid_cons
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kCfEigThreads = 512;
 constexpr int kCfQs = kCfB + 1;      // padded row stride of Q / Z (float2)
-constexpr int kCfKc = 8;             // columns of C staged per step
+constexpr int kCfKc = 16;            // columns of C staged per step
 __host__ __device__ inline int clutter_eig_smem_bytes(int n_t) {
-    return (2 * n_t * kCfQs + n_t * (kCfKc + 1) + 2 * kCfB * kCfQs) * 8 + 64 * 4;
+    return (2 * n_t * kCfQs + n_t * (kCfKc + 1) + 2 * kCfB * kCfQs) * 8 + 128 * 4;
 }
 
 struct CfEigParams {
     const float2 *cov;               // [event][n_t][n_t]
     float2 *uc;                      // [event][n_t][kCfB]  Ritz vectors, descending Ritz value
     float *lam;                      // [event][kCfB]       Ritz values, descending
-    int n_t, iters;
+    int n_t, iters;                  // iters = upper limit of the orthogonal iterations
+    int n_track;                     // the leading n_track (= rank) vectors decide convergence
 };
 
 __device__ __forceinline__ float2 cf_cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -285,7 +286,9 @@ __device__ __forceinline__ float cf_warp_sum(float v) {
 }
 
 // modified Gram-Schmidt of the kCfB columns of z (in place) -> q; both [n_t][kCfQs].  All threads of the CTA.
-__device__ void cf_mgs(float2 *z, float2 *q, int n_t) {
+// track != nullptr: track[c] keeps the squared norm of the orthogonalised column c < n_track (the running estimate of
+// lambda_c^2) and track[kCfB] is set to 1 when one of them moved by more than 1e-6 relative since the last call.
+__device__ void cf_mgs(float2 *z, float2 *q, int n_t, float *track = nullptr, int n_track = 0) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = kCfEigThreads / 32;
     for (int c = 0; c < kCfB; ++c) {
         // every warp forms the norm of column c itself (no extra barrier)
@@ -293,6 +296,10 @@ __device__ void cf_mgs(float2 *z, float2 *q, int n_t) {
         for (int i = lane; i < n_t; i += 32) { const float2 v = z[i * kCfQs + c]; nn += v.x * v.x + v.y * v.y; }
         nn = cf_warp_sum(nn);
         const float inv = nn > 0.f ? rsqrtf(nn) : 0.f, inv2 = nn > 0.f ? 1.f / nn : 0.f;
+        if (track && c < n_track && threadIdx.x == 0) {
+            if (fabsf(nn - track[c]) > 1e-6f * nn) track[kCfB] = 1.f;
+            track[c] = nn;
+        }
         for (int c2 = c + 1 + warp; c2 < kCfB; c2 += n_warps) {
             float pr = 0.f, pi = 0.f;
             for (int i = lane; i < n_t; i += 32) {
@@ -322,6 +329,7 @@ __global__ void __launch_bounds__(kCfEigThreads, 1) clutter_eig_kernel(const __g
     float2 *h = cs + n_t * (kCfKc + 1);                               // [kCfB][kCfQs]
     float2 *w = h + kCfB * kCfQs;                                     // [kCfB][kCfQs]
     int *order = reinterpret_cast<int *>(w + kCfB * kCfQs);           // [kCfB]
+    float *track = reinterpret_cast<float *>(order + kCfB);           // [kCfB + 1]
     const float2 *cov = P.cov + (long long)e * n_t * n_t;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
@@ -345,15 +353,28 @@ __global__ void __launch_bounds__(kCfEigThreads, 1) clutter_eig_kernel(const __g
         for (int a = 0; a < 5; ++a)
 #pragma unroll
             for (int b = 0; b < 4; ++b) acc[a][b] = make_float2(0.f, 0.f);
+        // the next chunk of C (kCfKc columns of all rows) is fetched into registers while the current one is used
+        constexpr int PF = (kCfMaxFrames * kCfKc + kCfEigThreads - 1) / kCfEigThreads;
+        float2 pre[PF];
+        auto fetch = [&](int k0) {
+#pragma unroll
+            for (int r_ = 0; r_ < PF; ++r_) {
+                const int i = tid + r_ * kCfEigThreads, r = i / kCfKc, kk = i - r * kCfKc;
+                pre[r_] = (r < n_t && k0 + kk < n_t) ? __ldg(cov + (long long)r * n_t + k0 + kk) : make_float2(0.f, 0.f);
+            }
+        };
+        fetch(0);
         for (int k0 = 0; k0 < n_t; k0 += kCfKc) {
             __syncthreads();                                          // previous chunk consumed
-            for (int i = tid; i < n_t * kCfKc; i += kCfEigThreads) {
-                const int r = i / kCfKc, kk = i - r * kCfKc;
-                cs[r * (kCfKc + 1) + kk] = (k0 + kk < n_t) ? __ldg(cov + (long long)r * n_t + k0 + kk) : make_float2(0.f, 0.f);
+#pragma unroll
+            for (int r_ = 0; r_ < PF; ++r_) {
+                const int i = tid + r_ * kCfEigThreads, r = i / kCfKc, kk = i - r * kCfKc;
+                if (r < n_t) cs[r * (kCfKc + 1) + kk] = pre[r_];
             }
             __syncthreads();
+            if (k0 + kCfKc < n_t) fetch(k0 + kCfKc);
             if (mm_ok) {
-#pragma unroll
+#pragma unroll 4
                 for (int kk = 0; kk < kCfKc; ++kk) {
                     const int k = min(k0 + kk, n_t - 1);              // a staged zero multiplies the clamped row
                     float2 qv[4];
@@ -380,9 +401,24 @@ __global__ void __launch_bounds__(kCfEigThreads, 1) clutter_eig_kernel(const __g
         __syncthreads();
     };
 
+    // Orthogonal iteration Q <- orth(C Q).  One Gram-Schmidt pass per step is enough while iterating (what it leaves
+    // of the dominant vectors in the later columns stays inside the span that matters); the basis is re-orthonormalised
+    // twice at the end.  Stop: three steps after the squared norms of the leading n_track orthogonalised columns -- the
+    // running lambda^2 estimates, which converge twice as fast as the vectors -- have settled to 1e-6, or at P.iters.
+    if (tid <= kCfB) track[tid] = 0.f;
+    __syncthreads();
+    int settled = -1;
     for (int it = 0; it < P.iters; ++it) {
         multiply();
-        cf_mgs(z, q, n_t);            // twice: the columns of C Q are very ill-conditioned (lambda_1 / lambda_32)
+        if (tid == 0) track[kCfB] = 0.f;
+        __syncthreads();
+        cf_mgs(z, q, n_t, track, P.n_track);
+        const bool moved = track[kCfB] != 0.f;                         // uniform: written before the barriers of cf_mgs
+        if (!moved && settled < 0) settled = it;
+        if (moved) settled = -1;
+        if (settled >= 0 && it >= settled + 3) break;
+    }
+    for (int pass = 0; pass < 2; ++pass) {
         for (int i = tid; i < n_t * kCfB; i += kCfEigThreads) { const int r = i / kCfB, c = i - r * kCfB; z[r * kCfQs + c] = q[r * kCfQs + c]; }
         __syncthreads();
         cf_mgs(z, q, n_t);

@@ -11,7 +11,7 @@ namespace ulm {
 
 struct ClutterPlan {
     bool ready = false;
-    int n_events = 0, max_t = 0, iters = 32, n_splits = 1;
+    int n_events = 0, max_t = 0, iters = 24, n_splits = 1;
     long long frame_stride = 0, k_max = 0, ld = 0;
     std::vector<long long> off;
     std::vector<int> n_pix;
@@ -20,7 +20,7 @@ struct ClutterPlan {
     size_t y_bytes = 0, partial_bytes = 0;
     int ntp_cached = 0;               // padded frame count the operand planes are currently laid out / cleared for
     CUtensorMap map_hi{}, map_lo{};
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     ~ClutterPlan() {
         for (void *p : {d_off, d_npix, y_hi, y_lo, partial, cov, uc, lam}) if (p) cudaFree(p);
         for (auto &e : ev) if (e) cudaEventDestroy(e);
@@ -120,19 +120,20 @@ inline cudaError_t clutter_launch(ClutterPlan &C, const float2 *x, int n_t, int 
     const int tiles = G.n_tiles_1d * (G.n_tiles_1d + 1) / 2;
     clutter_gram_kernel<<<dim3(tiles, C.n_splits, C.n_events), kCfGramThreads, kCfGramSmem, st>>>(C.map_hi, C.map_lo, G);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (C.ev[2] && (e = cudaEventRecord(C.ev[2], st)) != cudaSuccess) return e;
     CfAssembleParams A{};
     A.partial = static_cast<const float *>(C.partial); A.cov = static_cast<float2 *>(C.cov); A.nr = nr; A.ntp = ntp; A.n_t = n_t;
     A.n_splits = C.n_splits; A.n_events = C.n_events;
     clutter_assemble_kernel<<<dim3((n_t + 255) / 256, n_t, C.n_events), 256, 0, st>>>(A);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (C.ev[2] && (e = cudaEventRecord(C.ev[2], st)) != cudaSuccess) return e;
+    if (C.ev[3] && (e = cudaEventRecord(C.ev[3], st)) != cudaSuccess) return e;
 
     CfEigParams E{};
     E.cov = static_cast<const float2 *>(C.cov); E.uc = static_cast<float2 *>(C.uc); E.lam = static_cast<float *>(C.lam);
-    E.n_t = n_t; E.iters = C.iters;
+    E.n_t = n_t; E.iters = rank > 0 ? C.iters : 0; E.n_track = rank;
     clutter_eig_kernel<<<C.n_events, kCfEigThreads, clutter_eig_smem_bytes(n_t), st>>>(E);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (C.ev[3] && (e = cudaEventRecord(C.ev[3], st)) != cudaSuccess) return e;
+    if (C.ev[4] && (e = cudaEventRecord(C.ev[4], st)) != cudaSuccess) return e;
 
     CfProjectParams J{};
     J.x = x; J.out = out; J.frame_stride = C.frame_stride; J.ev = ev; J.uc = static_cast<const float2 *>(C.uc); J.n_t = n_t; J.rank = rank;
@@ -141,7 +142,7 @@ inline cudaError_t clutter_launch(ClutterPlan &C, const float2 *x, int n_t, int 
     else if (rank <= 16) clutter_project_kernel<16><<<pg, 128, n_t * 16 * 8, st>>>(J);
     else clutter_project_kernel<24><<<pg, 128, n_t * 24 * 8, st>>>(J);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if (C.ev[4] && (e = cudaEventRecord(C.ev[4], st)) != cudaSuccess) return e;
+    if (C.ev[5] && (e = cudaEventRecord(C.ev[5], st)) != cudaSuccess) return e;
     *launches += 5;
     if (lam_out && (e = cudaMemcpyAsync(lam_out, C.lam, (size_t)C.n_events * kCfB * sizeof(float), cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;
     if (cov_out && (e = cudaMemcpyAsync(cov_out, C.cov, (size_t)C.n_events * n_t * n_t * sizeof(float2), cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;

@@ -122,7 +122,7 @@ def test_config2_ensemble_size(torch_cuda):
         d_x = torch.from_numpy(x).cuda()
         out, lam, cov = plan.clutter_filter(d_x, rank, want_eigenvalues=True, want_covariance=True)
         torch.cuda.synchronize()
-        print("CLUTTER cfg2 kernel times (split, gram, eig, project) ms:", plan.clutter_timing())
+        print("CLUTTER cfg2 kernel times (split, gram, assemble, eig, project) ms:", plan.clutter_timing())
         lam, cov = lam.cpu().numpy(), cov.cpu().numpy()
         blocks = clutter.event_blocks(p)
         scale = np.abs(x).max()
