@@ -512,6 +512,87 @@ def run_clutter(args):
         "gpu_launches": int(info["launches_last_call"]) * args.steps}))
 
 
+def run_motion(args):
+    """NEXT-3: Fourier-domain NCC rigid motion estimation on the per-event slices of a
+    300-frame ensemble of config 2's shape (22 slices of 180 x 164 px per frame, 256 x 256 transforms), every frame
+    against frame 0; one step = ulm_rca_motion_estimate over the whole ensemble, slices resident in HBM."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(2).with_(compound=0)
+    kw = rounded_kwargs(cfg)
+    n_frames = cfg.n_frames
+    shapes = [(cfg.grid_xz[0], cfg.grid_xz[3])] * len(cfg.row_tx_angles) + [(cfg.grid_yz[0], cfg.grid_yz[3])] * len(cfg.col_tx_angles)
+    shifts = [(0.0, 0.0), (0.8, -0.6), (-1.4, 0.35), (2.6, 1.2)]
+    distinct = synth.moving_speckle(4, shapes, shifts, seed=2)
+    idx = torch.arange(n_frames, device="cuda") % 4
+    d = torch.from_numpy(distinct).cuda()[idx].contiguous()
+    warmup = max(args.warmup, 3)
+    with Plan(**kw, motion_frames=n_frames) as plan:
+        for _ in range(warmup):
+            mot, per = plan.motion_estimate(d, 0)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        stream = torch.cuda.current_stream()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            mot, per = plan.motion_estimate(d, 0)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        k_ms = plan.motion_timing()
+        info = plan.info()
+        h_in = torch.empty(d.shape, dtype=torch.complex64, pin_memory=True)
+        h_in.copy_(d)
+        d_in = torch.empty_like(d)
+        t0 = time.perf_counter()
+        for _ in range(2):
+            d_in.copy_(h_in, non_blocking=True)
+            m2, _ = plan.motion_estimate(d_in, 0)
+            m_host = m2.cpu()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / 2
+        per = per.cpu().numpy()
+    # HBM roofline: bytes the six kernels must move (slices read twice, T1 and T2 written and read once each) vs the
+    # minimum (slices read once); flops: 3 two-dimensional 256 x 256 transforms per image, 5 N log2 N each
+    n_img = n_frames * len(shapes)
+    fft_flop = sum(3 * 5.0 * (256 * 256) * 16 for _ in shapes) * n_frames
+    bytes_min = float(d.numel() * 8)
+    bytes_moved = float(d.numel() * 8 * 2 + n_img * (256 * 192 * 8 * 2 + 256 * 256 * 8 * 2))
+    peak_hbm, hbm_src = hbm_peak()
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        from oracle import motion
+        t0 = time.perf_counter()
+        per_ref, _ = motion.estimate(oracle.OracleParams(**kw), distinct.astype(np.complex128), 0)
+        dt = time.perf_counter() - t0
+        cpu = {"value": 4 / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
+               "sample": "the 4 distinct frames x 22 slices (oracle/motion.py, numpy.fft fp64), %.1f s" % dt,
+               "parity_max_shift_err_px": float(np.abs(per[:4, :, :2] - per_ref[:, :, :2]).max())}
+    print(json.dumps({
+        "metric": "motion-estimated frames/s (300-frame ensemble, 22 slices per frame)", "value": n_frames / (ms * 1e-3), "unit": "frames/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32 (hand-written radix-2 FFTs)",
+        "data": "synthetic: synth.moving_speckle, 4 distinct frames with programmed sub-pixel shifts tiled over 300 frames",
+        "config": {"workload": "SURVEY 8(f) NEXT-3 on BASELINE configs[2] shapes: 300 frames x 22 slices of 180x164 px, 256x256 transforms",
+                   "l2_policy": "inputs (%.2f GB) and the transform scratch (6 GB) larger than L2, no flush" % (d.numel() * 8 / 1e9), "plan": info},
+        "kernels_ms": {"all_six_kernels": k_ms},
+        "roofline": {"bound": "hbm", "achieved": bytes_min / (k_ms * 1e-3) / 1e9, "peak": peak_hbm, "unit": "GB/s",
+                     "frac": bytes_min / (k_ms * 1e-3) / 1e9 / peak_hbm, "traffic": None,
+                     "kernel": "motion_stats / fwd_z / lat / peak kernels (whole call)", "kernel_ms": k_ms,
+                     "algorithmic_bytes": bytes_min, "bytes_moved_by_design": bytes_moved,
+                     "frac_on_bytes_moved": bytes_moved / (k_ms * 1e-3) / 1e9 / peak_hbm, "fft_flop": fft_flop,
+                     "fft_tflops": fft_flop / (k_ms * 1e-3) / 1e12, "peak_source": hbm_src},
+        "cpu_baseline": cpu, "clocks": clocks,
+        "e2e": {"value": n_frames / (e2e_ms * 1e-3), "unit": "frames/s", "h2d_bytes_per_step": int(d.numel() * 8),
+                "d2h_bytes_per_step": int(n_frames * 16), "ms_per_step": e2e_ms, "steps": 2},
+        "gpu_launches": int(info["launches_last_call"]) * args.steps}))
+
+
 def run_volume(args):
     """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
     180 x 180 x 164 volume by unpack_frame_kernel + das_volume_kernel (one frame); reported as volumes/s next to the
@@ -649,7 +730,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
-    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter"],
+    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter", "motion"],
                     help="beamform = the BASELINE metric (Stage 1); stage2 = SURVEY 8(f) NEXT-1 on config 2's shapes")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
                     help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
@@ -678,6 +759,8 @@ def main():
         run_stage2(args)
     elif args.workload == "clutter":
         run_clutter(args)
+    elif args.workload == "motion":
+        run_motion(args)
     elif args.config == 4:
         run_volume(args)
     else:

@@ -106,7 +106,8 @@ typedef struct {
                                    (P = 8; needs identical axial grids); 0 = not prepared           */
     int32_t clutter_frames;     /* n_t > 0: also prepare ulm_rca_clutter_filter for ensembles of up to n_t frames
                                    (32 .. 320; sizes the bf16 operand planes: ~8 bytes per slice value); 0 = not    */
-    int32_t reserved[1];        /* must be 0                                                           */
+    int32_t motion_frames;      /* > 0: also prepare ulm_rca_motion_estimate for calls of up to this many frames
+                                   (scratch: ~20 MB per frame at the paper's slice sizes); 0 = not prepared        */
 } ulm_rca_options;
 
 /*
@@ -252,6 +253,31 @@ ulm_rca_status ulm_rca_clutter_filter(const ulm_rca_plan *plan, const void *d_sl
 /* Device time of the five kernels of the last ulm_rca_clutter_filter call: ms5[0] bf16 split, [1] Gram (tcgen05),
  * [2] assembly of C, [3] eigen-subspace, [4] projection.  Waits for the events.  Unavailable with options.no_timing. */
 ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms5);
+
+/*
+ * Rigid motion estimation on the Stage-1 slices by Fourier-domain normalised cross-correlation ("each
+ * frame is transformed into the Fourier domain, the correlation function between the two frames is computed, and the
+ * displacement versus the reference frame is determined by locating the subpixel peak of the correlation function.  This
+ * procedure requires two forward and one inverse Fourier transform"; "the K RC slices and K CR slices were used
+ * separately to estimate motion within the x-z plane and the y-z plane.  K displacement vectors ... were first averaged,
+ * and then the RC- and CR-averaged motions were vector-summed").  Reading: per slice, the B-mode
+ * image |S| with its mean removed is zero-padded to the next powers of two; c(d) = IFFT2(FFT2(a_f) conj(FFT2(a_ref))) /
+ * (|a_f| |a_ref|); the integer argmax (first in row-major order, signed) is refined by a 3-point parabola per axis; a
+ * frame whose content moved by +s pixels relative to the reference gives +s.  Per frame the lateral / axial shifts are
+ * averaged over the row-tx events (-> dx, dz) and the column-tx events (-> dy, dz) and scaled by the grid steps; the two
+ * axial estimates are averaged (a literal vector sum would count the axial motion twice).
+ *   d_slices    : complex fp32 [frame][event][lat][ax] (compound == 0 layout), device memory
+ *   ref_frame   : index of the reference frame inside this call
+ *   d_motion    : float4 [frame] = (dx, dy, dz in metres, mean NCC peak), device memory
+ *   d_per_event : NULL, or float4 [frame][event] = (lateral shift in pixels, axial shift in pixels, NCC peak, 0)
+ * Needs options.motion_frames >= n_frames and slices of at most 512 pixels along each axis.  Enqueues six kernels on
+ * cuda_stream (hand-written radix-2 FFTs; no library FFT), never synchronises; one call in flight per plan.
+ */
+ulm_rca_status ulm_rca_motion_estimate(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames, int32_t ref_frame,
+                                       void *d_motion, void *d_per_event, void *cuda_stream);
+
+/* Device time (ms) of the six kernels of the last ulm_rca_motion_estimate call.  Unavailable with options.no_timing. */
+ulm_rca_status ulm_rca_motion_timing(const ulm_rca_plan *plan, double *ms);
 
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets

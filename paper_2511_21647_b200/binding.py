@@ -22,7 +22,7 @@ _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
            "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
            "ulm_rca_stage2_project", "ulm_rca_stage2_sizes", "ulm_rca_stage2_timing",
-           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing",
+           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing", "ulm_rca_motion_estimate", "ulm_rca_motion_timing",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -47,7 +47,7 @@ class Options(C.Structure):
                 ("t_start_s", C.c_float), ("t0_s", C.POINTER(C.c_float)), ("f_number", C.c_float),
                 ("elem_window", C.POINTER(C.c_float)), ("demod_taps", C.c_int32), ("compound", C.c_int32),
                 ("max_frames", C.c_int32), ("build_volume", C.c_int32), ("kernel", C.c_int32),
-                ("precision", C.c_int32), ("no_timing", C.c_int32), ("stage2_block", C.c_int32), ("clutter_frames", C.c_int32), ("reserved", C.c_int32 * 1)]
+                ("precision", C.c_int32), ("no_timing", C.c_int32), ("stage2_block", C.c_int32), ("clutter_frames", C.c_int32), ("motion_frames", C.c_int32)]
 
 
 def library_path() -> str:
@@ -90,6 +90,10 @@ def load() -> C.CDLL:
     lib.ulm_rca_clutter_filter.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp]
     lib.ulm_rca_clutter_timing.restype = C.c_int
     lib.ulm_rca_clutter_timing.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.ulm_rca_motion_estimate.restype = C.c_int
+    lib.ulm_rca_motion_estimate.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+    lib.ulm_rca_motion_timing.restype = C.c_int
+    lib.ulm_rca_motion_timing.argtypes = [vp, C.POINTER(C.c_double)]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_ring_probe.restype = C.c_int
@@ -136,7 +140,8 @@ class Plan:
                  t_start: float = 0.0, t0: Optional[Sequence[float]] = None, f_number: float = 0.0,
                  elem_window: Optional[Sequence[float]] = None, demod_taps: int = 0, compound: int = 1,
                  max_frames: int = 0, build_volume: bool = False, kernel: int = 0, precision: int = 0,
-                 no_timing: bool = False, stage2_block: int = 0, clutter_frames: int = 0):
+                 no_timing: bool = False, stage2_block: int = 0, clutter_frames: int = 0,
+                 motion_frames: int = 0):
         lib = load()
         self._h = C.c_void_p()
         geo = Geometry(n_rows, n_cols, pitch)
@@ -150,7 +155,7 @@ class Plan:
             raise ValueError("elem_window must have n_cols + n_rows entries")
         opt = Options(int(input_kind), int(channels_per_event or 0), int(n_samples), float(t_start), tp,
                       float(f_number), wp, int(demod_taps), int(compound), int(max_frames),
-                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0, int(stage2_block), int(clutter_frames))
+                      1 if build_volume else 0, int(kernel), int(precision), 1 if no_timing else 0, int(stage2_block), int(clutter_frames), int(motion_frames))
         gx, gy = Grid(*grid_xz), Grid(*grid_yz)
         _check(lib.ulm_rca_plan_create(C.byref(geo), rp, len(row_tx_angles), cp, len(col_tx_angles),
                                        float(c), float(fs), float(fc), C.byref(gx), C.byref(gy), C.byref(opt),
@@ -165,6 +170,7 @@ class Plan:
         import torch
         self.device_index = torch.cuda.current_device()      # the plan belongs to the device current at creation
         self.clutter_frames = int(clutter_frames)
+        self.motion_frames = int(motion_frames)
         self.n_events = len(row_tx_angles) + len(col_tx_angles)
         self.slices_complex_per_frame = (len(row_tx_angles) * grid_xz[0] * grid_xz[3] + len(col_tx_angles) * grid_yz[0] * grid_yz[3])
         self.stage2_block = int(stage2_block)
@@ -303,6 +309,28 @@ class Plan:
         if want_eigenvalues or want_covariance:
             return out, lam, cov
         return out
+
+    def motion_estimate(self, slices, ref_frame: int = 0, stream=None):
+        """Fourier-domain NCC motion estimation (ulm_rca_motion_estimate).  Returns (motion float32 [frame][4] = dx, dy, dz
+        in metres and mean NCC; per_event float32 [frame][event][4] = lateral px, axial px, NCC, 0) as CUDA tensors."""
+        import torch
+        if not self.motion_frames:
+            raise ValueError("the plan was created without motion_frames")
+        if not (slices.is_cuda and slices.dtype == torch.complex64 and slices.is_contiguous()
+                and slices.device.index == self.device_index and slices.dim() == 2
+                and slices.shape[1] == self.slices_complex_per_frame):
+            raise ValueError("slices must be a contiguous complex64 CUDA tensor [frame][%d] on the plan's device" % self.slices_complex_per_frame)
+        n = int(slices.shape[0])
+        motion = torch.empty((n, 4), dtype=torch.float32, device=slices.device)
+        per = torch.empty((n, self.n_events, 4), dtype=torch.float32, device=slices.device)
+        _check(load().ulm_rca_motion_estimate(self._h, C.c_void_p(slices.data_ptr()), n, int(ref_frame), C.c_void_p(motion.data_ptr()),
+                                              C.c_void_p(per.data_ptr()), self._stream_ptr(stream)))
+        return motion, per
+
+    def motion_timing(self) -> float:
+        v = C.c_double()
+        _check(load().ulm_rca_motion_timing(self._h, C.byref(v)))
+        return float(v.value)
 
     def clutter_timing(self) -> tuple:
         """(split_ms, gram_ms, assemble_ms, eig_ms, project_ms) of the last clutter_filter() call."""

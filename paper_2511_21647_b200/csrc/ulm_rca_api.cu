@@ -17,6 +17,7 @@
 #include "ulm_rca_ring_host.cuh"
 #include "ulm_rca_stage2_host.cuh"
 #include "ulm_rca_clutter_host.cuh"
+#include "ulm_rca_motion_host.cuh"
 
 namespace {
 
@@ -128,6 +129,7 @@ struct ulm_rca_plan {
     bool timing = true;           // record CUDA events around the kernels (options.no_timing = 0)
     ulm::Stage2Plan s2;           // Stage 2 + sum-projection tables (options.stage2_block > 0)
     mutable ulm::ClutterPlan cf;  // clutter filter scratch (options.clutter_frames > 0)
+    ulm::MotionPlan mo;           // motion estimation scratch (options.motion_frames > 0)
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -493,7 +495,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
     if (!finite_pos(c_mps) || !finite_pos(fs_hz) || !finite_pos(fc_hz)) return fail(ULM_RCA_EINVAL, "c, fs, fc must be finite and > 0");
     if (ulm_rca_status s = check_grid(grid_xz, "grid_xz")) return s;
     if (ulm_rca_status s = check_grid(grid_yz, "grid_yz")) return s;
-    if (opt->reserved[0]) return fail(ULM_RCA_EINVAL, "options.reserved must be 0");
+    if (opt->motion_frames < 0 || opt->motion_frames > 65535) return fail(ULM_RCA_EINVAL, "motion_frames must be 0 .. 65535");
     if (opt->clutter_frames != 0 && (opt->clutter_frames < ulm::kCfB || opt->clutter_frames > ulm::kCfMaxFrames))
         return fail(ULM_RCA_EINVAL, "clutter_frames must be 0 or %d .. %d", ulm::kCfB, ulm::kCfMaxFrames);
     if (opt->stage2_block < 0 || opt->stage2_block > 4096) return fail(ULM_RCA_EINVAL, "stage2_block must be 0 .. 4096");
@@ -693,6 +695,22 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
             const cudaError_t e = cudaGetLastError();
             if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "clutter filter: %s: %s", why, cudaGetErrorString(e));
             return fail(ULM_RCA_EUNSUPPORTED, "clutter filter: %s", why);
+        }
+    }
+    if (opt->motion_frames > 0) {
+        std::vector<long long> off;
+        std::vector<int> nl, nz;
+        long long o = 0;
+        for (int a = 0; a < 2; ++a)
+            for (int k = 0; k < P.ap[a].n_tx; ++k) {
+                off.push_back(o); nl.push_back(P.ap[a].g.n_lat); nz.push_back(P.ap[a].g.n_ax);
+                o += (long long)P.ap[a].g.n_lat * P.ap[a].g.n_ax;
+            }
+        const float dl[2] = {(float)P.ap[0].g.dlat, (float)P.ap[1].g.dlat}, dzz[2] = {(float)P.ap[0].g.dz, (float)P.ap[1].g.dz};
+        if (const char *why = ulm::motion_build(P.mo, off, nl, nz, P.ap[0].n_tx, o, opt->motion_frames, dl, dzz, P.timing)) {
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ULM_RCA_ENOMEM : ULM_RCA_ECUDA, "motion estimation: %s: %s", why, cudaGetErrorString(e));
+            return fail(ULM_RCA_EUNSUPPORTED, "motion estimation: %s", why);
         }
     }
     CUDA_TRY(cudaDeviceSynchronize());
@@ -999,6 +1017,32 @@ ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms4) {
         CUDA_TRY(cudaEventElapsedTime(&v, plan->cf.ev[i], plan->cf.ev[i + 1]));
         ms5[i] = v;
     }
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_motion_estimate(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames, int32_t ref_frame,
+                                       void *d_motion, void *d_per_event, void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->mo.ready) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without motion_frames");
+    if (n_frames < 0 || n_frames > plan->mo.max_frames) return fail(ULM_RCA_EINVAL, "n_frames must be 0 .. motion_frames (%d)", plan->mo.max_frames);
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (ref_frame < 0 || ref_frame >= n_frames) return fail(ULM_RCA_EINVAL, "ref_frame must be a frame of this call");
+    if (!d_slices || !d_motion) return fail(ULM_RCA_EINVAL, "device pointer is NULL");
+    if (ulm_rca_status s = check_device(*plan)) return s;
+    int launches = 0;
+    CUDA_TRY(ulm::motion_launch(plan->mo, static_cast<const float2 *>(d_slices), n_frames, ref_frame, static_cast<float4 *>(d_motion),
+                                static_cast<float4 *>(d_per_event), (cudaStream_t)cuda_stream, &launches));
+    plan->last_launches = launches;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_motion_timing(const ulm_rca_plan *plan, double *ms) {
+    if (!plan || !ms) return fail(ULM_RCA_EINVAL, "plan / ms is NULL");
+    if (!plan->mo.ready || !plan->mo.ev[0]) return fail(ULM_RCA_EUNSUPPORTED, "no motion-estimation timing events on this plan");
+    float v = 0;
+    CUDA_TRY(cudaEventSynchronize(plan->mo.ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(&v, plan->mo.ev[0], plan->mo.ev[1]));
+    *ms = v;
     return ULM_RCA_OK;
 }
 

@@ -192,3 +192,26 @@ def clutter_ensemble(n_t: int, n_pix_per_event, seed: int, tissue_rank: int = 3,
             x = x + gain * drift * speckle[None, :]
         blocks.append(x)
     return np.concatenate(blocks, axis=1).astype(np.complex64)
+
+
+def moving_speckle(n_frames: int, shapes, shifts, seed: int, correlation_px: float = 3.0, noise: float = 0.02) -> np.ndarray:
+    """Seeded complex64 slices [n_frames][sum of n_lat * n_ax over `shapes`] whose B-mode images are one smooth random
+    speckle field per event, displaced in frame f by shifts[f] = (lateral px, axial px) (sub-pixel displacement by the
+    Fourier shift theorem on a larger canvas, then cropped) plus a little independent noise: stand-in for the slices of a
+    slowly moving organ."""
+    rng = _rng(seed, 17)
+    out = []
+    for (nl, nz) in shapes:
+        m1, m2 = 2 * nl + 32, 2 * nz + 32
+        k1, k2 = np.fft.fftfreq(m1)[:, None], np.fft.fftfreq(m2)[None, :]
+        spec = np.fft.fft2(rng.standard_normal((m1, m2)) + 1j * rng.standard_normal((m1, m2)))
+        spec *= np.exp(-2.0 * (np.pi * correlation_px) ** 2 * (k1 ** 2 + k2 ** 2))          # Gaussian low-pass
+        frames = []
+        for f in range(n_frames):
+            s1, s2 = shifts[f]
+            img = np.fft.ifft2(spec * np.exp(-2j * np.pi * (k1 * s1 + k2 * s2)))
+            crop = img[nl // 2 + 8:nl // 2 + 8 + nl, nz // 2 + 8:nz // 2 + 8 + nz]
+            crop = crop / np.abs(crop).max() + noise * (rng.standard_normal((nl, nz)) + 1j * rng.standard_normal((nl, nz)))
+            frames.append(crop.reshape(-1))
+        out.append(np.stack(frames))
+    return np.concatenate(out, axis=1).astype(np.complex64)

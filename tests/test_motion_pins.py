@@ -80,20 +80,22 @@ def test_combination_rule_by_hand():
     import synth
     from synth import centred_grid
     d = synth.LAMBDA_M / 2
-    cfg = synth.config(0).with_(compound=0, grid_xz=centred_grid(20, 2 * d, 24, 6e-3, d), grid_yz=centred_grid(18, 3 * d, 24, 6e-3, d),
+    cfg = synth.config(0).with_(compound=0, grid_xz=centred_grid(50, 2 * d, 56, 6e-3, d), grid_yz=centred_grid(48, 3 * d, 56, 6e-3, d),
                                 row_tx_angles=(0.0, 0.1), col_tx_angles=(0.05,))
     p = oracle.OracleParams(**cfg.plan_kwargs())
-    ref_xz = blob_image(20, 24, [(9, 11, 1.0), (13, 15, 0.6)])
-    ref_yz = blob_image(18, 24, [(8, 10, 1.0), (11, 16, 0.6)])
-    f1_xz_a = blob_image(20, 24, [(9 + 1, 11 + 2, 1.0), (13 + 1, 15 + 2, 0.6)])       # event 0: (+1, +2)
-    f1_xz_b = blob_image(20, 24, [(9 + 3, 11 + 2, 1.0), (13 + 3, 15 + 2, 0.6)])       # event 1: (+3, +2)
-    f1_yz = blob_image(18, 24, [(8 - 2, 10 + 4, 1.0), (11 - 2, 16 + 4, 0.6)])         # event 2: (-2, +4)
+    bx = [(20, 22, 1.0), (30, 30, 0.6), (24, 34, -0.9), (32, 20, -0.7)]             # zero-mean content, well inside
+    by = [(19, 21, 1.0), (28, 31, 0.6), (23, 35, -0.9), (30, 22, -0.7)]
+    mv = lambda b, s: [(x + s[0], z + s[1], a) for (x, z, a) in b]
+    ref_xz, ref_yz = blob_image(50, 56, bx) + 2.0, blob_image(48, 56, by) + 2.0     # + 2: a positive B-mode image
+    f1_xz_a = blob_image(50, 56, mv(bx, (1, 2))) + 2.0                              # event 0: (+1, +2)
+    f1_xz_b = blob_image(50, 56, mv(bx, (3, 2))) + 2.0                              # event 1: (+3, +2)
+    f1_yz = blob_image(48, 56, mv(by, (-2, 4))) + 2.0                               # event 2: (-2, +4)
     frames = np.stack([np.concatenate([ref_xz.ravel(), ref_xz.ravel(), ref_yz.ravel()]),
                        np.concatenate([f1_xz_a.ravel(), f1_xz_b.ravel(), f1_yz.ravel()])]).astype(complex) * np.exp(0.7j)
     per, mot = motion.estimate(p, frames)
     assert np.abs(per[0, :, :2]).max() < 1e-9 and np.abs(per[0, :, 2] - 1).max() < 1e-12
-    np.testing.assert_allclose(per[1, :, :2], [[1, 2], [3, 2], [-2, 4]], atol=5e-3)
+    np.testing.assert_allclose(per[1, :, :2], [[1, 2], [3, 2], [-2, 4]], atol=1e-5)
     dx, dy, dz, ncc = mot[1]
-    assert abs(dx - 2.0 * 2 * d) < 1e-2 * d and abs(dy - (-2.0) * 3 * d) < 1e-2 * d      # means (1 + 3)/2 and -2, times the lateral steps
-    assert abs(dz - 0.5 * (2.0 + 4.0) * d) < 1e-2 * d                                    # axial: mean of the RC and CR estimates
+    assert abs(dx - 2.0 * 2 * d) < 1e-4 * d and abs(dy - (-2.0) * 3 * d) < 1e-4 * d      # means (1 + 3)/2 and -2, times the lateral steps
+    assert abs(dz - 0.5 * (2.0 + 4.0) * d) < 1e-4 * d                                    # axial: mean of the RC and CR estimates
     assert 0.9 < ncc <= 1.0
