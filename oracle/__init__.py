@@ -18,3 +18,4 @@ from .oracle import (  # noqa: F401
 from . import stage2  # noqa: F401,E402
 from . import clutter  # noqa: F401,E402
 from . import motion  # noqa: F401,E402
+from . import localize  # noqa: F401,E402
