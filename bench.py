@@ -593,6 +593,74 @@ def run_motion(args):
         "gpu_launches": int(info["launches_last_call"]) * args.steps}))
 
 
+def run_localize(args):
+    """NEXT-4: separable sub-pixel 2-D NCC localization on the projected planes of a
+    300-frame ensemble of config 2's shape: 23 + 23 planes of 180 x 164 px per frame (3.26 GB of planes, resident in HBM);
+    one step = ulm_rca_localize over the whole ensemble."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build, fp32_peak_tflops
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(2).with_(compound=0)
+    kw = rounded_kwargs(cfg)
+    n_frames, sig = cfg.n_frames, (1.8, 1.4)
+    distinct = synth.bubble_planes(3, 23, 180, 23, 180, 164, seed=6, bubbles_per_plane=5, sigma=sig)
+    idx = torch.arange(n_frames, device="cuda") % 3
+    d = torch.from_numpy(distinct).cuda()[idx].contiguous()
+    warmup = max(args.warmup, 3)
+    with Plan(**kw, stage2_block=8, max_frames=n_frames) as plan:
+        for _ in range(warmup):
+            loc, count = plan.localize(d, sig[0], sig[1], 0.2, 0.7, 16)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        stream = torch.cuda.current_stream()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(args.steps):
+            loc, count = plan.localize(d, sig[0], sig[1], 0.2, 0.7, 16)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        ms = ev0.elapsed_time(ev1) / args.steps            # includes the allocation / clearing of the result tensors
+        info = plan.info()
+        h_in = torch.empty(d.shape, dtype=torch.complex64, pin_memory=True)
+        h_in.copy_(d)
+        d_in = torch.empty_like(d)
+        t0 = time.perf_counter()
+        for _ in range(2):
+            d_in.copy_(h_in, non_blocking=True)
+            l2, c2 = plan.localize(d_in, sig[0], sig[1], 0.2, 0.7, 16)
+            l_host, c_host = l2.cpu(), c2.cpu()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / 2
+        loc, count = loc.cpu().numpy(), count.cpu().numpy()
+    byts = float(d.numel() * 8 * 2)                        # planes read twice: frame maximum, then the NCC kernel
+    peak_hbm, hbm_src = hbm_peak()
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import localize
+        t0 = time.perf_counter()
+        ref = localize.localize_frame(distinct[0].astype(np.complex128), 23, 180, 23, 180, 164, sig[0], sig[1], 0.2, 0.7)
+        dt = time.perf_counter() - t0
+        ok = all(count[0, pl] == len(r) for pl, r in enumerate(ref))
+        cpu = {"value": 1 / dt, "unit": "frames/s", "cores": 1, "kind": "oracle",
+               "sample": "1 frame = 46 planes (oracle/localize.py, numpy fp64), %.1f s" % dt, "counts_agree": bool(ok)}
+    print(json.dumps({
+        "metric": "localized frames/s (300-frame ensemble, 46 projected planes per frame)", "value": n_frames / (ms * 1e-3), "unit": "frames/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic: synth.bubble_planes, 3 distinct frames tiled over 300 frames",
+        "config": {"workload": "SURVEY 8(f) NEXT-4 on BASELINE configs[2] shapes: 300 frames x 46 planes of 180x164 px, 11-tap separable NCC",
+                   "l2_policy": "inputs (%.2f GB) larger than L2, no flush" % (d.numel() * 8 / 1e9), "plan": info},
+        "localizations_per_frame": float(count.sum()) / n_frames,
+        "roofline": {"bound": "hbm", "achieved": byts / (ms * 1e-3) / 1e9, "peak": peak_hbm, "unit": "GB/s",
+                     "frac": byts / (ms * 1e-3) / 1e9 / peak_hbm, "traffic": None, "kernel": "localize_max_kernel + localize_kernel (whole call)",
+                     "algorithmic_bytes": byts, "peak_source": hbm_src},
+        "cpu_baseline": cpu, "clocks": clocks,
+        "e2e": {"value": n_frames / (e2e_ms * 1e-3), "unit": "frames/s", "h2d_bytes_per_step": int(d.numel() * 8),
+                "d2h_bytes_per_step": int(loc.size * 4 + count.size * 4), "ms_per_step": e2e_ms, "steps": 2},
+        "gpu_launches": int(info["launches_last_call"]) * args.steps}))
+
+
 def run_volume(args):
     """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
     180 x 180 x 164 volume by unpack_frame_kernel + das_volume_kernel (one frame); reported as volumes/s next to the
@@ -730,7 +798,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
-    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter", "motion"],
+    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter", "motion", "localize"],
                     help="beamform = the BASELINE metric (Stage 1); stage2 = SURVEY 8(f) NEXT-1 on config 2's shapes")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
                     help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
@@ -761,6 +829,8 @@ def main():
         run_clutter(args)
     elif args.workload == "motion":
         run_motion(args)
+    elif args.workload == "localize":
+        run_localize(args)
     elif args.config == 4:
         run_volume(args)
     else:

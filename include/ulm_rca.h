@@ -279,6 +279,35 @@ ulm_rca_status ulm_rca_motion_estimate(const ulm_rca_plan *plan, const void *d_s
 /* Device time (ms) of the six kernels of the last ulm_rca_motion_estimate call.  Unavailable with options.no_timing. */
 ulm_rca_status ulm_rca_motion_timing(const ulm_rca_plan *plan, double *ms);
 
+/* Parameters of ulm_rca_localize (none of them is given by the paper; PAPER.md:117 fixes only the 11-tap kernels). */
+typedef struct {
+    float sigma_lat_px, sigma_ax_px;   /* widths of the Gaussian-fitted PSF template along the lateral axis / depth, pixels  */
+    float threshold_rel;               /* intensity threshold as a fraction of the frame's maximum |V|                         */
+    float ncc_min;                     /* smallest NCC value of a localization                                                */
+    int32_t capacity;                  /* localizations stored per plane at most                                               */
+} ulm_rca_localize_params;
+
+/*
+ * Microbubble localization on the projected planes by separable sub-pixel 2-D normalised cross-correlation
+ * ("the two projections are first normalized cross-correlated with the corresponding Gaussian-fitted 2D
+ * PSFs ... sub-pixel regional peaks in the resulting correlating map are identified as localizations ... the 2D operation
+ * was further decomposed into successive 1D correlations along each dimension"; 11-tap 1-D kernels;
+ * "the maximum intensity of each volume was obtained ... for thresholding").  Reading:
+ *   B = |V_p| of a plane (0 outside), g(a, b) = exp(-a^2 / 2 s_lat^2) exp(-b^2 / 2 s_ax^2), a, b = -5 .. 5;
+ *   ncc(p) = sum_W (B - Bm)(g - gm) / sqrt(sum_W (B - Bm)^2 sum_W (g - gm)^2) over the 11 x 11 window W around p;
+ *   a localization = an interior pixel with B >= threshold_rel * max over the frame's planes of B and ncc >= ncc_min
+ *   whose ncc exceeds the 4 neighbours that follow it in row-major order and is not below the 4 that precede it, refined
+ *   by a 3-point parabola of the NCC map along each axis.
+ *   d_planes : complex fp32, the output layout of ulm_rca_stage2_project, n_frames frames, device memory
+ *   d_loc    : float4 [frame][plane][capacity] = (lateral position, depth position in pixels, ncc, B), device memory;
+ *              the order of the localizations of a plane is not fixed (atomic append), the set is
+ *   d_count  : int32 [frame][plane] number of localizations found (if > capacity the surplus was dropped)
+ * Needs options.stage2_block (the planes' geometry).  Enqueues two kernels per batch of max_frames frames; one call in
+ * flight per plan.
+ */
+ulm_rca_status ulm_rca_localize(const ulm_rca_plan *plan, const void *d_planes, int32_t n_frames,
+                                const ulm_rca_localize_params *params, void *d_loc, void *d_count, void *cuda_stream);
+
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets
  * `t0_s` (NULL = 0), image grid `grid`.  Returns the number of tiles in *n_tiles, the stage length in entries in

@@ -22,7 +22,7 @@ _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
            "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
            "ulm_rca_stage2_project", "ulm_rca_stage2_sizes", "ulm_rca_stage2_timing",
-           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing", "ulm_rca_motion_estimate", "ulm_rca_motion_timing",
+           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing", "ulm_rca_motion_estimate", "ulm_rca_motion_timing", "ulm_rca_localize",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -40,6 +40,11 @@ class Geometry(C.Structure):
 class Grid(C.Structure):
     _fields_ = [("n_lat", C.c_int32), ("lat0_m", C.c_float), ("dlat_m", C.c_float),
                 ("n_ax", C.c_int32), ("z0_m", C.c_float), ("dz_m", C.c_float), ("ref_m", C.c_float)]
+
+
+class LocalizeParams(C.Structure):
+    _fields_ = [("sigma_lat_px", C.c_float), ("sigma_ax_px", C.c_float), ("threshold_rel", C.c_float), ("ncc_min", C.c_float),
+                ("capacity", C.c_int32)]
 
 
 class Options(C.Structure):
@@ -94,6 +99,8 @@ def load() -> C.CDLL:
     lib.ulm_rca_motion_estimate.argtypes = [vp, vp, i32, i32, vp, vp, vp]
     lib.ulm_rca_motion_timing.restype = C.c_int
     lib.ulm_rca_motion_timing.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.ulm_rca_localize.restype = C.c_int
+    lib.ulm_rca_localize.argtypes = [vp, vp, i32, C.POINTER(LocalizeParams), vp, vp, vp]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_ring_probe.restype = C.c_int
@@ -309,6 +316,25 @@ class Plan:
         if want_eigenvalues or want_covariance:
             return out, lam, cov
         return out
+
+    def localize(self, planes, sigma_lat_px: float, sigma_ax_px: float, threshold_rel: float, ncc_min: float, capacity: int = 64,
+                 stream=None):
+        """Separable 2-D NCC localization (ulm_rca_localize) on complex64 CUDA planes [frame][stage2 output].  Returns
+        (loc float32 [frame][plane][capacity][4], count int32 [frame][plane]) as CUDA tensors."""
+        import torch
+        if not self.stage2_block:
+            raise ValueError("the plan was created without stage2_block")
+        if not (planes.is_cuda and planes.dtype == torch.complex64 and planes.is_contiguous() and planes.device.index == self.device_index
+                and planes.dim() == 2 and planes.shape[1] * 8 == self.planes_bytes_per_frame):
+            raise ValueError("planes must be a contiguous complex64 CUDA tensor [frame][%d]" % (self.planes_bytes_per_frame // 8))
+        n = int(planes.shape[0])
+        n_pl = self.n_planes_xz + self.n_planes_yz
+        loc = torch.zeros((n, n_pl, int(capacity), 4), dtype=torch.float32, device=planes.device)
+        count = torch.zeros((n, n_pl), dtype=torch.int32, device=planes.device)
+        prm = LocalizeParams(float(sigma_lat_px), float(sigma_ax_px), float(threshold_rel), float(ncc_min), int(capacity))
+        _check(load().ulm_rca_localize(self._h, C.c_void_p(planes.data_ptr()), n, C.byref(prm), C.c_void_p(loc.data_ptr()),
+                                       C.c_void_p(count.data_ptr()), self._stream_ptr(stream)))
+        return loc, count
 
     def motion_estimate(self, slices, ref_frame: int = 0, stream=None):
         """Fourier-domain NCC motion estimation (ulm_rca_motion_estimate).  Returns (motion float32 [frame][4] = dx, dy, dz

@@ -18,6 +18,7 @@
 #include "ulm_rca_stage2_host.cuh"
 #include "ulm_rca_clutter_host.cuh"
 #include "ulm_rca_motion_host.cuh"
+#include "ulm_rca_localize.cuh"
 
 namespace {
 
@@ -130,6 +131,7 @@ struct ulm_rca_plan {
     ulm::Stage2Plan s2;           // Stage 2 + sum-projection tables (options.stage2_block > 0)
     mutable ulm::ClutterPlan cf;  // clutter filter scratch (options.clutter_frames > 0)
     ulm::MotionPlan mo;           // motion estimation scratch (options.motion_frames > 0)
+    DeviceBuf loc_frame_max;      // per-frame maximum |V| for ulm_rca_localize (with stage2_block)
     // CUDA events around the kernels of the last kTimedCalls calls (per batch: before demod, after demod,
     // after DAS; the first kTimedBatches batches of a call)
     static constexpr int kTimedCalls = 64, kTimedBatches = 4;
@@ -681,6 +683,10 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
             return fail(ULM_RCA_EUNSUPPORTED, "stage 2: %s", why);
         }
     }
+    if (P.s2.ready) {
+        CUDA_TRY(cudaMalloc(&P.loc_frame_max.p, (size_t)P.max_frames * sizeof(unsigned int)));
+        CUDA_TRY(cudaFuncSetAttribute(ulm::localize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ulm::kLoSmem));
+    }
     if (opt->clutter_frames > 0) {
         std::vector<long long> off;
         std::vector<int> npix;
@@ -1043,6 +1049,57 @@ ulm_rca_status ulm_rca_motion_timing(const ulm_rca_plan *plan, double *ms) {
     CUDA_TRY(cudaEventSynchronize(plan->mo.ev[1]));
     CUDA_TRY(cudaEventElapsedTime(&v, plan->mo.ev[0], plan->mo.ev[1]));
     *ms = v;
+    return ULM_RCA_OK;
+}
+
+ulm_rca_status ulm_rca_localize(const ulm_rca_plan *plan, const void *d_planes, int32_t n_frames,
+                                const ulm_rca_localize_params *prm, void *d_loc, void *d_count, void *cuda_stream) {
+    if (!plan) return fail(ULM_RCA_EINVAL, "plan is NULL");
+    if (!plan->s2.ready) return fail(ULM_RCA_EUNSUPPORTED, "plan was created without stage2_block (the planes' geometry)");
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!d_planes || !prm || !d_loc || !d_count) return fail(ULM_RCA_EINVAL, "pointer is NULL");
+    if (!(prm->sigma_lat_px > 0) || !(prm->sigma_ax_px > 0) || !std::isfinite(prm->sigma_lat_px) || !std::isfinite(prm->sigma_ax_px) ||
+        !std::isfinite(prm->threshold_rel) || !std::isfinite(prm->ncc_min) || prm->capacity < 1)
+        return fail(ULM_RCA_EINVAL, "localize parameters invalid");
+    if (ulm_rca_status s = check_device(*plan)) return s;
+    const ulm::Stage2Plan &S = plan->s2;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    ulm::LoParams L{};
+    L.planes_per_frame = S.planes_per_frame; L.n_z = S.n_z;
+    for (int a = 0; a < 2; ++a) { L.n_planes[a] = S.n_g[a]; L.n_lat[a] = S.n_lat[a]; }
+    L.set_off[0] = 0; L.set_off[1] = (long long)S.n_g[0] * S.n_lat[0] * S.n_z;
+    double gm = 0, g1[ulm::kLoTaps], g2[ulm::kLoTaps];
+    for (int k = 0; k < ulm::kLoTaps; ++k) {
+        const double a = k - ulm::kLoHalf;
+        g1[k] = std::exp(-a * a / (2.0 * prm->sigma_lat_px * prm->sigma_lat_px));
+        g2[k] = std::exp(-a * a / (2.0 * prm->sigma_ax_px * prm->sigma_ax_px));
+        L.g1[k] = (float)g1[k]; L.g2[k] = (float)g2[k];
+    }
+    for (int i = 0; i < ulm::kLoTaps; ++i) for (int j = 0; j < ulm::kLoTaps; ++j) gm += g1[i] * g2[j];
+    gm /= 121.0;
+    double gd = 0;
+    for (int i = 0; i < ulm::kLoTaps; ++i) for (int j = 0; j < ulm::kLoTaps; ++j) gd += (g1[i] * g2[j] - gm) * (g1[i] * g2[j] - gm);
+    L.g_mean = (float)gm; L.g_den = (float)gd;
+    L.threshold_rel = prm->threshold_rel; L.ncc_min = prm->ncc_min; L.capacity = prm->capacity;
+    const int n_pl = S.n_g[0] + S.n_g[1];
+    int launches = 0;
+    for (int f0 = 0; f0 < n_frames; f0 += plan->max_frames) {
+        const int nb = std::min(plan->max_frames, n_frames - f0);
+        L.planes = static_cast<const float2 *>(d_planes) + (long long)f0 * S.planes_per_frame;
+        L.n_frames = nb;
+        L.frame_max = plan->loc_frame_max.as<unsigned int>();
+        L.loc = static_cast<float4 *>(d_loc) + (long long)f0 * n_pl * prm->capacity;
+        L.count = static_cast<int *>(d_count) + (long long)f0 * n_pl;
+        CUDA_TRY(cudaMemsetAsync(L.frame_max, 0, (size_t)nb * sizeof(unsigned int), st));
+        CUDA_TRY(cudaMemsetAsync(L.count, 0, (size_t)nb * n_pl * sizeof(int), st));
+        ulm::localize_max_kernel<<<dim3(64, nb), 256, 0, st>>>(L);
+        const int lat_tiles = (std::max(S.n_lat[0], S.n_lat[1]) + ulm::kLoTl - 1) / ulm::kLoTl, z_tiles = (S.n_z + ulm::kLoTa - 1) / ulm::kLoTa;
+        ulm::localize_kernel<<<dim3(lat_tiles, z_tiles, nb * n_pl), ulm::kLoThreads, ulm::kLoSmem, st>>>(L);
+        CUDA_TRY(cudaGetLastError());
+        launches += 2;
+    }
+    plan->last_launches = launches;
     return ULM_RCA_OK;
 }
 

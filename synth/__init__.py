@@ -5,4 +5,4 @@ echo simulator; it holds none of the beamformer's arithmetic and imports neither
 ``paper_2511_21647_b200``.
 """
 from .configs import RcaConfig, Scene, centred_grid, config, small_config, LAMBDA_M  # noqa: F401
-from .scene import build, clutter_ensemble, moving_speckle, random_channel, random_complex, render, scatterers  # noqa: F401
+from .scene import build, bubble_planes, clutter_ensemble, moving_speckle, random_channel, random_complex, render, scatterers  # noqa: F401

@@ -215,3 +215,32 @@ def moving_speckle(n_frames: int, shapes, shifts, seed: int, correlation_px: flo
             frames.append(crop.reshape(-1))
         out.append(np.stack(frames))
     return np.concatenate(out, axis=1).astype(np.complex64)
+
+
+def bubble_planes(n_frames: int, n_planes_xz: int, nx: int, n_planes_yz: int, ny: int, nz: int, seed: int, bubbles_per_plane: int = 4,
+                  sigma=(1.8, 1.4), noise: float = 0.01) -> np.ndarray:
+    """Seeded complex64 projected planes [n_frames][layout of ulm_rca_stage2_project]: every plane holds a few Gaussian
+    blobs (width `sigma` pixels along lateral / depth, amplitudes 0.3 .. 1, random phase) at random sub-pixel positions at
+    least 9 pixels apart, plus weak complex noise: stand-in for separated microbubble planes."""
+    rng = _rng(seed, 19)
+    out = np.zeros((n_frames, (n_planes_xz * nx + n_planes_yz * ny) * nz), dtype=np.complex64)
+    for f in range(n_frames):
+        off = 0
+        for (n_pl, nl) in ((n_planes_xz, nx), (n_planes_yz, ny)):
+            for _ in range(n_pl):
+                img = noise * (rng.standard_normal((nl, nz)) + 1j * rng.standard_normal((nl, nz)))
+                ll, zz = np.meshgrid(np.arange(nl), np.arange(nz), indexing="ij")
+                placed = []
+                for _b in range(bubbles_per_plane):
+                    for _try in range(50):
+                        c = (rng.uniform(7, nl - 8), rng.uniform(7, nz - 8))
+                        if all((c[0] - q[0]) ** 2 + (c[1] - q[1]) ** 2 >= 81 for q in placed):
+                            placed.append(c)
+                            break
+                    else:
+                        continue
+                    amp = rng.uniform(0.3, 1.0) * np.exp(2j * np.pi * rng.random())
+                    img = img + amp * np.exp(-((ll - c[0]) ** 2) / (2 * sigma[0] ** 2) - ((zz - c[1]) ** 2) / (2 * sigma[1] ** 2))
+                out[f, off:off + nl * nz] = img.reshape(-1)
+                off += nl * nz
+    return out
