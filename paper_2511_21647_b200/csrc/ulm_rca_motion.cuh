@@ -7,9 +7,11 @@
 //   ME-4  per frame: mean over the row-tx events -> (dx, dz_RC), over the column-tx events -> (dy, dz_CR),
 //         motion = (dx, dy, (dz_RC + dz_CR) / 2) in metres
 //
-// The paper uses cuFFT (cufftPlanMany) plus a correlation kernel; here the transforms are hand-written radix-2 FFTs, one
-// warp per line in shared memory, organised so that every pass over global memory is coalesced and the product with
-// the reference spectrum and the inverse lateral transform are fused into the forward lateral pass:
+// The paper uses cuFFT (cufftPlanMany) plus a correlation kernel; here the transforms are hand-written: one warp per
+// line, the whole transform in registers (R-point butterflies per lane, 32-point butterflies across the lanes by
+// shuffles; forward = decimation in frequency, inverse = the same network backwards, so no bit-reversal pass exists),
+// every pass over global memory coalesced, and the product with the reference spectrum and the inverse lateral
+// transform fused into the forward lateral pass:
 //   motion_stats_kernel     mean and mean-removed energy of every B-mode image
 //   motion_fwd_z_kernel     FFT along depth of 32 lateral lines per CTA, written transposed  T1[img][kz][l]
 //   motion_lat_kernel<REF>  FFT along the lateral axis of 32 kz rows per CTA; REF: store the reference spectrum;
@@ -49,26 +51,115 @@ constexpr int kMoMaxN = 512;      // padded FFT length at most
 constexpr int kMoLines = 32;      // lines per CTA of the transposing kernels
 constexpr int kMoThreads = 256;
 
-// In-place radix-2 FFT of n = 2^logn points held BIT-REVERSED in s[] (shared memory) by one warp.
-// tw[k] = exp(-2 pi i k / 1024); INV conjugates the twiddles (no 1/n scaling).
-template <bool INV>
-__device__ __forceinline__ void mo_warp_fft(float2 *s, int logn, const float2 *tw, int lane) {
-    const int n = 1 << logn;
-    for (int lg = 1; lg <= logn; ++lg) {
-        const int half = 1 << (lg - 1), tstep = 1024 >> lg;
-        for (int b = lane; b < n / 2; b += 32) {
-            const int pos = b & (half - 1), i0 = ((b >> (lg - 1)) << lg) + pos, i1 = i0 + half;
-            float2 w = tw[pos * tstep];
-            if (INV) w.y = -w.y;
-            const float2 u = s[i0], v = s[i1];
-            const float2 t = make_float2(w.x * v.x - w.y * v.y, w.x * v.y + w.y * v.x);
-            s[i0] = make_float2(u.x + t.x, u.y + t.y);
-            s[i1] = make_float2(u.x - t.x, u.y - t.y);
+// ------------------------------------------------------------------------------------------------------------------
+// Warp FFT in registers.  N = 32 R points (R = 2^LOGR <= 16): lane m holds x[32 r + m] in v[r] (the layout of a
+// coalesced load).  N = R x 32 Cooley-Tukey:
+//     X[k1 + R k2] = sum_m W_32^{m k2} W_N^{m k1} sum_r x[32 r + m] W_R^{r k1}
+// mo_fft_dif: R-point DIF butterflies in registers, twiddle W_N^{m k1}, 32-point DIF butterflies across the lanes with
+// xor shuffles.  Result in PERMUTED order: register slot q of lane l holds X[brev_R(q) + R brev_5(l)]
+// (mo_perm).  mo_fft_dit runs the same network backwards (DIT butterflies with the conjugate twiddles): it takes the
+// permuted order and returns natural order, x[32 r + m] in v[r] of lane m.  A forward transform, a pointwise product
+// and the inverse therefore never need a bit-reversal pass, and no stage goes through shared memory.
+// SIGN = -1: exponent -2 pi i nk/N (forward); +1: the (unnormalised) inverse.  tw[k] = exp(-2 pi i k / 1024).
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 mo_cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <int SIGN> __device__ __forceinline__ float2 mo_tw(const float2 *tw, int idx) {
+    float2 w = __ldg(tw + idx);
+    if (SIGN > 0) w.y = -w.y;
+    return w;
+}
+// exp(SIGN 2 pi i j / len) for the register butterflies, len <= 16: compile-time constants after unrolling
+template <int SIGN> __device__ __forceinline__ float2 mo_w16(int j16) {
+    constexpr float c[8] = {1.f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f, 0.f, -0.38268343236508977f,
+                            -0.70710678118654752f, -0.92387953251128674f};
+    constexpr float s[8] = {0.f, 0.38268343236508977f, 0.70710678118654752f, 0.92387953251128674f, 1.f, 0.92387953251128674f,
+                            0.70710678118654752f, 0.38268343236508977f};
+    return make_float2(c[j16], SIGN > 0 ? s[j16] : -s[j16]);
+}
+__host__ __device__ constexpr int mo_brev_c(int q, int bits) {
+    int r = 0;
+    for (int b = 0; b < bits; ++b) r |= ((q >> b) & 1) << (bits - 1 - b);
+    return r;
+}
+// frequency index held by (register slot q, lane l) after mo_fft_dif
+template <int LOGR> __device__ __forceinline__ int mo_perm(int q, int l) {
+    return mo_brev_c(q, LOGR) + ((int)(__brev((unsigned)l) >> 27) << LOGR);
+}
+
+template <int LOGR, int SIGN>
+__device__ __forceinline__ void mo_fft_dif(float2 (&v)[1 << LOGR], const float2 *tw, int lane) {
+    constexpr int R = 1 << LOGR;
+    // R-point DIF over the register index (natural r -> bit-reversed slot)
+#pragma unroll
+    for (int len = R; len >= 2; len >>= 1) {
+        const int half = len / 2;
+#pragma unroll
+        for (int base = 0; base < R; base += len)
+#pragma unroll
+            for (int j = 0; j < half; ++j) {
+                const float2 u = v[base + j], w = v[base + j + half];
+                v[base + j] = make_float2(u.x + w.x, u.y + w.y);
+                const float2 d = make_float2(u.x - w.x, u.y - w.y);
+                v[base + j + half] = j == 0 ? d : mo_cmul(d, mo_w16<SIGN>(j * (16 / len)));
+            }
+    }
+    // twiddle W_N^{m k1}, k1 = brev_R(slot)
+#pragma unroll
+    for (int q = 1; q < R; ++q) v[q] = mo_cmul(v[q], mo_tw<SIGN>(tw, (lane * mo_brev_c(q, LOGR) * (32 >> LOGR)) & 1023));
+    // 32-point DIF across the lanes
+#pragma unroll
+    for (int h = 16; h >= 1; h >>= 1) {
+        const bool upper = (lane & h) != 0;
+        const float2 w = mo_tw<SIGN>(tw, (lane & (h - 1)) * (512 / h));
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const float bx = __shfl_xor_sync(0xffffffffu, v[q].x, h), by = __shfl_xor_sync(0xffffffffu, v[q].y, h);
+            if (upper) v[q] = mo_cmul(make_float2(bx - v[q].x, by - v[q].y), w);
+            else v[q] = make_float2(v[q].x + bx, v[q].y + by);
         }
-        __syncwarp();
     }
 }
-__device__ __forceinline__ int mo_brev(int i, int logn) { return (int)(__brev((unsigned)i) >> (32 - logn)); }
+
+template <int LOGR, int SIGN>
+__device__ __forceinline__ void mo_fft_dit(float2 (&v)[1 << LOGR], const float2 *tw, int lane) {
+    constexpr int R = 1 << LOGR;
+#pragma unroll
+    for (int h = 1; h <= 16; h <<= 1) {
+        const bool upper = (lane & h) != 0;
+        const float2 w = mo_tw<SIGN>(tw, (lane & (h - 1)) * (512 / h));
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const float2 t = upper ? mo_cmul(v[q], w) : v[q];
+            const float bx = __shfl_xor_sync(0xffffffffu, t.x, h), by = __shfl_xor_sync(0xffffffffu, t.y, h);
+            v[q] = upper ? make_float2(bx - t.x, by - t.y) : make_float2(t.x + bx, t.y + by);
+        }
+    }
+#pragma unroll
+    for (int q = 1; q < R; ++q) v[q] = mo_cmul(v[q], mo_tw<SIGN>(tw, (lane * mo_brev_c(q, LOGR) * (32 >> LOGR)) & 1023));
+#pragma unroll
+    for (int len = 2; len <= R; len <<= 1) {
+        const int half = len / 2;
+#pragma unroll
+        for (int base = 0; base < R; base += len)
+#pragma unroll
+            for (int j = 0; j < half; ++j) {
+                const float2 u = v[base + j];
+                const float2 t = j == 0 ? v[base + j + half] : mo_cmul(v[base + j + half], mo_w16<SIGN>(j * (16 / len)));
+                v[base + j] = make_float2(u.x + t.x, u.y + t.y);
+                v[base + j + half] = make_float2(u.x - t.x, u.y - t.y);
+            }
+    }
+}
+
+// call(LOGR) for the run-time transform length 2^logn (32 .. 512), LOGR = logn - 5 as a compile-time constant
+#define ULM_MO_DISPATCH(logn, call)                    \
+    switch (logn) {                                    \
+        case 5: call(0); break;                        \
+        case 6: call(1); break;                        \
+        case 7: call(2); break;                        \
+        case 8: call(3); break;                        \
+        default: call(4); break;                       \
+    }
 
 __global__ void __launch_bounds__(kMoThreads) motion_stats_kernel(const __grid_constant__ MoParams P) {
     const int e = blockIdx.x, f = blockIdx.y;
@@ -95,6 +186,28 @@ __global__ void __launch_bounds__(kMoThreads) motion_stats_kernel(const __grid_c
     (void)s_mean;
 }
 
+// depth FFT of the CTA's 32 lateral lines (one warp per line, 4 lines per warp) into the shared-memory tile s[line][position]
+template <int LOGR>
+__device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int rs, const float2 *x, int n_lat, int n_ax, int l0,
+                                               float mean, int warp, int lane) {
+    constexpr int R = 1 << LOGR;
+    for (int li = warp; li < kMoLines; li += kMoThreads / 32) {
+        const int l = l0 + li;
+        if (l >= n_lat) continue;                                      // warp-uniform; such lines are written as zeros below
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = 32 * r + lane;
+            float a = 0.f;
+            if (i < n_ax) { const float2 c = __ldg(x + (long long)l * n_ax + i); a = sqrtf(c.x * c.x + c.y * c.y) - mean; }
+            v[r] = make_float2(a, 0.f);
+        }
+        mo_fft_dif<LOGR, -1>(v, P.tw, lane);
+#pragma unroll
+        for (int q = 0; q < R; ++q) s[li * rs + 32 * q + lane] = v[q];
+    }
+}
+
 // grid = (lateral tiles of 32 lines, events, frames)
 __global__ void __launch_bounds__(kMoThreads) motion_fwd_z_kernel(const __grid_constant__ MoParams P) {
     extern __shared__ __align__(16) unsigned char mo_smem[];
@@ -107,23 +220,47 @@ __global__ void __launch_bounds__(kMoThreads) motion_fwd_z_kernel(const __grid_c
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float mean = P.stats[(long long)f * P.n_events + e].x;
     const float2 *x = P.x + (long long)f * P.frame_stride + P.ev.off[e];
-    for (int li = warp; li < kMoLines; li += kMoThreads / 32) {
-        const int l = l0 + li;
-        float2 *row = s + li * rs;
-        for (int i = lane; i < n2; i += 32) {
-            float a = 0.f;
-            if (l < n_lat && i < n_ax) { const float2 v = __ldg(x + (long long)l * n_ax + i); a = sqrtf(v.x * v.x + v.y * v.y) - mean; }
-            row[mo_brev(i, log2_)] = make_float2(a, 0.f);
-        }
-        __syncwarp();
-        mo_warp_fft<false>(row, log2_, P.tw, lane);
-    }
+#define ULM_MO_CALL(LR) mo_fwd_z_lines<LR>(P, s, rs, x, n_lat, n_ax, l0, mean, warp, lane)
+    ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
+#undef ULM_MO_CALL
     __syncthreads();
-    // transposed, coalesced write: T1[frame][event block][kz][l]
+    // transposed, coalesced write: T1[frame][event block][kz position][l]  (kz in the permuted order of mo_fft_dif: every
+    // later pass treats the kz rows independently and the final inverse depth transform takes exactly that order)
     float2 *t1 = P.t1 + (long long)f * P.t1_frame + P.ev.t1_off[e];
     const int n_lat_p = (n_lat + 31) / 32 * 32;
     for (int kz = warp; kz < n2; kz += kMoThreads / 32)
         t1[(long long)kz * n_lat_p + l0 + lane] = (l0 + lane < n_lat) ? s[lane * rs + kz] : make_float2(0.f, 0.f);
+}
+
+// lateral FFT of the CTA's 32 kz rows; REF: store the spectrum (permuted order); else product with the conjugate
+// reference spectrum (same permuted order on both sides), inverse lateral FFT (natural order out) into the tile s[row][dl]
+template <int LOGR, bool REF>
+__device__ __forceinline__ void mo_lat_rows(const MoParams &P, float2 *s, int rs, const float2 *t1, float2 *fref, int n_lat,
+                                            int n_lat_p, int n1, int kz0, int warp, int lane) {
+    constexpr int R = 1 << LOGR;
+    for (int ri = warp; ri < kMoLines; ri += kMoThreads / 32) {
+        const int kz = kz0 + ri;                                       // n2 is a multiple of 32: always a valid row
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int l = 32 * r + lane;
+            v[r] = l < n_lat ? __ldg(t1 + (long long)kz * n_lat_p + l) : make_float2(0.f, 0.f);
+        }
+        mo_fft_dif<LOGR, -1>(v, P.tw, lane);
+        if (REF) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) fref[(long long)kz * n1 + 32 * q + lane] = v[q];
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                const float2 a = v[q], r = __ldg(fref + (long long)kz * n1 + 32 * q + lane);
+                v[q] = make_float2(a.x * r.x + a.y * r.y, a.y * r.x - a.x * r.y);     // a conj(r)
+            }
+            mo_fft_dit<LOGR, +1>(v, P.tw, lane);
+#pragma unroll
+            for (int r = 0; r < R; ++r) s[ri * rs + 32 * r + lane] = v[r];
+        }
+    }
 }
 
 // grid = (kz tiles of 32 rows, events, frames [REF: 1])
@@ -140,40 +277,68 @@ __global__ void __launch_bounds__(kMoThreads) motion_lat_kernel(const __grid_con
     const int n_lat_p = (n_lat + 31) / 32 * 32;
     const float2 *t1 = P.t1 + (long long)f * P.t1_frame + P.ev.t1_off[e];
     float2 *fref = P.fref + P.ev.ref_off[e];
-    for (int ri = warp; ri < kMoLines; ri += kMoThreads / 32) {
-        const int kz = kz0 + ri;                                       // n2 is a multiple of 32: always a valid row
-        float2 *row = s + ri * rs;
-        for (int l = lane; l < n1; l += 32)
-            row[mo_brev(l, log1)] = l < n_lat ? __ldg(t1 + (long long)kz * n_lat_p + l) : make_float2(0.f, 0.f);
-        __syncwarp();
-        mo_warp_fft<false>(row, log1, P.tw, lane);
-        if (REF) {
-            for (int k = lane; k < n1; k += 32) fref[(long long)kz * n1 + k] = row[k];
-        } else {
-            // product with the conjugate reference spectrum, permuted in place into bit-reversed order for the inverse
-            for (int k = lane; k < n1; k += 32) {
-                const int j = mo_brev(k, log1);
-                if (k <= j) {
-                    const float2 a = row[k], r = __ldg(fref + (long long)kz * n1 + k);
-                    const float2 b = row[j], q = __ldg(fref + (long long)kz * n1 + j);
-                    row[j] = make_float2(a.x * r.x + a.y * r.y, a.y * r.x - a.x * r.y);     // a conj(r)
-                    row[k] = make_float2(b.x * q.x + b.y * q.y, b.y * q.x - b.x * q.y);
-                }
-            }
-            __syncwarp();
-            mo_warp_fft<true>(row, log1, P.tw, lane);
-        }
-    }
+#define ULM_MO_CALL(LR) mo_lat_rows<LR, REF>(P, s, rs, t1, fref, n_lat, n_lat_p, n1, kz0, warp, lane)
+    ULM_MO_DISPATCH(log1, ULM_MO_CALL)
+#undef ULM_MO_CALL
     if (REF) return;
     __syncthreads();
-    // transposed, coalesced write: T2[frame][event block][dl][kz]
+    // transposed, coalesced write: T2[frame][event block][dl][kz position]
     float2 *t2 = P.t2 + (long long)f * P.t2_frame + P.ev.t2_off[e];
     for (int dl = warp; dl < n1; dl += kMoThreads / 32) t2[(long long)dl * n2 + kz0 + lane] = s[lane * rs + dl];
 }
 
+// running maximum of c over the lateral-shift lines of one warp: inverse depth FFT of each line in registers, real parts
+// to the warp's row in shared memory (the depth neighbours of a new maximum are read from it)
+struct MoBest { float val, m, p; int idx; };
+template <int LOGR>
+__device__ __forceinline__ void mo_peak_lines(const MoParams &P, float *row, const float2 *t2, int n1, int n2, int warp, int lane,
+                                              MoBest &B) {
+    constexpr int R = 1 << LOGR;
+    for (int dl = warp; dl < n1; dl += kMoThreads / 32) {
+        float2 v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = __ldg(t2 + (long long)dl * n2 + 32 * q + lane);
+        mo_fft_dit<LOGR, +1>(v, P.tw, lane);
+        float best = -3.0e38f;
+        int bi = 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {                                  // depth shift 32 r + lane, ascending: first maximum
+            row[32 * r + lane] = v[r].x;
+            if (v[r].x > best) { best = v[r].x; bi = 32 * r + lane; }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        __syncwarp();
+        const int idx = dl * n2 + bi;
+        if (best > B.val || (best == B.val && idx < B.idx)) {
+            B.val = best; B.idx = idx;
+            B.m = row[(bi + n2 - 1) & (n2 - 1)];
+            B.p = row[(bi + 1) & (n2 - 1)];
+        }
+        __syncwarp();
+    }
+}
+
+// c(dl, dz) by one direct inverse DFT sum over the (permuted) kz positions of line dl: Re sum_kz T2[dl][pos] exp(+2 pi i kz dz / n2)
+template <int LOGR>
+__device__ __forceinline__ float mo_direct(const MoParams &P, const float2 *t2, int dl, int dz, int n2, int lane) {
+    float acc = 0.f;
+    for (int pos = lane; pos < n2; pos += 32) {
+        const int kz = mo_perm<LOGR>(pos >> 5, pos & 31);
+        const float2 v = __ldg(t2 + (long long)dl * n2 + pos);
+        const float2 w = __ldg(P.tw + ((kz * dz) & (n2 - 1)) * (32 >> LOGR));      // exp(-2 pi i kz dz / n2); the inverse uses its conjugate
+        acc += v.x * w.x + v.y * w.y;                                                  // Re(v conj(w))
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    return acc;
+}
+
 // grid = (events, frames): inverse FFT along depth of every lateral-shift line, running maximum, sub-pixel peak
 __global__ void __launch_bounds__(kMoThreads) motion_peak_kernel(const __grid_constant__ MoParams P) {
-    __shared__ __align__(16) float2 s[kMoThreads / 32][kMoMaxN];
+    __shared__ float rows[kMoThreads / 32][kMoMaxN];
     __shared__ float b_val[kMoThreads / 32], b_m[kMoThreads / 32], b_p[kMoThreads / 32];
     __shared__ int b_idx[kMoThreads / 32];
     __shared__ float nb[2];
@@ -181,46 +346,24 @@ __global__ void __launch_bounds__(kMoThreads) motion_peak_kernel(const __grid_co
     const int log1 = P.ev.log1[e], log2_ = P.ev.log2[e], n1 = 1 << log1, n2 = 1 << log2_;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const float2 *t2 = P.t2 + (long long)f * P.t2_frame + P.ev.t2_off[e];
-    float best = -3.0e38f, best_m = 0.f, best_p = 0.f;
-    int best_idx = 0x7fffffff;
-    for (int dl = warp; dl < n1; dl += kMoThreads / 32) {
-        float2 *row = s[warp];
-        for (int k = lane; k < n2; k += 32) row[mo_brev(k, log2_)] = __ldg(t2 + (long long)dl * n2 + k);
-        __syncwarp();
-        mo_warp_fft<true>(row, log2_, P.tw, lane);
-        float v = -3.0e38f;
-        int vi = 0;
-        for (int k = lane; k < n2; k += 32) if (row[k].x > v) { v = row[k].x; vi = k; }      // first maximum of this lane
-        for (int o = 16; o > 0; o >>= 1) {
-            const float ov = __shfl_xor_sync(0xffffffffu, v, o);
-            const int oi = __shfl_xor_sync(0xffffffffu, vi, o);
-            if (ov > v || (ov == v && oi < vi)) { v = ov; vi = oi; }
-        }
-        const int idx = dl * n2 + vi;
-        if (v > best || (v == best && idx < best_idx)) {
-            best = v; best_idx = idx;
-            best_m = row[(vi + n2 - 1) & (n2 - 1)].x;
-            best_p = row[(vi + 1) & (n2 - 1)].x;
-        }
-        __syncwarp();
-    }
-    if (lane == 0) { b_val[warp] = best; b_idx[warp] = best_idx; b_m[warp] = best_m; b_p[warp] = best_p; }
+    MoBest B{-3.0e38f, 0.f, 0.f, 0x7fffffff};
+#define ULM_MO_CALL(LR) mo_peak_lines<LR>(P, rows[warp], t2, n1, n2, warp, lane, B)
+    ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
+#undef ULM_MO_CALL
+    if (lane == 0) { b_val[warp] = B.val; b_idx[warp] = B.idx; b_m[warp] = B.m; b_p[warp] = B.p; }
     __syncthreads();
     int w_best = 0;
     for (int w = 1; w < kMoThreads / 32; ++w)
         if (b_val[w] > b_val[w_best] || (b_val[w] == b_val[w_best] && b_idx[w] < b_idx[w_best])) w_best = w;
     const float c0 = b_val[w_best], cm2 = b_m[w_best], cp2 = b_p[w_best];
     const int pk = b_idx[w_best], dl_pk = pk / n2, dz_pk = pk - dl_pk * n2;
-    // the lateral neighbours c(dl +- 1, dz): one direct inverse DFT sum over kz each (warps 0 and 1)
+    // the lateral neighbours c(dl +- 1, dz) (warps 0 and 1)
     if (warp < 2) {
         const int dl = (dl_pk + (warp == 0 ? n1 - 1 : 1)) & (n1 - 1);
         float acc = 0.f;
-        for (int k = lane; k < n2; k += 32) {
-            const float2 v = __ldg(t2 + (long long)dl * n2 + k);
-            const float2 w = P.tw[((k * dz_pk) & (n2 - 1)) * (1024 >> log2_)];       // exp(-2 pi i k dz / n2); the inverse needs its conjugate
-            acc += v.x * w.x + v.y * w.y;                                                    // Re(v conj(w))
-        }
-        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+#define ULM_MO_CALL(LR) acc = mo_direct<LR>(P, t2, dl, dz_pk, n2, lane)
+        ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
+#undef ULM_MO_CALL
         if (lane == 0) nb[warp] = acc;
     }
     __syncthreads();
