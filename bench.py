@@ -661,6 +661,70 @@ def run_localize(args):
         "gpu_launches": int(info["launches_last_call"]) * args.steps}))
 
 
+def run_chain(args):
+    """All built steps of the paper's chain on one ensemble, back to back on one stream (context figure, not a BASELINE
+    metric): channel data -> per-event slices (Stage 1, compound = 0) -> motion estimation on the slices -> clutter filter
+    (in place) -> Stage 2 + compounding + P = 8 sum-projection -> localization.  cfg 2; the paper quotes 0.52 s per
+    0.75 s ensemble for its whole pipeline on its GPU, which also contains separation, pairing and tracking."""
+    import torch
+    from paper_2511_21647_b200 import Plan, build
+    torch.cuda.set_device(0)
+    build.build()
+    cfg = synth.config(2).with_(compound=0)
+    n_frames = cfg.n_frames
+    channel, host_frames, distinct = make_ensemble(cfg, torch, torch.device("cuda", 0))
+    warmup = max(args.warmup, 3)
+    with Plan(**rounded_kwargs(cfg), max_frames=n_frames, stage2_block=8, clutter_frames=n_frames, motion_frames=n_frames,
+              precision=args.precision) as plan:
+        slices = torch.empty((n_frames, plan.slices_complex_per_frame), dtype=torch.complex64, device="cuda")
+        planes = torch.empty((n_frames, plan.planes_bytes_per_frame // 8), dtype=torch.complex64, device="cuda")
+
+        def step():
+            plan.beamform(channel, out=slices)
+            plan.motion_estimate(slices, 0)
+            plan.clutter_filter(slices, 4, out=slices)
+            plan.stage2_project(slices, out=planes)
+            return plan.localize(planes, 1.8, 1.4, 0.2, 0.7, 16)
+
+        for _ in range(warmup):
+            step()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(0)
+        sampler.start()
+        stream = torch.cuda.current_stream()
+        names = ["stage1_per_event", "motion", "clutter", "stage2_projection", "localize"]
+        acc = dict.fromkeys(names, 0.0)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        marks = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+        ev0.record(stream)
+        for s in range(args.steps):
+            m = marks[s]
+            m[0].record(stream); plan.beamform(channel, out=slices)
+            m[1].record(stream); plan.motion_estimate(slices, 0)
+            m[2].record(stream); plan.clutter_filter(slices, 4, out=slices)
+            m[3].record(stream); plan.stage2_project(slices, out=planes)
+            m[4].record(stream); plan.localize(planes, 1.8, 1.4, 0.2, 0.7, 16)
+            m[5].record(stream)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.result()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        for m in marks:
+            for i, n in enumerate(names):
+                acc[n] += m[i].elapsed_time(m[i + 1]) / args.steps
+        info = plan.info()
+    print(json.dumps({
+        "metric": "ensembles through Stage 1 -> motion -> clutter filter -> Stage 2 + projection -> localization (frames/s)",
+        "value": n_frames / (ms * 1e-3), "unit": "frames/s", "n_gpus": 1, "steps": args.steps, "warmup": warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_OF_PRECISION[info["precision"]] + "; later stages f32 (covariance bf16 x 3)",
+        "data": "synthetic: cfg 2 channel data (frames %s of the moving scene tiled); no real bubbles or tissue statistics, so the "
+                "filter / localizer outputs are not meaningful -- a timing chain only" % (list(distinct),),
+        "config": {"workload": "BASELINE configs[2] through every built step of the chain (context; PAPER.md:5 quotes 520 ms per "
+                               "ensemble for the paper's whole pipeline on its GPU)", "plan": info},
+        "stage_ms": acc, "acquisition_ms": 1e3 * n_frames / cfg.frame_rate_hz, "paper_whole_pipeline_ms": 520.0,
+        "clocks": clocks, "gpu_launches": None}))
+
+
 def run_volume(args):
     """Config 4, the paper's conventional comparator: cfg 1's data beamformed as a full
     180 x 180 x 164 volume by unpack_frame_kernel + das_volume_kernel (one frame); reported as volumes/s next to the
@@ -798,7 +862,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
-    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter", "motion", "localize"],
+    ap.add_argument("--workload", default="beamform", choices=["beamform", "stage2", "clutter", "motion", "localize", "chain"],
                     help="beamform = the BASELINE metric (Stage 1); stage2 = SURVEY 8(f) NEXT-1 on config 2's shapes")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2, 3],
                     help="scratch format of the main arm (ulm_rca_options.precision; 0 = the library's default)")
@@ -831,6 +895,8 @@ def main():
         run_motion(args)
     elif args.workload == "localize":
         run_localize(args)
+    elif args.workload == "chain":
+        run_chain(args)
     elif args.config == 4:
         run_volume(args)
     else:

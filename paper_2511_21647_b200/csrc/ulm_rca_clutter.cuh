@@ -290,12 +290,17 @@ __device__ __forceinline__ float cf_warp_sum(float v) {
 // lambda_c^2) and track[kCfB] is set to 1 when one of them moved by more than 1e-6 relative since the last call.
 __device__ void cf_mgs(float2 *z, float2 *q, int n_t, float *track = nullptr, int n_track = 0) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = kCfEigThreads / 32;
+    float nn_max = 0.f;
     for (int c = 0; c < kCfB; ++c) {
         // every warp forms the norm of column c itself (no extra barrier)
         float nn = 0.f;
         for (int i = lane; i < n_t; i += 32) { const float2 v = z[i * kCfQs + c]; nn += v.x * v.x + v.y * v.y; }
         nn = cf_warp_sum(nn);
-        const float inv = nn > 0.f ? rsqrtf(nn) : 0.f, inv2 = nn > 0.f ? 1.f / nn : 0.f;
+        // a column that has (numerically) no component outside the span of the previous ones -- C of rank < 32, e.g. an
+        // ensemble of repeated frames -- is deflated to zero instead of being normalised into noise
+        nn_max = fmaxf(nn_max, nn);
+        const bool live = nn > 1e-12f * nn_max && nn > 1e-36f;
+        const float inv = live ? rsqrtf(nn) : 0.f, inv2 = live ? 1.f / nn : 0.f;
         if (track && c < n_track && threadIdx.x == 0) {
             if (fabsf(nn - track[c]) > 1e-6f * nn) track[kCfB] = 1.f;
             track[c] = nn;
@@ -484,9 +489,11 @@ __global__ void __launch_bounds__(kCfEigThreads, 1) clutter_eig_kernel(const __g
                 }
         }
         // descending order of the Ritz values (rank by counting; ties by index)
-        const float mine = h[lane * kCfQs + lane].x;
+        // (a non-finite value can only come from non-finite input; it is ranked last so that the order stays a permutation)
+        auto clean = [](float v) { return (v == v && fabsf(v) < 3.0e38f) ? v : -3.0e38f; };
+        const float mine = clean(h[lane * kCfQs + lane].x);
         int rank = 0;
-        for (int b = 0; b < kCfB; ++b) { const float o = h[b * kCfQs + b].x; rank += (o > mine) || (o == mine && b < lane); }
+        for (int b = 0; b < kCfB; ++b) { const float o = clean(h[b * kCfQs + b].x); rank += (o > mine) || (o == mine && b < lane); }
         order[rank] = lane;
         P.lam[e * kCfB + rank] = mine;
     }

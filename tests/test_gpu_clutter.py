@@ -86,6 +86,25 @@ def test_rank_zero_is_the_identity_and_in_place_works(torch_cuda):
     np.testing.assert_array_equal(a, b)
 
 
+def test_rank_deficient_covariance_is_deflated_not_normalised_into_noise(torch_cuda):
+    """An ensemble of repeated frames (here 3 distinct frames, so C has rank 3 < the 32 iteration vectors): the
+    surplus vectors have nothing to converge to and are deflated to zero; asking for the 3 (or more) clutter components
+    removes everything, exactly as the oracle does.  (Found by chaining the stages on bench.py's tiled ensemble.)"""
+    cfg = small_cfg()
+    base = synth.clutter_ensemble(3, n_pix_list(cfg), seed=8, tissue_rank=2)
+    x = np.ascontiguousarray(base[np.arange(48) % 3])
+    p = oracle.OracleParams(**rounded_kwargs(cfg))
+    for rank in (3, 5):
+        got, lam, _ = run(torch_cuda, cfg, x, rank)
+        ref, lam_ref = clutter.clutter_filter(p, x.astype(np.complex128), rank)
+        assert np.isfinite(got).all() and np.isfinite(lam).all()
+        assert np.abs(got - ref).max() <= 1e-4 * np.abs(x).max()
+        assert np.abs(lam[:, :5] - lam_ref[:, :5]).max() <= 1e-4 * lam_ref[:, 0].max()
+    got, _, _ = run(torch_cuda, cfg, x, 1)                    # one component of three: still well defined
+    ref, _ = clutter.clutter_filter(p, x.astype(np.complex128), 1)
+    assert np.abs(got - ref).max() <= 1e-4 * np.abs(x).max()
+
+
 def test_smaller_call_on_a_larger_plan_and_bad_arguments(torch_cuda):
     torch = torch_cuda
     from paper_2511_21647_b200 import Plan, UlmRcaError
