@@ -308,6 +308,27 @@ typedef struct {
 ulm_rca_status ulm_rca_localize(const ulm_rca_plan *plan, const void *d_planes, int32_t n_frames,
                                 const ulm_rca_localize_params *params, void *d_loc, void *d_count, void *cuda_stream);
 
+/*
+ * ulm_rca_localize without a plan and WITHOUT ANY ALLOCATION -- for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  Same operation, same kernels and same results as
+ * ulm_rca_localize; the planes' geometry is passed as plain numbers:
+ *   d_planes : complex fp32 [frame][n_planes_xz planes of n_lat_xz x n_z | n_planes_yz planes of n_lat_yz x n_z], depth
+ *              index fastest (the output layout of ulm_rca_stage2_project), device memory; either plane set may be empty
+ *   d_loc, d_count, params : as for ulm_rca_localize (outputs in device memory, owned by the caller)
+ * The one scratch buffer of the operation -- the per-frame maximum of |V| that the intensity threshold needs -- lives in
+ * a file-scope device array of ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES unsigned ints (16 KB) that every GPU holding the
+ * library keeps until the process exits; n_frames beyond that limit is refused with ULM_RCA_EINVAL (split the call).
+ * The call clears the entries it uses (and d_count) on cuda_stream, enqueues the two kernels there and never
+ * synchronises; it calls no cudaMalloc / cudaFree / allocating library routine (the first call on a device only looks up
+ * the array's device address).  ALL calls on a device share that array: calls that can overlap on the GPU (different
+ * streams without an ordering between them, or different host threads) race on it and may threshold against the wrong
+ * maximum -- order them on one stream or with events.  The array keeps the last call's contents between calls.
+ */
+#define ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES 4096
+ulm_rca_status ulm_rca_localize_static(const void *d_planes, int32_t n_frames, int32_t n_z, int32_t n_planes_xz,
+                                       int32_t n_lat_xz, int32_t n_planes_yz, int32_t n_lat_yz,
+                                       const ulm_rca_localize_params *params, void *d_loc, void *d_count, void *cuda_stream);
+
 /* Host-only view of the ring kernel's tile / window planning for ONE aperture (no CUDA device needed; used by the
  * CPU tests of the host logic): receive elements n_rx at `pitch_m`, transmit angles `angles_rad[n_tx]` with offsets
  * `t0_s` (NULL = 0), image grid `grid`.  Returns the number of tiles in *n_tiles, the stage length in entries in

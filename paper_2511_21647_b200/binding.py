@@ -22,7 +22,7 @@ _STATUS = {1: "EINVAL", 2: "ENOMEM", 3: "ECUDA", 4: "EUNSUPPORTED"}
 EXPORTS = ["ulm_rca_plan_create", "ulm_rca_beamform", "ulm_rca_beamform_volume", "ulm_rca_beamform_host",
            "ulm_rca_plan_sizes", "ulm_rca_plan_info", "ulm_rca_plan_timing", "ulm_rca_fp32_peak", "ulm_rca_ring_probe", "ulm_rca_fold_probe",
            "ulm_rca_stage2_project", "ulm_rca_stage2_sizes", "ulm_rca_stage2_timing",
-           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing", "ulm_rca_motion_estimate", "ulm_rca_motion_timing", "ulm_rca_localize",
+           "ulm_rca_clutter_filter", "ulm_rca_clutter_timing", "ulm_rca_motion_estimate", "ulm_rca_motion_timing", "ulm_rca_localize", "ulm_rca_localize_static",
            "ulm_rca_plan_destroy",
            "ulm_rca_last_error"]
 
@@ -101,6 +101,8 @@ def load() -> C.CDLL:
     lib.ulm_rca_motion_timing.argtypes = [vp, C.POINTER(C.c_double)]
     lib.ulm_rca_localize.restype = C.c_int
     lib.ulm_rca_localize.argtypes = [vp, vp, i32, C.POINTER(LocalizeParams), vp, vp, vp]
+    lib.ulm_rca_localize_static.restype = C.c_int
+    lib.ulm_rca_localize_static.argtypes = [vp, i32, i32, i32, i32, i32, i32, C.POINTER(LocalizeParams), vp, vp, vp]
     lib.ulm_rca_fp32_peak.restype = C.c_int
     lib.ulm_rca_fp32_peak.argtypes = [C.POINTER(C.c_double), vp]
     lib.ulm_rca_ring_probe.restype = C.c_int
@@ -133,6 +135,37 @@ def _farr(v):
 INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
              "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame", "events_executed",
              "stage2_taps", "stage2_tile_cols"]
+
+
+LOCALIZE_STATIC_MAX_FRAMES = 4096        # ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES of include/ulm_rca.h
+
+
+def localize_static(planes, n_z: int, n_planes_xz: int, n_lat_xz: int, n_planes_yz: int, n_lat_yz: int, loc, count,
+                    sigma_lat_px: float, sigma_ax_px: float, threshold_rel: float, ncc_min: float, stream=None):
+    """ulm_rca_localize_static: the localization without a plan and without any allocation.  planes: contiguous complex64
+    CUDA tensor [frame][planes of a frame]; loc (float32 [frame][plane][capacity][4]) and count (int32 [frame][plane]) are
+    the CALLER's CUDA tensors (nothing is allocated here either); all calls on a device share one static scratch array,
+    so calls that may overlap on the GPU race (see include/ulm_rca.h)."""
+    import torch
+    n_pl = int(n_planes_xz) + int(n_planes_yz)
+    per_frame = (int(n_planes_xz) * int(n_lat_xz) + int(n_planes_yz) * int(n_lat_yz)) * int(n_z)
+    if not (planes.is_cuda and planes.dtype == torch.complex64 and planes.is_contiguous() and planes.dim() == 2
+            and planes.shape[1] == per_frame):
+        raise ValueError("planes must be a contiguous complex64 CUDA tensor [frame][%d]" % per_frame)
+    n = int(planes.shape[0])
+    if not (loc.is_cuda and loc.dtype == torch.float32 and loc.is_contiguous() and loc.dim() == 4 and loc.shape[0] == n
+            and loc.shape[1] == n_pl and loc.shape[3] == 4 and loc.device == planes.device):
+        raise ValueError("loc must be a contiguous float32 CUDA tensor [frame][plane][capacity][4] on the planes' device")
+    if not (count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and tuple(count.shape) == (n, n_pl)
+            and count.device == planes.device):
+        raise ValueError("count must be a contiguous int32 CUDA tensor [frame][plane] on the planes' device")
+    prm = LocalizeParams(float(sigma_lat_px), float(sigma_ax_px), float(threshold_rel), float(ncc_min), int(loc.shape[2]))
+    s = stream if stream is not None else torch.cuda.current_stream(planes.device)
+    with torch.cuda.device(planes.device):
+        _check(load().ulm_rca_localize_static(C.c_void_p(planes.data_ptr()), n, int(n_z), int(n_planes_xz), int(n_lat_xz),
+                                              int(n_planes_yz), int(n_lat_yz), C.byref(prm), C.c_void_p(loc.data_ptr()),
+                                              C.c_void_p(count.data_ptr()), C.c_void_p(s.cuda_stream)))
+    return loc, count
 
 
 class Plan:

@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1100,6 +1101,94 @@ ulm_rca_status ulm_rca_localize(const ulm_rca_plan *plan, const void *d_planes, 
         launches += 2;
     }
     plan->last_launches = launches;
+    return ULM_RCA_OK;
+}
+
+// ---- ulm_rca_localize_static: the same two kernels, no plan, no allocation ------------------------------------------
+// The per-frame maximum (the only scratch of the operation) lives in this file-scope device array.  Its name is a
+// host-side stand-in in host code: the device address is looked up once per device (that device current) with
+// cudaGetSymbolAddress and handed to the kernels in LoParams::frame_max like the plan-owned buffer of ulm_rca_localize.
+static __device__ __align__(256) unsigned int g_lo_static_frame_max[ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_lo_static_mutex;
+unsigned int *g_lo_static_ptr[kStaticMaxDevices] = {};      // device address of g_lo_static_frame_max, per device
+
+// set-up of the current device (once per device): address of the scratch array, shared-memory attribute of the kernel
+ulm_rca_status lo_static_setup(unsigned int **out) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(ULM_RCA_EUNSUPPORTED, "device index %d beyond %d", dev, kStaticMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_lo_static_mutex);
+    if (!g_lo_static_ptr[dev]) {
+        unsigned int *ptr = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress((void **)&ptr, g_lo_static_frame_max));
+        if (!ptr) return fail(ULM_RCA_ECUDA, "cudaGetSymbolAddress returned a NULL address");
+        CUDA_TRY(cudaFuncSetAttribute(ulm::localize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ulm::kLoSmem));
+        g_lo_static_ptr[dev] = ptr;
+    }
+    *out = g_lo_static_ptr[dev];
+    return ULM_RCA_OK;
+}
+}  // namespace
+
+ulm_rca_status ulm_rca_localize_static(const void *d_planes, int32_t n_frames, int32_t n_z, int32_t n_planes_xz,
+                                       int32_t n_lat_xz, int32_t n_planes_yz, int32_t n_lat_yz,
+                                       const ulm_rca_localize_params *prm, void *d_loc, void *d_count, void *cuda_stream) {
+    if (n_frames < 0) return fail(ULM_RCA_EINVAL, "n_frames < 0");
+    if (n_frames > ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES)
+        return fail(ULM_RCA_EINVAL, "n_frames %d exceeds the static scratch of %d frames (ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES): split the call",
+                    n_frames, ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES);
+    if (n_z < 1 || n_planes_xz < 0 || n_planes_yz < 0 || n_planes_xz + n_planes_yz < 1 || (n_planes_xz > 0 && n_lat_xz < 1) ||
+        (n_planes_yz > 0 && n_lat_yz < 1))
+        return fail(ULM_RCA_EINVAL, "plane geometry invalid");
+    if (n_frames == 0) return ULM_RCA_OK;
+    if (!d_planes || !prm || !d_loc || !d_count) return fail(ULM_RCA_EINVAL, "pointer is NULL");
+    if (!(prm->sigma_lat_px > 0) || !(prm->sigma_ax_px > 0) || !std::isfinite(prm->sigma_lat_px) || !std::isfinite(prm->sigma_ax_px) ||
+        !std::isfinite(prm->threshold_rel) || !std::isfinite(prm->ncc_min) || prm->capacity < 1)
+        return fail(ULM_RCA_EINVAL, "localize parameters invalid");
+    const int n_pl = n_planes_xz + n_planes_yz;
+    const int lat_max = std::max(n_planes_xz > 0 ? n_lat_xz : 0, n_planes_yz > 0 ? n_lat_yz : 0);
+    const long long lat_tiles = (lat_max + ulm::kLoTl - 1) / ulm::kLoTl, z_tiles = (n_z + ulm::kLoTa - 1) / ulm::kLoTa;
+    if (z_tiles > 65535 || n_pl > 65535) return fail(ULM_RCA_EINVAL, "grid too large (planes per frame, or depth tiles, beyond 65535)");
+    unsigned int *frame_max = nullptr;
+    if (ulm_rca_status s = lo_static_setup(&frame_max)) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    ulm::LoParams L{};
+    L.n_z = n_z;
+    L.n_planes[0] = n_planes_xz; L.n_lat[0] = n_planes_xz > 0 ? n_lat_xz : 0;
+    L.n_planes[1] = n_planes_yz; L.n_lat[1] = n_planes_yz > 0 ? n_lat_yz : 0;
+    L.set_off[0] = 0; L.set_off[1] = (long long)n_planes_xz * L.n_lat[0] * n_z;
+    L.planes_per_frame = L.set_off[1] + (long long)n_planes_yz * L.n_lat[1] * n_z;
+    double gm = 0, g1[ulm::kLoTaps], g2[ulm::kLoTaps];
+    for (int k = 0; k < ulm::kLoTaps; ++k) {
+        const double a = k - ulm::kLoHalf;
+        g1[k] = std::exp(-a * a / (2.0 * prm->sigma_lat_px * prm->sigma_lat_px));
+        g2[k] = std::exp(-a * a / (2.0 * prm->sigma_ax_px * prm->sigma_ax_px));
+        L.g1[k] = (float)g1[k]; L.g2[k] = (float)g2[k];
+    }
+    for (int i = 0; i < ulm::kLoTaps; ++i) for (int j = 0; j < ulm::kLoTaps; ++j) gm += g1[i] * g2[j];
+    gm /= 121.0;
+    double gd = 0;
+    for (int i = 0; i < ulm::kLoTaps; ++i) for (int j = 0; j < ulm::kLoTaps; ++j) gd += (g1[i] * g2[j] - gm) * (g1[i] * g2[j] - gm);
+    L.g_mean = (float)gm; L.g_den = (float)gd;
+    L.threshold_rel = prm->threshold_rel; L.ncc_min = prm->ncc_min; L.capacity = prm->capacity;
+    const int batch = std::min(n_frames, 65535 / n_pl);        // grid.z = frames x planes of a launch
+    for (int f0 = 0; f0 < n_frames; f0 += batch) {
+        const int nb = std::min(batch, n_frames - f0);
+        L.planes = static_cast<const float2 *>(d_planes) + (long long)f0 * L.planes_per_frame;
+        L.n_frames = nb;
+        L.frame_max = frame_max + f0;
+        L.loc = static_cast<float4 *>(d_loc) + (long long)f0 * n_pl * prm->capacity;
+        L.count = static_cast<int *>(d_count) + (long long)f0 * n_pl;
+        // the array keeps the previous call's maxima: the entries of this call start at zero
+        CUDA_TRY(cudaMemsetAsync(L.frame_max, 0, (size_t)nb * sizeof(unsigned int), st));
+        CUDA_TRY(cudaMemsetAsync(L.count, 0, (size_t)nb * n_pl * sizeof(int), st));
+        ulm::localize_max_kernel<<<dim3(64, nb), 256, 0, st>>>(L);
+        ulm::localize_kernel<<<dim3((unsigned)lat_tiles, (unsigned)z_tiles, (unsigned)(nb * n_pl)), ulm::kLoThreads, ulm::kLoSmem, st>>>(L);
+    }
+    CUDA_TRY(cudaGetLastError());
     return ULM_RCA_OK;
 }
 
