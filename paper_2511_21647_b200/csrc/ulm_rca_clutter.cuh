@@ -287,10 +287,13 @@ __device__ __forceinline__ float cf_warp_sum(float v) {
 
 // modified Gram-Schmidt of the kCfB columns of z (in place) -> q; both [n_t][kCfQs].  All threads of the CTA.
 // track != nullptr: track[c] keeps the squared norm of the orthogonalised column c < n_track (the running estimate of
-// lambda_c^2) and track[kCfB] is set to 1 when one of them moved by more than 1e-6 relative since the last call.
+// lambda_c^2) and track[kCfB] is set to 1 when their PRODUCT moved by more than 2e-6 relative since the last call (the
+// sum of the logarithms of the ratios).  The product of the leading diagonal of R is |det| of C restricted to
+// the span of the leading n_track columns: it does not see rotations INSIDE that span (which the Rayleigh-Ritz step
+// resolves exactly and the filter does not depend on), only the convergence of the span itself.
 __device__ void cf_mgs(float2 *z, float2 *q, int n_t, float *track = nullptr, int n_track = 0) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = kCfEigThreads / 32;
-    float nn_max = 0.f;
+    float nn_max = 0.f, drift = 0.f;
     for (int c = 0; c < kCfB; ++c) {
         // every warp forms the norm of column c itself (no extra barrier)
         float nn = 0.f;
@@ -302,8 +305,10 @@ __device__ void cf_mgs(float2 *z, float2 *q, int n_t, float *track = nullptr, in
         const bool live = nn > 1e-12f * nn_max && nn > 1e-36f;
         const float inv = live ? rsqrtf(nn) : 0.f, inv2 = live ? 1.f / nn : 0.f;
         if (track && c < n_track && threadIdx.x == 0) {
-            if (fabsf(nn - track[c]) > 1e-6f * nn) track[kCfB] = 1.f;
-            track[c] = nn;
+            // log of the ratio to the last call's value; a column that died or came to life counts as a move
+            drift += (live && track[c] > 0.f) ? log1pf((nn - track[c]) / track[c]) : ((live || track[c] != 0.f) ? 1.f : 0.f);
+            track[c] = live ? nn : 0.f;
+            if (c == n_track - 1 && fabsf(drift) > 2e-6f) track[kCfB] = 1.f;
         }
         for (int c2 = c + 1 + warp; c2 < kCfB; c2 += n_warps) {
             float pr = 0.f, pi = 0.f;
