@@ -90,6 +90,7 @@ struct Aperture {
     TxTables proj;      // 1 plane: the reference slice; one table row block per FOLDED event
     TxTables vol;       // volume comparator: one plane per pixel of the other lateral axis
     ulm::RingTables ring;
+    ulm::RingTables ring2;            // tiles of the two-group work items (ring_plan_dual)
     long long out_base = 0;
 };
 
@@ -666,6 +667,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
                                        P.ap[1].ring, &why);
         if (ok) {
             P.kernel = 2;
+            if (!P.d32) ulm::ring_plan_dual(desc, P.pitch, P.c, P.fs, P.t_start, P.l_row, P.ring, P.ap[0].ring2, P.ap[1].ring2);
             CUDA_TRY(ulm::ring_set_attributes());       // per-device function attribute, set on the plan's device
         } else if (opt->kernel == 2) return fail(ULM_RCA_EUNSUPPORTED, "ring kernel unavailable: %s", why ? why : "?");
         if (cudaGetLastError() != cudaSuccess) return fail(ULM_RCA_ECUDA, "ring table upload failed");
@@ -791,7 +793,8 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
                 R.n0 = A.proj.n0.as<int>(); R.f0m = A.proj.f0m.as<float>();
                 R.out_base = A.out_base;
             }
-            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, L, group_frames(nb), P.d32, P.w2, P.apod, st);
+            P.last_launches += ulm::ring_launch(P.ring, P.ap[0].ring, P.ap[1].ring, P.ap[0].ring2, P.ap[1].ring2, L, group_frames(nb),
+                                                P.d32, P.w2, P.apod, st);
         } else {
             for (int a = 0; a < 2; ++a) {
                 const Aperture &A = P.ap[a];

@@ -70,6 +70,11 @@ struct RingLaunch {
     // whose partial sums go to `partial` [v][thread][PX][F] and are added in slice order by ring_combine_kernel.
     int n_items, n_whole, split_s;
     float2 *partial;
+    // DUAL kernels: a work item covers TWO consecutive frame groups (2 F frames) of a tile of PX = 2 rows: the stage
+    // brings the windows of both groups (identical delays) and the index / weight / phasor arithmetic of a (pixel,
+    // element, angle) term is shared by 2 F frames.  n_groups then counts PAIRS; n_fgroups = the real frame groups.
+    int n_fgroups, stage_half;     // stage_half = byte offset of the second group's window inside a ring slot
+    int g_first;                   // first frame group (pair) this launch works on: item w belongs to group g_first + w / (items per group)
 };
 
 // (item, slice) of work item w; slice = -1: whole item
@@ -138,10 +143,12 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 // run-time index would copy the whole struct to local memory)
 #define ULM_AP(field) (a ? P.ap[1].field : P.ap[0].field)
 
-template <int F, int PX, bool D32, bool APOD, bool W2 = false>
+template <int F, int PX, bool D32, bool APOD, bool W2 = false, bool DUAL = false>
 __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_constant__ RingLaunch P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int EB = entry_bytes(F, D32);
+    constexpr int NAB = DUAL ? 2 : 1, FE = NAB * F;      // frame groups / frames of a work item
+    static_assert(!(DUAL && D32), "the two-group items exist for compact entries only");
     const int NS = P.n_stages;
     unsigned char *p_misc = smem + (size_t)NS * P.stage_stride;
     // [k][row] {frac(U0_k(z_row)) - 0.5, floor(U0_k(z_row)) - floor(U0_k(z_iz0))}: the integer row offset is added
@@ -184,8 +191,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
                 int w, slice;
                 ring_work(P, ww, w, slice);
-                const int g = w / tiles_all;
-                int tt = w - g * tiles_all;
+                const int gl = w / tiles_all, g = gl + P.g_first;
+                int tt = w - gl * tiles_all;
                 const int a = tt >= items0 ? 1 : 0;
                 if (a) tt -= items0;
                 const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
@@ -228,8 +235,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
             int w, slice;
             ring_work(P, ww, w, slice);
-            const int g = w / tiles_all;
-            int tt = w - g * tiles_all;
+            const int gl = w / tiles_all, g = gl + P.g_first;
+            int tt = w - gl * tiles_all;
             const int a = tt >= items0 ? 1 : 0;
             if (a) tt -= items0;
             const int n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
@@ -243,7 +250,9 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
             const int *n0 = ULM_AP(n0), *dj = ULM_AP(dj) + (size_t)tt * n_rx, *wj = ULM_AP(wj) + (size_t)tt * n_rx;
             const int iz0 = ((tt * kRingConsumers) / n_lat) * PX;          // first row of the tile
             const int n_st = nj * n_tx;
-            const unsigned char *grp = P.iq + (size_t)g * P.n_events * P.n_rx_max * P.l_row * EB;
+            const size_t grp_bytes = (size_t)P.n_events * P.n_rx_max * P.l_row * EB;
+            const unsigned char *grp = P.iq + (size_t)(NAB * g) * grp_bytes;
+            const bool has_b = DUAL && NAB * g + 1 < P.n_fgroups;      // the last pair may hold one group only
             for (int sb = 0; sb < n_st; sb += 32) {
                 // each lane fetches the (unclamped) window start of one stage
                 const int my = sb + lane;
@@ -266,9 +275,10 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                         s_hdr[slot] = s0_raw - s0 - kMagicBits;     // entry shift, with the magic-constant bits folded in
                         const uint32_t bar = smem_u32(&s_full[slot]);
                         const uint32_t bytes = (uint32_t)wlen * EB;
-                        mbar_expect_tx(bar, bytes);
+                        mbar_expect_tx(bar, has_b ? 2u * bytes : bytes);
                         const unsigned char *src = grp + (((size_t)(e0 + k) * P.n_rx_max + j) * P.l_row + s0) * EB;
                         bulk_g2s(smem_u32(smem) + slot * P.stage_stride, src, bytes, bar);
+                        if (has_b) bulk_g2s(smem_u32(smem) + slot * P.stage_stride + P.stage_half, src + grp_bytes, bytes, bar);
                     }
                     if (++slot == (uint32_t)NS) { slot = 0; phase ^= 1; }
                 }
@@ -285,8 +295,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
     for (int ww = blockIdx.x; ww < P.n_work; ww += gridDim.x) {
         int w, slice;
         ring_work(P, ww, w, slice);
-        const int g = w / tiles_all;
-        int tt = w - g * tiles_all;
+        const int gl = w / tiles_all, g = gl + P.g_first;
+        int tt = w - gl * tiles_all;
         const int a = tt >= items0 ? 1 : 0;
         if (a) tt -= items0;
         const int n_tx = ULM_AP(n_tx), n_rx = ULM_AP(n_rx), n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax);
@@ -334,11 +344,11 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         for (int m = 0; m < PX; ++m) tab_off[m] = (uint32_t)(min(r0 + m, rows - 1) - min(r0, rows - 1)) * 8u;
 
         // accumulators: (frame 2p, frame 2p+1) pairs of real / imaginary parts for FFMA2
-        unsigned long long accR2[PX][F / 2], accI2[PX][F / 2];
+        unsigned long long accR2[PX][FE / 2], accI2[PX][FE / 2];
 #pragma unroll
         for (int m = 0; m < PX; ++m)
 #pragma unroll
-            for (int f = 0; f < F / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
+            for (int f = 0; f < FE / 2; ++f) accR2[m][f] = accI2[m][f] = 0ull;
 
         bool ready = false;      // the full barrier of the next stage was already seen complete
         for (int j = jb; j < n_rx; j += js) {
@@ -405,7 +415,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                 } else {
                     // software pipeline over (pixel, 4-frame chunk): the five LDS.64 of step i + 1 (three mid word
                     // pairs, two d word pairs) are issued before the 32 FMAs of step i
-                    constexpr int NQ = F / 4, NSTEP = PX * NQ;
+                    constexpr int NQ = F / 4, NS2 = NAB * NQ, NSTEP = PX * NS2;
+                    const uint32_t half = DUAL ? (uint32_t)P.stage_half : 0u;      // window of the second frame group
                     unsigned long long buf[2][5];
                     PixCtx cur = prep_tb(0, tbn), nxt = cur;
                     if (PX > 1) tbn = lds64(tk + tab_off[1]);
@@ -413,23 +424,24 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                     buf[0][3] = lds64(cur.addr + 6u * F); buf[0][4] = lds64(cur.addr + 6u * F + 8u);
 #pragma unroll
                     for (int st = 0; st < NSTEP; ++st) {
-                        const int m = st / NQ, q = st % NQ;
+                        const int m = st / NS2, r = st % NS2, ab = r / NQ, q = r % NQ;
                         if (st + 1 < NSTEP) {
-                            const int m1 = (st + 1) / NQ, q1 = (st + 1) % NQ;
-                            if (q1 == 0) {
-                                // the table row of pixel m1 was requested a whole pixel (NQ chunks) earlier
+                            const int m1 = (st + 1) / NS2, r1 = (st + 1) % NS2, ab1 = r1 / NQ, q1 = r1 % NQ;
+                            if (r1 == 0) {
+                                // the table row of pixel m1 was requested a whole pixel earlier
                                 nxt = prep_tb(m1, tbn);
                                 if (m1 + 1 < PX) tbn = lds64(tk + tab_off[m1 + 1]);
                             }
-                            const uint32_t a1 = q1 == 0 ? nxt.addr : cur.addr;
+                            const uint32_t a1 = (r1 == 0 ? nxt.addr : cur.addr) + (ab1 ? half : 0u);
                             unsigned long long *b = buf[(st + 1) & 1];
                             b[0] = lds64(a1 + 24u * q1); b[1] = lds64(a1 + 24u * q1 + 8u); b[2] = lds64(a1 + 24u * q1 + 16u);
                             b[3] = lds64(a1 + 6u * F + 16u * q1); b[4] = lds64(a1 + 6u * F + 16u * q1 + 8u);
                         }
                         const unsigned long long *b = buf[st & 1];
                         chunk_mac2<W2>(b[0], b[1], b[2], b[3], b[4], cur.A.ah, cur.A.ah2, pack_f2(cur.c, cur.c),
-                                   pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + 2 * q, accI2[m] + 2 * q);
-                        if (q == NQ - 1) cur = nxt;
+                                   pack_f2(cur.s, cur.s), pack_f2(-cur.s, -cur.s), accR2[m] + ab * (F / 2) + 2 * q,
+                                   accI2[m] + ab * (F / 2) + 2 * q);
+                        if (r == NS2 - 1) cur = nxt;
                     }
                 }
                 __syncwarp();
@@ -439,16 +451,16 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
         __syncwarp();
         if (lane == 0) mbar_arrive(my_tab_empty);      // this warp is done with the item's tables
         if (slice >= 0) {
-            // partial sums of a slice: [work item - n_whole][thread][PX][F], added in slice order by ring_combine_kernel
-            float2 *dst = P.partial + ((size_t)(ww - P.n_whole) * kRingConsumers + t) * (PX * F);
+            // partial sums of a slice: [work item - n_whole][thread][PX][FE], added in slice order by ring_combine_kernel
+            float2 *dst = P.partial + ((size_t)(ww - P.n_whole) * kRingConsumers + t) * (PX * FE);
 #pragma unroll
             for (int m = 0; m < PX; ++m)
 #pragma unroll
-                for (int f = 0; f < F; f += 2) {
+                for (int f = 0; f < FE; f += 2) {
                     float r0, r1, i0, i1;
                     unpack_f2(accR2[m][f / 2], r0, r1);
                     unpack_f2(accI2[m][f / 2], i0, i1);
-                    *reinterpret_cast<float4 *>(dst + m * F + f) = make_float4(r0, i0, r1, i1);
+                    *reinterpret_cast<float4 *>(dst + m * FE + f) = make_float4(r0, i0, r1, i1);
                 }
         } else if (active) {
             // projection write: one float2 per pixel and frame; the PX pixels of a thread are contiguous in memory
@@ -459,8 +471,8 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
                              (((P.out_frame_stride | out_base | (long long)n_ax) & 1) == 0) &&
                              ((reinterpret_cast<unsigned long long>(P.out) & 15ull) == 0);
 #pragma unroll
-            for (int f = 0; f < F; ++f) {
-                const int fr = g * F + f;
+            for (int f = 0; f < FE; ++f) {
+                const int fr = g * FE + f;       // (the frames of the NAB groups of an item are consecutive)
                 if (fr >= P.n_frames) break;
                 float2 *dst = P.out + (long long)fr * P.out_frame_stride + out_base + (long long)ix * n_ax + izs;
                 float re[PX], im[PX];
@@ -487,14 +499,14 @@ __global__ void __launch_bounds__(kRingThreads, 1) das_ring_kernel(const __grid_
 }
 
 // Adds the split_s partial sums of every split work item in slice order (deterministic) and writes the pixels.
-// grid = (split items, PX), block = kRingConsumers.
+// grid = (split items, PX), block = kRingConsumers.  F = frames of a work item (2 x 12 for the two-group items).
 template <int F, int PX>
 __global__ void __launch_bounds__(kRingConsumers) ring_combine_kernel(const __grid_constant__ RingLaunch P) {
     const int w = P.n_whole + blockIdx.x, m = blockIdx.y, t = threadIdx.x;
     const int items0 = P.ap[0].n_tiles * (P.per_angle ? P.ap[0].n_tx : 1);
     const int tiles_all = items0 + P.ap[1].n_tiles * (P.per_angle ? P.ap[1].n_tx : 1);
-    const int g = w / tiles_all;
-    int tt = w - g * tiles_all;
+    const int gl = w / tiles_all, g = gl + P.g_first;
+    int tt = w - gl * tiles_all;
     const int a = tt >= items0 ? 1 : 0;
     if (a) tt -= items0;
     const int n_lat = ULM_AP(n_lat), n_ax = ULM_AP(n_ax), n_tiles_a = ULM_AP(n_tiles);
