@@ -184,8 +184,10 @@ def das_roofline(cfg, args, arm, gathers, fp32_probe, world_ms=None):
             "frac": achieved / NOMINAL_FP32_TFLOPS,
             "peak_measured": fp32_probe, "frac_of_measured": (achieved / fp32_probe) if fp32_probe else None,
             "traffic": measured_traffic(args.config, info["precision"]) if not args.per_angle else None,
-            "kernel": ("das_ring_kernel<12,4,%s,0,%s>" % ("1" if info["precision"] == 2 else "0", "1" if info["precision"] == 3 else "0"))
-            if info["kernel"] == 2 else "das_generic_kernel",
+            # compact entries, more than 12 frames: work items of two frame groups, 2 pixel rows (template <F, PX, D32, APOD, W2, DUAL>)
+            "kernel": (("das_ring_kernel<12,4,1,0,0,0>" if info["precision"] == 2 else
+                        "das_ring_kernel<12,2,0,0,%d,1> (+ <12,4,0,0,%d,0> for an odd last frame group)" % ((info["precision"] == 3,) * 2))
+                       if info["kernel"] == 2 else "das_generic_kernel"),
             "precision": info["precision"], "kernel_ms": arm["das_ms"], "prepass_ms": arm["demod_ms"],
             "flop_per_gather_sample": FLOP_PER_GATHER, "gather_samples_per_launch": gathers_exec,
             "gather_samples_of_the_definition": gathers, "events_executed_per_frame": info["events_executed"],
