@@ -271,7 +271,8 @@ ulm_rca_status ulm_rca_clutter_timing(const ulm_rca_plan *plan, double *ms5);
  *   d_motion    : float4 [frame] = (dx, dy, dz in metres, mean NCC peak), device memory
  *   d_per_event : NULL, or float4 [frame][event] = (lateral shift in pixels, axial shift in pixels, NCC peak, 0)
  * Needs options.motion_frames >= n_frames and slices of at most 512 pixels along each axis.  Enqueues six kernels on
- * cuda_stream (hand-written radix-2 FFTs; no library FFT), never synchronises; one call in flight per plan.
+ * cuda_stream (hand-written warp FFTs in registers, two frames per complex transform; no library FFT), never
+ * synchronises; one call in flight per plan.
  */
 ulm_rca_status ulm_rca_motion_estimate(const ulm_rca_plan *plan, const void *d_slices, int32_t n_frames, int32_t ref_frame,
                                        void *d_motion, void *d_per_event, void *cuda_stream);

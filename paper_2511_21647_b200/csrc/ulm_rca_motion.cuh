@@ -13,7 +13,9 @@
 // every pass over global memory coalesced, and the product with the reference spectrum and the inverse lateral
 // transform fused into the forward lateral pass:
 //   motion_stats_kernel     mean and mean-removed energy of every B-mode image
-//   motion_fwd_z_kernel     FFT along depth of 32 lateral lines per CTA, written transposed  T1[img][kz][l]
+//   motion_fwd_z_kernel     FFT along depth of 32 lateral lines per CTA, written transposed  T1[img][kz][l]; an image =
+//                           TWO frames, (a_2p, a_2p+1) as real / imaginary part: correlating with the fixed reference is
+//                           linear in the frame, so Re / Im of the final map are the two frames' correlation maps
 //   motion_lat_kernel<REF>  FFT along the lateral axis of 32 kz rows per CTA; REF: store the reference spectrum;
 //                           else multiply by its conjugate, inverse lateral FFT, write transposed  T2[img][dl][kz]
 //   motion_peak_kernel      inverse FFT along depth line by line, running argmax, neighbours, parabola -> (d_lat, d_ax, ncc)
@@ -37,9 +39,10 @@ struct MoParams {
     long long frame_stride;
     MoEvents ev;
     int n_events, n_frames, ref_frame;
+    int n_pairs;                  // packed images: frames (2 p, 2 p + 1) in the real / imaginary part; image n_pairs = the reference frame alone
     float2 *stats;                // [frame][event] {mean, sum of squares of the mean-removed image}
     float2 *t1, *t2, *fref;       // scratch
-    long long t1_frame, t2_frame; // float2 per frame of T1 / T2
+    long long t1_frame, t2_frame; // float2 per packed image of T1 / T2
     const float2 *tw;             // twiddles exp(-2 pi i k / 1024), k < 1024
     float4 *per_event;            // [frame][event] {d_lat px, d_ax px, ncc, 0}
     float4 *motion;               // [frame] {dx, dy, dz (m), mean ncc}
@@ -188,8 +191,8 @@ __global__ void __launch_bounds__(kMoThreads) motion_stats_kernel(const __grid_c
 
 // depth FFT of the CTA's 32 lateral lines (one warp per line, 4 lines per warp) into the shared-memory tile s[line][position]
 template <int LOGR>
-__device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int rs, const float2 *x, int n_lat, int n_ax, int l0,
-                                               float mean, int warp, int lane) {
+__device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int rs, const float2 *xa, const float2 *xb, int n_lat,
+                                               int n_ax, int l0, float mean_a, float mean_b, int warp, int lane) {
     constexpr int R = 1 << LOGR;
     for (int li = warp; li < kMoLines; li += kMoThreads / 32) {
         const int l = l0 + li;
@@ -198,9 +201,13 @@ __device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int i = 32 * r + lane;
-            float a = 0.f;
-            if (i < n_ax) { const float2 c = __ldg(x + (long long)l * n_ax + i); a = sqrtf(c.x * c.x + c.y * c.y) - mean; }
-            v[r] = make_float2(a, 0.f);
+            float a = 0.f, b = 0.f;
+            if (i < n_ax) {
+                const float2 c = __ldg(xa + (long long)l * n_ax + i);
+                a = sqrtf(c.x * c.x + c.y * c.y) - mean_a;
+                if (xb) { const float2 d = __ldg(xb + (long long)l * n_ax + i); b = sqrtf(d.x * d.x + d.y * d.y) - mean_b; }
+            }
+            v[r] = make_float2(a, b);
         }
         mo_fft_dif<LOGR, -1>(v, P.tw, lane);
 #pragma unroll
@@ -208,25 +215,30 @@ __device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int
     }
 }
 
-// grid = (lateral tiles of 32 lines, events, frames)
+// grid = (lateral tiles of 32 lines, events, packed images + 1): image p < n_pairs = frames (2 p, 2 p + 1) as real and
+// imaginary part (the correlation with the fixed reference is linear in the frame, so the whole transform chain runs once
+// for two frames and the real / imaginary part of the result is the correlation map of the first / second one); image
+// n_pairs = the reference frame alone (its spectrum is the other factor and must stay unmixed)
 __global__ void __launch_bounds__(kMoThreads) motion_fwd_z_kernel(const __grid_constant__ MoParams P) {
     extern __shared__ __align__(16) unsigned char mo_smem[];
-    const int e = blockIdx.y, f = blockIdx.z;
+    const int e = blockIdx.y, img = blockIdx.z;
+    const int fa = img < P.n_pairs ? 2 * img : P.ref_frame, fb = (img < P.n_pairs && 2 * img + 1 < P.n_frames) ? 2 * img + 1 : -1;
     const int n_lat = P.ev.n_lat[e], n_ax = P.ev.n_ax[e], log2_ = P.ev.log2[e], n2 = 1 << log2_;
     const int l0 = blockIdx.x * kMoLines;
     if (l0 >= n_lat) return;
     float2 *s = reinterpret_cast<float2 *>(mo_smem);                  // [32][n2 + 1]
     const int rs = n2 + 1;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const float mean = P.stats[(long long)f * P.n_events + e].x;
-    const float2 *x = P.x + (long long)f * P.frame_stride + P.ev.off[e];
-#define ULM_MO_CALL(LR) mo_fwd_z_lines<LR>(P, s, rs, x, n_lat, n_ax, l0, mean, warp, lane)
+    const float mean_a = P.stats[(long long)fa * P.n_events + e].x, mean_b = fb >= 0 ? P.stats[(long long)fb * P.n_events + e].x : 0.f;
+    const float2 *xa = P.x + (long long)fa * P.frame_stride + P.ev.off[e];
+    const float2 *xb = fb >= 0 ? P.x + (long long)fb * P.frame_stride + P.ev.off[e] : nullptr;
+#define ULM_MO_CALL(LR) mo_fwd_z_lines<LR>(P, s, rs, xa, xb, n_lat, n_ax, l0, mean_a, mean_b, warp, lane)
     ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
 #undef ULM_MO_CALL
     __syncthreads();
-    // transposed, coalesced write: T1[frame][event block][kz position][l]  (kz in the permuted order of mo_fft_dif: every
+    // transposed, coalesced write: T1[image][event block][kz position][l]  (kz in the permuted order of mo_fft_dif: every
     // later pass treats the kz rows independently and the final inverse depth transform takes exactly that order)
-    float2 *t1 = P.t1 + (long long)f * P.t1_frame + P.ev.t1_off[e];
+    float2 *t1 = P.t1 + (long long)img * P.t1_frame + P.ev.t1_off[e];
     const int n_lat_p = (n_lat + 31) / 32 * 32;
     for (int kz = warp; kz < n2; kz += kMoThreads / 32)
         t1[(long long)kz * n_lat_p + l0 + lane] = (l0 + lane < n_lat) ? s[lane * rs + kz] : make_float2(0.f, 0.f);
@@ -263,11 +275,11 @@ __device__ __forceinline__ void mo_lat_rows(const MoParams &P, float2 *s, int rs
     }
 }
 
-// grid = (kz tiles of 32 rows, events, frames [REF: 1])
+// grid = (kz tiles of 32 rows, events, packed images [REF: 1, the reference image])
 template <bool REF>
 __global__ void __launch_bounds__(kMoThreads) motion_lat_kernel(const __grid_constant__ MoParams P) {
     extern __shared__ __align__(16) unsigned char mo_smem[];
-    const int e = blockIdx.y, f = REF ? P.ref_frame : blockIdx.z;
+    const int e = blockIdx.y, img = REF ? P.n_pairs : blockIdx.z;
     const int n_lat = P.ev.n_lat[e], log1 = P.ev.log1[e], n1 = 1 << log1, n2 = 1 << P.ev.log2[e];
     const int kz0 = blockIdx.x * kMoLines;
     if (kz0 >= n2) return;
@@ -275,106 +287,122 @@ __global__ void __launch_bounds__(kMoThreads) motion_lat_kernel(const __grid_con
     float2 *s = reinterpret_cast<float2 *>(mo_smem);                  // [32][n1 + 1]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_lat_p = (n_lat + 31) / 32 * 32;
-    const float2 *t1 = P.t1 + (long long)f * P.t1_frame + P.ev.t1_off[e];
+    const float2 *t1 = P.t1 + (long long)img * P.t1_frame + P.ev.t1_off[e];
     float2 *fref = P.fref + P.ev.ref_off[e];
 #define ULM_MO_CALL(LR) mo_lat_rows<LR, REF>(P, s, rs, t1, fref, n_lat, n_lat_p, n1, kz0, warp, lane)
     ULM_MO_DISPATCH(log1, ULM_MO_CALL)
 #undef ULM_MO_CALL
     if (REF) return;
     __syncthreads();
-    // transposed, coalesced write: T2[frame][event block][dl][kz position]
-    float2 *t2 = P.t2 + (long long)f * P.t2_frame + P.ev.t2_off[e];
+    // transposed, coalesced write: T2[image][event block][dl][kz position]
+    float2 *t2 = P.t2 + (long long)img * P.t2_frame + P.ev.t2_off[e];
     for (int dl = warp; dl < n1; dl += kMoThreads / 32) t2[(long long)dl * n2 + kz0 + lane] = s[lane * rs + dl];
 }
 
-// running maximum of c over the lateral-shift lines of one warp: inverse depth FFT of each line in registers, real parts
-// to the warp's row in shared memory (the depth neighbours of a new maximum are read from it)
+// running maxima of the two correlation maps (real part: first frame of the image, imaginary part: second frame) over the
+// lateral-shift lines of one warp: inverse depth FFT of each line in registers, the values to the warp's rows in shared
+// memory (the depth neighbours of a new maximum are read from them)
 struct MoBest { float val, m, p; int idx; };
+__device__ __forceinline__ void mo_best_update(MoBest &B, const float *row, float best, int bi, int dl, int n2) {
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+    }
+    const int idx = dl * n2 + bi;
+    if (best > B.val || (best == B.val && idx < B.idx)) {
+        B.val = best; B.idx = idx;
+        B.m = row[(bi + n2 - 1) & (n2 - 1)];
+        B.p = row[(bi + 1) & (n2 - 1)];
+    }
+}
 template <int LOGR>
-__device__ __forceinline__ void mo_peak_lines(const MoParams &P, float *row, const float2 *t2, int n1, int n2, int warp, int lane,
-                                              MoBest &B) {
+__device__ __forceinline__ void mo_peak_lines(const MoParams &P, float *row_a, float *row_b, const float2 *t2, int n1, int n2,
+                                              int warp, int lane, MoBest &Ba, MoBest &Bb) {
     constexpr int R = 1 << LOGR;
     for (int dl = warp; dl < n1; dl += kMoThreads / 32) {
         float2 v[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = __ldg(t2 + (long long)dl * n2 + 32 * q + lane);
         mo_fft_dit<LOGR, +1>(v, P.tw, lane);
-        float best = -3.0e38f;
-        int bi = 0;
+        float best_a = -3.0e38f, best_b = -3.0e38f;
+        int bi_a = 0, bi_b = 0;
 #pragma unroll
         for (int r = 0; r < R; ++r) {                                  // depth shift 32 r + lane, ascending: first maximum
-            row[32 * r + lane] = v[r].x;
-            if (v[r].x > best) { best = v[r].x; bi = 32 * r + lane; }
-        }
-        for (int o = 16; o > 0; o >>= 1) {
-            const float ov = __shfl_xor_sync(0xffffffffu, best, o);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+            row_a[32 * r + lane] = v[r].x;
+            row_b[32 * r + lane] = v[r].y;
+            if (v[r].x > best_a) { best_a = v[r].x; bi_a = 32 * r + lane; }
+            if (v[r].y > best_b) { best_b = v[r].y; bi_b = 32 * r + lane; }
         }
         __syncwarp();
-        const int idx = dl * n2 + bi;
-        if (best > B.val || (best == B.val && idx < B.idx)) {
-            B.val = best; B.idx = idx;
-            B.m = row[(bi + n2 - 1) & (n2 - 1)];
-            B.p = row[(bi + 1) & (n2 - 1)];
-        }
+        mo_best_update(Ba, row_a, best_a, bi_a, dl, n2);
+        mo_best_update(Bb, row_b, best_b, bi_b, dl, n2);
         __syncwarp();
     }
 }
 
-// c(dl, dz) by one direct inverse DFT sum over the (permuted) kz positions of line dl: Re sum_kz T2[dl][pos] exp(+2 pi i kz dz / n2)
+// c(dl, dz) by one direct inverse DFT sum over the (permuted) kz positions of line dl:
+// sum_kz T2[dl][pos] exp(+2 pi i kz dz / n2)  (real part: first frame, imaginary part: second frame)
 template <int LOGR>
-__device__ __forceinline__ float mo_direct(const MoParams &P, const float2 *t2, int dl, int dz, int n2, int lane) {
-    float acc = 0.f;
+__device__ __forceinline__ float2 mo_direct(const MoParams &P, const float2 *t2, int dl, int dz, int n2, int lane) {
+    float ar = 0.f, ai = 0.f;
     for (int pos = lane; pos < n2; pos += 32) {
         const int kz = mo_perm<LOGR>(pos >> 5, pos & 31);
         const float2 v = __ldg(t2 + (long long)dl * n2 + pos);
         const float2 w = __ldg(P.tw + ((kz * dz) & (n2 - 1)) * (32 >> LOGR));      // exp(-2 pi i kz dz / n2); the inverse uses its conjugate
-        acc += v.x * w.x + v.y * w.y;                                                  // Re(v conj(w))
+        ar += v.x * w.x + v.y * w.y;                                                   // v conj(w)
+        ai += v.y * w.x - v.x * w.y;
     }
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    return acc;
+    for (int o = 16; o > 0; o >>= 1) { ar += __shfl_xor_sync(0xffffffffu, ar, o); ai += __shfl_xor_sync(0xffffffffu, ai, o); }
+    return make_float2(ar, ai);
 }
 
-// grid = (events, frames): inverse FFT along depth of every lateral-shift line, running maximum, sub-pixel peak
+// grid = (events, packed images): inverse FFT along depth of every lateral-shift line, running maxima, sub-pixel peaks of
+// the image's two frames
 __global__ void __launch_bounds__(kMoThreads) motion_peak_kernel(const __grid_constant__ MoParams P) {
-    __shared__ float rows[kMoThreads / 32][kMoMaxN];
-    __shared__ float b_val[kMoThreads / 32], b_m[kMoThreads / 32], b_p[kMoThreads / 32];
-    __shared__ int b_idx[kMoThreads / 32];
-    __shared__ float nb[2];
-    const int e = blockIdx.x, f = blockIdx.y;
+    __shared__ float rows[kMoThreads / 32][2][kMoMaxN];
+    __shared__ float b_val[2][kMoThreads / 32], b_m[2][kMoThreads / 32], b_p[2][kMoThreads / 32];
+    __shared__ int b_idx[2][kMoThreads / 32];
+    __shared__ float nb[2][2];
+    const int e = blockIdx.x, img = blockIdx.y;
     const int log1 = P.ev.log1[e], log2_ = P.ev.log2[e], n1 = 1 << log1, n2 = 1 << log2_;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const float2 *t2 = P.t2 + (long long)f * P.t2_frame + P.ev.t2_off[e];
-    MoBest B{-3.0e38f, 0.f, 0.f, 0x7fffffff};
-#define ULM_MO_CALL(LR) mo_peak_lines<LR>(P, rows[warp], t2, n1, n2, warp, lane, B)
+    const float2 *t2 = P.t2 + (long long)img * P.t2_frame + P.ev.t2_off[e];
+    MoBest B[2] = {{-3.0e38f, 0.f, 0.f, 0x7fffffff}, {-3.0e38f, 0.f, 0.f, 0x7fffffff}};
+#define ULM_MO_CALL(LR) mo_peak_lines<LR>(P, rows[warp][0], rows[warp][1], t2, n1, n2, warp, lane, B[0], B[1])
     ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
 #undef ULM_MO_CALL
-    if (lane == 0) { b_val[warp] = B.val; b_idx[warp] = B.idx; b_m[warp] = B.m; b_p[warp] = B.p; }
+    if (lane == 0)
+        for (int h = 0; h < 2; ++h) { b_val[h][warp] = B[h].val; b_idx[h][warp] = B[h].idx; b_m[h][warp] = B[h].m; b_p[h][warp] = B[h].p; }
     __syncthreads();
-    int w_best = 0;
-    for (int w = 1; w < kMoThreads / 32; ++w)
-        if (b_val[w] > b_val[w_best] || (b_val[w] == b_val[w_best] && b_idx[w] < b_idx[w_best])) w_best = w;
-    const float c0 = b_val[w_best], cm2 = b_m[w_best], cp2 = b_p[w_best];
-    const int pk = b_idx[w_best], dl_pk = pk / n2, dz_pk = pk - dl_pk * n2;
-    // the lateral neighbours c(dl +- 1, dz) (warps 0 and 1)
-    if (warp < 2) {
-        const int dl = (dl_pk + (warp == 0 ? n1 - 1 : 1)) & (n1 - 1);
-        float acc = 0.f;
+    int w_best[2] = {0, 0};
+    for (int h = 0; h < 2; ++h)
+        for (int w = 1; w < kMoThreads / 32; ++w)
+            if (b_val[h][w] > b_val[h][w_best[h]] || (b_val[h][w] == b_val[h][w_best[h]] && b_idx[h][w] < b_idx[h][w_best[h]])) w_best[h] = w;
+    // the lateral neighbours c(dl +- 1, dz) of either frame's peak (warps 0, 1: first frame; warps 2, 3: second frame)
+    if (warp < 4) {
+        const int h = warp >> 1, pk = b_idx[h][w_best[h]], dl_pk = pk / n2, dz_pk = pk - dl_pk * n2;
+        const int dl = (dl_pk + ((warp & 1) == 0 ? n1 - 1 : 1)) & (n1 - 1);
+        float2 acc = make_float2(0.f, 0.f);
 #define ULM_MO_CALL(LR) acc = mo_direct<LR>(P, t2, dl, dz_pk, n2, lane)
         ULM_MO_DISPATCH(log2_, ULM_MO_CALL)
 #undef ULM_MO_CALL
-        if (lane == 0) nb[warp] = acc;
+        if (lane == 0) nb[h][warp & 1] = h ? acc.y : acc.x;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        const float2 sf = P.stats[(long long)f * P.n_events + e], sr = P.stats[(long long)P.ref_frame * P.n_events + e];
-        const float den = sqrtf(sf.y) * sqrtf(sr.y) * (float)n1 * (float)n2;
-        const float inv = den > 0.f ? 1.f / den : 0.f;
-        auto parab = [](float m, float c, float p) { const float d = m - 2.f * c + p; return d == 0.f ? 0.f : 0.5f * (m - p) / d; };
-        const float d1 = parab(nb[0], c0, nb[1]), d2 = parab(cm2, c0, cp2);
-        const int s1 = dl_pk < n1 / 2 ? dl_pk : dl_pk - n1, s2 = dz_pk < n2 / 2 ? dz_pk : dz_pk - n2;
-        P.per_event[(long long)f * P.n_events + e] = make_float4((float)s1 + d1, (float)s2 + d2, c0 * inv, 0.f);
+    if (threadIdx.x < 2) {
+        const int h = threadIdx.x, f = 2 * img + h;
+        if (f < P.n_frames) {
+            const float c0 = b_val[h][w_best[h]], cm2 = b_m[h][w_best[h]], cp2 = b_p[h][w_best[h]];
+            const int pk = b_idx[h][w_best[h]], dl_pk = pk / n2, dz_pk = pk - dl_pk * n2;
+            const float2 sf = P.stats[(long long)f * P.n_events + e], sr = P.stats[(long long)P.ref_frame * P.n_events + e];
+            const float den = sqrtf(sf.y) * sqrtf(sr.y) * (float)n1 * (float)n2;
+            const float inv = den > 0.f ? 1.f / den : 0.f;
+            auto parab = [](float m, float c, float p) { const float d = m - 2.f * c + p; return d == 0.f ? 0.f : 0.5f * (m - p) / d; };
+            const float d1 = parab(nb[h][0], c0, nb[h][1]), d2 = parab(cm2, c0, cp2);
+            const int s1 = dl_pk < n1 / 2 ? dl_pk : dl_pk - n1, s2 = dz_pk < n2 / 2 ? dz_pk : dz_pk - n2;
+            P.per_event[(long long)f * P.n_events + e] = make_float4((float)s1 + d1, (float)s2 + d2, c0 * inv, 0.f);
+        }
     }
 }
 

@@ -60,8 +60,9 @@ inline const char *motion_build(MotionPlan &M, const std::vector<long long> &off
         !up(&M.d_t1off, t1off) || !up(&M.d_t2off, t2off) || !up(&M.d_refoff, refoff) || !up(&M.tw, tw))
         return "table upload failed";
     if (cudaMalloc(&M.stats, (size_t)max_frames * M.n_events * sizeof(float2)) != cudaSuccess ||
-        cudaMalloc(&M.t1, (size_t)max_frames * M.t1_frame * sizeof(float2)) != cudaSuccess ||
-        cudaMalloc(&M.t2, (size_t)max_frames * M.t2_frame * sizeof(float2)) != cudaSuccess ||
+        // packed images: two frames each, + the reference frame alone (T1 only)
+        cudaMalloc(&M.t1, (size_t)((max_frames + 1) / 2 + 1) * M.t1_frame * sizeof(float2)) != cudaSuccess ||
+        cudaMalloc(&M.t2, (size_t)((max_frames + 1) / 2) * M.t2_frame * sizeof(float2)) != cudaSuccess ||
         cudaMalloc(&M.fref, (size_t)M.ref_total * sizeof(float2)) != cudaSuccess ||
         cudaMalloc(&M.per_event, (size_t)max_frames * M.n_events * sizeof(float4)) != cudaSuccess)
         return "scratch allocation failed";
@@ -84,7 +85,7 @@ inline cudaError_t motion_launch(const MotionPlan &M, const float2 *x, int n_fra
     P.ev = MoEvents{static_cast<const long long *>(M.d_off), static_cast<const int *>(M.d_nlat), static_cast<const int *>(M.d_nax),
                     static_cast<const int *>(M.d_log1), static_cast<const int *>(M.d_log2), static_cast<const long long *>(M.d_t1off),
                     static_cast<const long long *>(M.d_t2off), static_cast<const long long *>(M.d_refoff)};
-    P.n_events = M.n_events; P.n_frames = n_frames; P.ref_frame = ref_frame;
+    P.n_events = M.n_events; P.n_frames = n_frames; P.ref_frame = ref_frame; P.n_pairs = (n_frames + 1) / 2;
     P.stats = static_cast<float2 *>(M.stats); P.t1 = static_cast<float2 *>(M.t1); P.t2 = static_cast<float2 *>(M.t2);
     P.fref = static_cast<float2 *>(M.fref); P.t1_frame = M.t1_frame; P.t2_frame = M.t2_frame; P.tw = static_cast<const float2 *>(M.tw);
     P.per_event = static_cast<float4 *>(M.per_event); P.motion = motion; P.n_row_tx = M.n_row_tx;
@@ -92,10 +93,10 @@ inline cudaError_t motion_launch(const MotionPlan &M, const float2 *x, int n_fra
     const int smem1 = kMoLines * (M.max_n2 + 1) * 8, smem2 = kMoLines * (M.max_n1 + 1) * 8;
     if (M.ev[0] && (e = cudaEventRecord(M.ev[0], st)) != cudaSuccess) return e;
     motion_stats_kernel<<<dim3(M.n_events, n_frames), kMoThreads, 0, st>>>(P);
-    motion_fwd_z_kernel<<<dim3(M.max_lat_tiles, M.n_events, n_frames), kMoThreads, smem1, st>>>(P);
+    motion_fwd_z_kernel<<<dim3(M.max_lat_tiles, M.n_events, P.n_pairs + 1), kMoThreads, smem1, st>>>(P);
     motion_lat_kernel<true><<<dim3(M.max_kz_tiles, M.n_events, 1), kMoThreads, smem2, st>>>(P);
-    motion_lat_kernel<false><<<dim3(M.max_kz_tiles, M.n_events, n_frames), kMoThreads, smem2, st>>>(P);
-    motion_peak_kernel<<<dim3(M.n_events, n_frames), kMoThreads, 0, st>>>(P);
+    motion_lat_kernel<false><<<dim3(M.max_kz_tiles, M.n_events, P.n_pairs), kMoThreads, smem2, st>>>(P);
+    motion_peak_kernel<<<dim3(M.n_events, P.n_pairs), kMoThreads, 0, st>>>(P);
     motion_combine_kernel<<<(n_frames + 127) / 128, 128, 0, st>>>(P);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (M.ev[1] && (e = cudaEventRecord(M.ev[1], st)) != cudaSuccess) return e;
