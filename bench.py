@@ -558,13 +558,13 @@ def run_motion(args):
             m_host = m2.cpu()
         e2e_ms = (time.perf_counter() - t0) * 1e3 / 2
         per = per.cpu().numpy()
-    # HBM roofline: bytes the six kernels must move (slices read three times: two statistics passes and the forward
+    # HBM roofline: bytes the six kernels must move (slices read twice: the statistics pass and the forward
     # transform; T1 and T2 written and read once each per PACKED image = two frames) vs the minimum (slices read once);
     # flops: 2 two-dimensional 256 x 256 transforms per packed image (forward, inverse), 5 N log2 N each
     n_img = ((n_frames + 1) // 2) * len(shapes)
     fft_flop = 2 * 5.0 * (256 * 256) * 16 * n_img
     bytes_min = float(d.numel() * 8)
-    bytes_moved = float(d.numel() * 8 * 3 + n_img * (256 * 192 * 8 * 2 + 256 * 256 * 8 * 2))
+    bytes_moved = float(d.numel() * 8 * 2 + n_img * (256 * 192 * 8 * 2 + 256 * 256 * 8 * 2))
     peak_hbm, hbm_src = hbm_peak()
     cpu = None
     if not args.no_cpu_baseline:

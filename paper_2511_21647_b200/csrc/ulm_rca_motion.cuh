@@ -12,7 +12,7 @@
 // shuffles; forward = decimation in frequency, inverse = the same network backwards, so no bit-reversal pass exists),
 // every pass over global memory coalesced, and the product with the reference spectrum and the inverse lateral
 // transform fused into the forward lateral pass:
-//   motion_stats_kernel     mean and mean-removed energy of every B-mode image
+//   motion_stats_kernel     mean and mean-removed energy of every B-mode image (one pass)
 //   motion_fwd_z_kernel     FFT along depth of 32 lateral lines per CTA, written transposed  T1[img][kz][l]; an image =
 //                           TWO frames, (a_2p, a_2p+1) as real / imaginary part: correlating with the fixed reference is
 //                           linear in the frame, so Re / Im of the final map are the two frames' correlation maps
@@ -164,29 +164,41 @@ __device__ __forceinline__ void mo_fft_dit(float2 (&v)[1 << LOGR], const float2 
         default: call(4); break;                       \
     }
 
+// One pass over the image: sums of (a - c) and (a - c)^2 with the pilot value c = a[0] (a large common offset of the
+// image then cancels before the squares are taken); mean = c + S1 / n, mean-removed energy = S2 - S1^2 / n.
 __global__ void __launch_bounds__(kMoThreads) motion_stats_kernel(const __grid_constant__ MoParams P) {
     const int e = blockIdx.x, f = blockIdx.y;
     const int n = P.ev.n_lat[e] * P.ev.n_ax[e];
     const float2 *x = P.x + (long long)f * P.frame_stride + P.ev.off[e];
-    __shared__ float red[kMoThreads / 32];
-    __shared__ float s_mean;
-    auto block_sum = [&](float v) {
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        __syncthreads();
-        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-        __syncthreads();
-        float t = 0.f;
-        for (int i = 0; i < kMoThreads / 32; ++i) t += red[i];
-        return t;
-    };
-    float s = 0.f;
-    for (int i = threadIdx.x; i < n; i += kMoThreads) { const float2 v = __ldg(x + i); s += sqrtf(v.x * v.x + v.y * v.y); }
-    const float mean = block_sum(s) / (float)n;
-    float q = 0.f;
-    for (int i = threadIdx.x; i < n; i += kMoThreads) { const float2 v = __ldg(x + i); const float d = sqrtf(v.x * v.x + v.y * v.y) - mean; q += d * d; }
-    const float ss = block_sum(q);
-    if (threadIdx.x == 0) P.stats[(long long)f * P.n_events + e] = make_float2(mean, ss);
-    (void)s_mean;
+    __shared__ float red[2][kMoThreads / 32];
+    const float2 x0 = __ldg(x);
+    const float c = sqrtf(x0.x * x0.x + x0.y * x0.y);
+    float s1 = 0.f, s2 = 0.f;
+    auto add = [&](float re, float im) { const float d = sqrtf(re * re + im * im) - c; s1 += d; s2 = fmaf(d, d, s2); };
+    if ((reinterpret_cast<unsigned long long>(x) & 15ull) == 0) {
+        const float4 *x4 = reinterpret_cast<const float4 *>(x);
+        const int n4 = n >> 1;
+        int i = threadIdx.x;
+        for (; i + 3 * kMoThreads < n4; i += 4 * kMoThreads) {
+            float4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = __ldg(x4 + i + u * kMoThreads);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { add(v[u].x, v[u].y); add(v[u].z, v[u].w); }
+        }
+        for (; i < n4; i += kMoThreads) { const float4 v = __ldg(x4 + i); add(v.x, v.y); add(v.z, v.w); }
+        if ((n & 1) && threadIdx.x == 0) { const float2 v = __ldg(x + n - 1); add(v.x, v.y); }
+    } else {
+        for (int i = threadIdx.x; i < n; i += kMoThreads) { const float2 v = __ldg(x + i); add(v.x, v.y); }
+    }
+    for (int o = 16; o > 0; o >>= 1) { s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o); }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = s1; red[1][threadIdx.x >> 5] = s2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float t1 = 0.f, t2 = 0.f;
+        for (int i = 0; i < kMoThreads / 32; ++i) { t1 += red[0][i]; t2 += red[1][i]; }
+        P.stats[(long long)f * P.n_events + e] = make_float2(c + t1 / (float)n, fmaxf(t2 - t1 * t1 / (float)n, 0.f));
+    }
 }
 
 // depth FFT of the CTA's 32 lateral lines (one warp per line, 4 lines per warp) into the shared-memory tile s[line][position]
