@@ -23,8 +23,8 @@
 //
 // Kernel mapping: CTA = (frame, plane set, 32 lateral positions, block of 8 groups), walking the depth tiles of 16
 // depths; warp = one group m, lane = one lateral position, thread = 2 chunks of 8 consecutive depths (a register window
-// of 8 + NT - 1 slice values per chunk feeds 8 NT complex multiply-adds as FFMA2).  A stage = the slice tile of one
-// event (zero-extended halo included), brought in with 8-byte LDGSTS two stages ahead through three buffers (one
+// of 8 + NT - 1 slice values per chunk feeds 8 NT complex multiply-adds as FFMA2).  A stage = the slice tiles of two
+// events (zero-extended halo included), brought in with 8-byte LDGSTS two stages ahead through three buffers (one
 // barrier per stage); the stage stream runs across depth-tile boundaries; rows are padded to an odd stride so the 32
 // lanes of a warp read 32 different bank pairs.
 #pragma once
@@ -37,6 +37,7 @@ namespace ulm {
 constexpr int kS2Lat = 32;        // lateral positions per CTA (= lanes)
 constexpr int kS2Chunks = 2;      // chunks of 8 depths per thread
 constexpr int kS2Stages = 3;      // shared-memory buffers of the asynchronous tile pipeline
+constexpr int kS2Ev = 2;          // events per stage (one barrier per stage)
 constexpr int kS2Zt = 8 * kS2Chunks;
 constexpr int kS2Warps = 8;       // groups per CTA
 constexpr int kS2Threads = 32 * kS2Warps;
@@ -153,10 +154,12 @@ __global__ void __launch_bounds__(kS2Threads, 2) stage2_project_kernel(const __g
     const int lat = min(lat0 + lane, n_lat - 1);
     const int ncol = P.ncol, rs = P.rs, n_z = P.n_z;
     const int own_n = ULM_S2(own_n), cross_n = ULM_S2(cross_n);
-    const int n_st = own_n + cross_n;                              // stages of a depth tile: own events, then cross events
-    // shared memory: kS2Stages buffers of {own slice tile [kS2Lat][rs], group-sum tile [kS2Warps][ncol]}, then the tap
+    // stages of a depth tile: the own events kS2Ev at a time, then the cross events kS2Ev at a time
+    const int st_own = (own_n + kS2Ev - 1) / kS2Ev, n_st = st_own + (cross_n + kS2Ev - 1) / kS2Ev;
+    // shared memory: kS2Stages buffers of {kS2Ev own slice tiles [kS2Lat][rs], kS2Ev group-sum tiles [kS2Warps][ncol]}, then the tap
     // tables: own [own_n][kS2Warps][1 + NT] float2 ({offset bits, -}, taps), cross [cross_n][kS2Lat][3] float2
-    const int buf_elems = kS2Lat * rs + kS2Warps * ncol;
+    const int own_tile = kS2Lat * rs, gs_tile = kS2Warps * ncol;
+    const int buf_elems = kS2Ev * (own_tile + gs_tile);
     float2 *smem = reinterpret_cast<float2 *>(s2_smem);
     float2 *tab_own = smem + kS2Stages * buf_elems;
     float2 *tab_cross = tab_own + own_n * kS2Warps * (1 + NT);
@@ -198,7 +201,7 @@ __global__ void __launch_bounds__(kS2Threads, 2) stage2_project_kernel(const __g
     const float2 *row_c = P.gsum + ((long long)f * P.n_events + ULM_S2(cross_goff)) * P.g_max * n_z +
                           (long long)min(m, n_g - 1) * n_z + lane;
     const long long step_o = (long long)n_lat * n_z, step_c = (long long)P.g_max * n_z;
-    const uint32_t dst_o = (uint32_t)(frow * rs + fcl) * 8u, dst_c = (uint32_t)(kS2Lat * rs + warp * ncol + lane) * 8u;
+    const uint32_t dst_o = (uint32_t)(frow * rs + fcl) * 8u, dst_c = (uint32_t)(kS2Ev * own_tile + warp * ncol + lane) * 8u;
     int zt_issue = zt_begin, s_issue = 0;
     uint32_t buf_issue = smem_u;
     const float2 *src_o = row_o, *src_c = row_c;
@@ -221,22 +224,34 @@ __global__ void __launch_bounds__(kS2Threads, 2) stage2_project_kernel(const __g
     uint32_t zero_o = 0, zero_c = 0;
     auto issue = [&]() {
         if (zt_issue < zt_end) {
-            if (s_issue < own_n) {
+            if (s_issue < st_own) {
 #pragma unroll
-                for (int r = 0; r < RO; ++r)
-                    if (in_o & (1u << r)) s2_cp_async8(buf_issue + dst_o + r * 64u, src_o + 8 * r, true);
-                if (zero_o)
-                    for (int r = 0; r < RO; ++r)
-                        if (zero_o & (1u << r)) smem[(buf_issue - smem_u + dst_o) / 8u + 8 * r] = make_float2(0.f, 0.f);
-                src_o += step_o;
+                for (int u = 0; u < kS2Ev; ++u) {
+                    if (s_issue * kS2Ev + u < own_n) {
+                        const uint32_t d = buf_issue + dst_o + (uint32_t)(u * own_tile) * 8u;
+#pragma unroll
+                        for (int r = 0; r < RO; ++r)
+                            if (in_o & (1u << r)) s2_cp_async8(d + r * 64u, src_o + 8 * r, true);
+                        if (zero_o)
+                            for (int r = 0; r < RO; ++r)
+                                if (zero_o & (1u << r)) smem[(d - smem_u) / 8u + 8 * r] = make_float2(0.f, 0.f);
+                        src_o += step_o;
+                    }
+                }
             } else {
 #pragma unroll
-                for (int r = 0; r < RC; ++r)
-                    if (in_c & (1u << r)) s2_cp_async8(buf_issue + dst_c + r * 256u, src_c + 32 * r, true);
-                if (zero_c)
-                    for (int r = 0; r < RC; ++r)
-                        if (zero_c & (1u << r)) smem[(buf_issue - smem_u + dst_c) / 8u + 32 * r] = make_float2(0.f, 0.f);
-                src_c += step_c;
+                for (int u = 0; u < kS2Ev; ++u) {
+                    if ((s_issue - st_own) * kS2Ev + u < cross_n) {
+                        const uint32_t d = buf_issue + dst_c + (uint32_t)(u * gs_tile) * 8u;
+#pragma unroll
+                        for (int r = 0; r < RC; ++r)
+                            if (in_c & (1u << r)) s2_cp_async8(d + r * 256u, src_c + 32 * r, true);
+                        if (zero_c)
+                            for (int r = 0; r < RC; ++r)
+                                if (zero_c & (1u << r)) smem[(d - smem_u) / 8u + 32 * r] = make_float2(0.f, 0.f);
+                        src_c += step_c;
+                    }
+                }
             }
             if (++s_issue == n_st) {
                 s_issue = 0;
@@ -272,45 +287,57 @@ __global__ void __launch_bounds__(kS2Threads, 2) stage2_project_kernel(const __g
             __syncthreads();                       // this stage has landed; every warp is done with the previous one
             issue();                               // refills the buffer the previous stage used
             if (m_ok) {
-                if (s < own_n) {
-                    const float2 *tb = tab_own + (s * kS2Warps + warp) * (1 + NT);
-                    const int o = __float_as_int(tb[0].x);
-                    unsigned long long WR[NT], WI[NT];
+                if (s < st_own) {
 #pragma unroll
-                    for (int t2 = 0; t2 < NT; ++t2) { const float2 w = tb[1 + t2]; WR[t2] = s2_pack(w.x, w.x); WI[t2] = s2_pack(w.y, w.y); }
-                    const uint32_t base = buf + (uint32_t)(lane * rs + o) * 8u;
+                    for (int u = 0; u < kS2Ev; ++u) {
+                        const int ev = s * kS2Ev + u;
+                        if (ev < own_n) {
+                            const float2 *tb = tab_own + (ev * kS2Warps + warp) * (1 + NT);
+                            const int o = __float_as_int(tb[0].x);
+                            unsigned long long WR[NT], WI[NT];
 #pragma unroll
-                    for (int c = 0; c < kS2Chunks; ++c) {
-                        unsigned long long win[8 + NT - 1];
+                            for (int t2 = 0; t2 < NT; ++t2) { const float2 w = tb[1 + t2]; WR[t2] = s2_pack(w.x, w.x); WI[t2] = s2_pack(w.y, w.y); }
+                            const uint32_t base = buf + (uint32_t)(u * own_tile + lane * rs + o) * 8u;
 #pragma unroll
-                        for (int q = 0; q < 8 + NT - 1; ++q) win[q] = s2_lds64(base + (c * 8 + q) * 8u);
+                            for (int c = 0; c < kS2Chunks; ++c) {
+                                unsigned long long win[8 + NT - 1];
 #pragma unroll
-                        for (int q = 0; q < 8; ++q)
+                                for (int q = 0; q < 8 + NT - 1; ++q) win[q] = s2_lds64(base + (c * 8 + q) * 8u);
 #pragma unroll
-                            for (int t2 = 0; t2 < NT; ++t2) {
-                                accA[c][q] = s2_ffma2(WR[t2], win[q + t2], accA[c][q]);
-                                accB[c][q] = s2_ffma2(WI[t2], win[q + t2], accB[c][q]);
+                                for (int q = 0; q < 8; ++q)
+#pragma unroll
+                                    for (int t2 = 0; t2 < NT; ++t2) {
+                                        accA[c][q] = s2_ffma2(WR[t2], win[q + t2], accA[c][q]);
+                                        accB[c][q] = s2_ffma2(WI[t2], win[q + t2], accB[c][q]);
+                                    }
                             }
+                        }
                     }
                 } else {
-                    const float2 *tb = tab_cross + ((s - own_n) * kS2Lat + lane) * 3;
-                    const int o = __float_as_int(tb[0].x);
-                    unsigned long long WR[2], WI[2];
 #pragma unroll
-                    for (int t2 = 0; t2 < 2; ++t2) { const float2 w = tb[1 + t2]; WR[t2] = s2_pack(w.x, w.x); WI[t2] = s2_pack(w.y, w.y); }
-                    const uint32_t base = buf + (uint32_t)(kS2Lat * rs + warp * ncol + o) * 8u;
+                    for (int u = 0; u < kS2Ev; ++u) {
+                        const int ev = (s - st_own) * kS2Ev + u;
+                        if (ev < cross_n) {
+                            const float2 *tb = tab_cross + (ev * kS2Lat + lane) * 3;
+                            const int o = __float_as_int(tb[0].x);
+                            unsigned long long WR[2], WI[2];
 #pragma unroll
-                    for (int c = 0; c < kS2Chunks; ++c) {
-                        unsigned long long win[9];
+                            for (int t2 = 0; t2 < 2; ++t2) { const float2 w = tb[1 + t2]; WR[t2] = s2_pack(w.x, w.x); WI[t2] = s2_pack(w.y, w.y); }
+                            const uint32_t base = buf + (uint32_t)(kS2Ev * own_tile + u * gs_tile + warp * ncol + o) * 8u;
 #pragma unroll
-                        for (int q = 0; q < 9; ++q) win[q] = s2_lds64(base + (c * 8 + q) * 8u);
+                            for (int c = 0; c < kS2Chunks; ++c) {
+                                unsigned long long win[9];
 #pragma unroll
-                        for (int q = 0; q < 8; ++q)
+                                for (int q = 0; q < 9; ++q) win[q] = s2_lds64(base + (c * 8 + q) * 8u);
 #pragma unroll
-                            for (int t2 = 0; t2 < 2; ++t2) {
-                                accA[c][q] = s2_ffma2(WR[t2], win[q + t2], accA[c][q]);
-                                accB[c][q] = s2_ffma2(WI[t2], win[q + t2], accB[c][q]);
+                                for (int q = 0; q < 8; ++q)
+#pragma unroll
+                                    for (int t2 = 0; t2 < 2; ++t2) {
+                                        accA[c][q] = s2_ffma2(WR[t2], win[q + t2], accA[c][q]);
+                                        accB[c][q] = s2_ffma2(WI[t2], win[q + t2], accB[c][q]);
+                                    }
                             }
+                        }
                     }
                 }
             }

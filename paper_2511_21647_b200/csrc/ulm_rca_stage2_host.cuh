@@ -64,8 +64,8 @@ inline void shift_of(double w, double ref, double th, double dz, int &n, double 
 
 inline int stage2_smem_bytes(const Stage2Plan &S) {
     const int n_tx_max = std::max(S.n_row_tx, S.n_events - S.n_row_tx);
-    // tile buffers + the CTA's tap tables (own: [events][8 groups][1 + NT], cross: [events][32 positions][3])
-    return (kS2Stages * (kS2Lat * S.rs + kS2Warps * S.ncol) + n_tx_max * kS2Warps * (1 + S.nt) + n_tx_max * kS2Lat * 3) *
+    // tile buffers (kS2Ev events per stage) + the CTA's tap tables (own: [events][8 groups][1 + NT], cross: [events][32 positions][3])
+    return (kS2Stages * kS2Ev * (kS2Lat * S.rs + kS2Warps * S.ncol) + n_tx_max * kS2Warps * (1 + S.nt) + n_tx_max * kS2Lat * 3) *
            (int)sizeof(float2);
 }
 
