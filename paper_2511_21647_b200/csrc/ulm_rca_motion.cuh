@@ -206,21 +206,36 @@ template <int LOGR>
 __device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int rs, const float2 *xa, const float2 *xb, int n_lat,
                                                int n_ax, int l0, float mean_a, float mean_b, int warp, int lane) {
     constexpr int R = 1 << LOGR;
+    // the raw samples of the warp's next line are requested before the transform of the current one
+    float2 ca[R], cb[R];
+    auto fetch = [&](int li) {
+        const int l = l0 + li;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = 32 * r + lane;
+            ca[r] = cb[r] = make_float2(0.f, 0.f);
+            if (l < n_lat && i < n_ax) {
+                ca[r] = __ldg(xa + (long long)l * n_ax + i);
+                if (xb) cb[r] = __ldg(xb + (long long)l * n_ax + i);
+            }
+        }
+    };
+    fetch(warp);
     for (int li = warp; li < kMoLines; li += kMoThreads / 32) {
         const int l = l0 + li;
-        if (l >= n_lat) continue;                                      // warp-uniform; such lines are written as zeros below
         float2 v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int i = 32 * r + lane;
             float a = 0.f, b = 0.f;
             if (i < n_ax) {
-                const float2 c = __ldg(xa + (long long)l * n_ax + i);
-                a = sqrtf(c.x * c.x + c.y * c.y) - mean_a;
-                if (xb) { const float2 d = __ldg(xb + (long long)l * n_ax + i); b = sqrtf(d.x * d.x + d.y * d.y) - mean_b; }
+                a = sqrtf(ca[r].x * ca[r].x + ca[r].y * ca[r].y) - mean_a;
+                if (xb) b = sqrtf(cb[r].x * cb[r].x + cb[r].y * cb[r].y) - mean_b;
             }
             v[r] = make_float2(a, b);
         }
+        if (li + kMoThreads / 32 < kMoLines) fetch(li + kMoThreads / 32);
+        if (l >= n_lat) continue;                                      // warp-uniform; such lines are written as zeros below
         mo_fft_dif<LOGR, -1>(v, P.tw, lane);
 #pragma unroll
         for (int q = 0; q < R; ++q) s[li * rs + 32 * q + lane] = v[q];
@@ -262,14 +277,22 @@ template <int LOGR, bool REF>
 __device__ __forceinline__ void mo_lat_rows(const MoParams &P, float2 *s, int rs, const float2 *t1, float2 *fref, int n_lat,
                                             int n_lat_p, int n1, int kz0, int warp, int lane) {
     constexpr int R = 1 << LOGR;
-    for (int ri = warp; ri < kMoLines; ri += kMoThreads / 32) {
+    float2 nx[R];                                                      // the next row, requested a row ahead
+    auto fetch = [&](int ri) {
         const int kz = kz0 + ri;                                       // n2 is a multiple of 32: always a valid row
-        float2 v[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int l = 32 * r + lane;
-            v[r] = l < n_lat ? __ldg(t1 + (long long)kz * n_lat_p + l) : make_float2(0.f, 0.f);
+            nx[r] = l < n_lat ? __ldg(t1 + (long long)kz * n_lat_p + l) : make_float2(0.f, 0.f);
         }
+    };
+    fetch(warp);
+    for (int ri = warp; ri < kMoLines; ri += kMoThreads / 32) {
+        const int kz = kz0 + ri;
+        float2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = nx[r];
+        if (ri + kMoThreads / 32 < kMoLines) fetch(ri + kMoThreads / 32);
         mo_fft_dif<LOGR, -1>(v, P.tw, lane);
         if (REF) {
 #pragma unroll
@@ -332,10 +355,17 @@ template <int LOGR>
 __device__ __forceinline__ void mo_peak_lines(const MoParams &P, float *row_a, float *row_b, const float2 *t2, int n1, int n2,
                                               int warp, int lane, MoBest &Ba, MoBest &Bb) {
     constexpr int R = 1 << LOGR;
+    float2 nx[R];                                                      // the next line, requested a line ahead
+    auto fetch = [&](int dl) {
+#pragma unroll
+        for (int q = 0; q < R; ++q) nx[q] = __ldg(t2 + (long long)dl * n2 + 32 * q + lane);
+    };
+    if (warp < n1) fetch(warp);
     for (int dl = warp; dl < n1; dl += kMoThreads / 32) {
         float2 v[R];
 #pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = __ldg(t2 + (long long)dl * n2 + 32 * q + lane);
+        for (int q = 0; q < R; ++q) v[q] = nx[q];
+        if (dl + kMoThreads / 32 < n1) fetch(dl + kMoThreads / 32);
         mo_fft_dit<LOGR, +1>(v, P.tw, lane);
         float best_a = -3.0e38f, best_b = -3.0e38f;
         int bi_a = 0, bi_b = 0;
