@@ -246,7 +246,10 @@ __device__ __forceinline__ void mo_fwd_z_lines(const MoParams &P, float2 *s, int
 // imaginary part (the correlation with the fixed reference is linear in the frame, so the whole transform chain runs once
 // for two frames and the real / imaginary part of the result is the correlation map of the first / second one); image
 // n_pairs = the reference frame alone (its spectrum is the other factor and must stay unmixed)
-__global__ void __launch_bounds__(kMoThreads) motion_fwd_z_kernel(const __grid_constant__ MoParams P) {
+#ifndef ULM_MO_FZ
+#define ULM_MO_FZ 2
+#endif
+__global__ void __launch_bounds__(kMoThreads, ULM_MO_FZ) motion_fwd_z_kernel(const __grid_constant__ MoParams P) {
     extern __shared__ __align__(16) unsigned char mo_smem[];
     const int e = blockIdx.y, img = blockIdx.z;
     const int fa = img < P.n_pairs ? 2 * img : P.ref_frame, fb = (img < P.n_pairs && 2 * img + 1 < P.n_frames) ? 2 * img + 1 : -1;
@@ -311,8 +314,11 @@ __device__ __forceinline__ void mo_lat_rows(const MoParams &P, float2 *s, int rs
 }
 
 // grid = (kz tiles of 32 rows, events, packed images [REF: 1, the reference image])
+#ifndef ULM_MO_LAT
+#define ULM_MO_LAT 2
+#endif
 template <bool REF>
-__global__ void __launch_bounds__(kMoThreads) motion_lat_kernel(const __grid_constant__ MoParams P) {
+__global__ void __launch_bounds__(kMoThreads, ULM_MO_LAT) motion_lat_kernel(const __grid_constant__ MoParams P) {
     extern __shared__ __align__(16) unsigned char mo_smem[];
     const int e = blockIdx.y, img = REF ? P.n_pairs : blockIdx.z;
     const int n_lat = P.ev.n_lat[e], log1 = P.ev.log1[e], n1 = 1 << log1, n2 = 1 << P.ev.log2[e];
@@ -401,7 +407,10 @@ __device__ __forceinline__ float2 mo_direct(const MoParams &P, const float2 *t2,
 
 // grid = (events, packed images): inverse FFT along depth of every lateral-shift line, running maxima, sub-pixel peaks of
 // the image's two frames
-__global__ void __launch_bounds__(kMoThreads) motion_peak_kernel(const __grid_constant__ MoParams P) {
+#ifndef ULM_MO_PK
+#define ULM_MO_PK 2
+#endif
+__global__ void __launch_bounds__(kMoThreads, ULM_MO_PK) motion_peak_kernel(const __grid_constant__ MoParams P) {
     __shared__ float rows[kMoThreads / 32][2][kMoMaxN];
     __shared__ float b_val[2][kMoThreads / 32], b_m[2][kMoThreads / 32], b_p[2][kMoThreads / 32];
     __shared__ int b_idx[2][kMoThreads / 32];
