@@ -639,6 +639,41 @@ def _random_case(rng):
     return cfg, nf, extra
 
 
+def test_two_group_items_on_random_shapes(torch_cuda):
+    """The work items of two frame groups against the one-group items of the SAME compact scratch format on seeded
+    random configurations (tile and window planning with 2-row strips, odd last groups, per-angle output, f-number
+    masks, all three pre-pass kernels): a call of 13..45 frames (two-group items, + a one-group launch for an odd last
+    group) must reproduce the same frames beamformed 12 at a time (one-group items; frames keep their 4-frame chunk
+    mates inside full chunks).  What may differ: the order of the fp32 additions (split tail items add their element
+    slices in slice order, and which items are split depends on the item count) and, in a partly filled last chunk, the
+    foreign low mantissa byte of the fp24 mid values (include/ulm_rca.h; bounded at 5e-5 of the image maximum by
+    test_plan_reuse_and_determinism): measured <= 2.3e-5 over 660 seeded shapes, tested at 5e-5 -- three orders of
+    magnitude below what a planning or indexing mistake gives."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    done = 0
+    for it in range(60):
+        rng = np.random.default_rng(9100 + it)
+        cfg, _, extra = _random_case(rng)
+        if cfg.input_kind == 1:
+            continue                          # IQ input is staged as full entries: one-group items only
+        nf = int(rng.integers(13, 46))
+        cfg = cfg.with_(n_frames=nf)
+        ch = synth.random_channel(cfg, nf, seed=int(rng.integers(1 << 30)), amplitude=5000)
+        kw = rounded_kwargs(cfg)
+        with Plan(**kw, max_frames=nf, precision=int(rng.choice([1, 3])), kernel=2) as plan:
+            d_ch = torch.from_numpy(ch).cuda()
+            whole = plan.beamform(d_ch).cpu().numpy()
+            launches = plan.info()["launches_last_call"]
+            parts = np.concatenate([plan.beamform(d_ch[f0:f0 + 12]).cpu().numpy() for f0 in range(0, nf, 12)])
+        scale = np.abs(parts).max()
+        assert scale > 0 and launches >= 2
+        err = np.abs(whole - parts).max() / scale
+        assert err <= 5e-5, (it, nf, err, cfg)
+        done += 1
+    assert done >= 40
+
+
 @pytest.mark.parametrize("block", range(4))
 def test_random_shapes(torch_cuda, block):
     """Seeded random configurations (40 per block) against the oracle with full-precision entries, where only fp32
