@@ -110,7 +110,7 @@ inline cudaError_t clutter_launch(ClutterPlan &C, const float2 *x, int n_t, int 
     CfSplitParams S{};
     S.x = x; S.frame_stride = C.frame_stride; S.ev = ev; S.y_hi = static_cast<__nv_bfloat16 *>(C.y_hi);
     S.y_lo = static_cast<__nv_bfloat16 *>(C.y_lo); S.ld = C.ld; S.n_t = n_t; S.ntp = ntp; S.n_events = C.n_events;
-    clutter_split_kernel<<<dim3((unsigned)((C.k_max + 255) / 256), n_t, C.n_events), 256, 0, st>>>(S);
+    clutter_split_kernel<<<dim3((unsigned)((C.k_max + 2047) / 2048), n_t, C.n_events), 256, 0, st>>>(S);      // 8 pixels per thread
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (C.ev[1] && (e = cudaEventRecord(C.ev[1], st)) != cudaSuccess) return e;
 
