@@ -175,12 +175,16 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [3] kernel in use (1/2)   [4] frames per thread (F)       [5] pixels per tile
  *   [6] window entries per stage (W)  [7] ring stages  [8] tiles per projection (x-z)
  *   [9] dynamic shared memory bytes   [10] kernels launched by the last beamform call
- *   [11] tiles per projection (y-z)   [12] precision in use (1 compact / 2 full)
+ *   [11] tiles per projection (y-z)   [12] precision in use (1 compact-fast / 2 full / 3 compact)
  *   [13] scratch bytes per (sample, frame)   [14] bytes per frame ulm_rca_beamform_host uploads
  *   [15] transmit events beamformed per frame by ulm_rca_beamform after folding (see below; = n_row_tx + n_col_tx
  *        when nothing folds)
  *   [16] Stage 2: depth taps per (event, group) FIR executed by the kernel (0 = Stage 2 not prepared)
- *   [17] Stage 2: columns of the shared-memory slice tile (16 depths + halo) */
+ *   [17] Stage 2: columns of the shared-memory slice tile (16 depths + halo)
+ *   [18] .. [21] the ring kernel's work items of TWO frame groups (24 frames x 2 pixel rows per thread; used by calls
+ *        of more than 12 frames when the scratch holds compact entries; 0 = not planned): window entries per group and
+ *        stage, ring stages (each holds both groups' windows), tiles per projection x-z, y-z
+ * [4] .. [9], [11] describe the work items of one frame group (12 frames x 4 pixel rows per thread). */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 
 /* Mean device time per call of the kernels of the last n_calls (1..64) ulm_rca_beamform calls on this

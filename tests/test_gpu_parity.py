@@ -539,6 +539,7 @@ def test_two_group_work_items(torch_cuda, compound, f_number, precision, frames)
         extra["precision"] = precision
     gpu, ref, info = check_noise(torch_cuda, cfg, ch, plan_extra=extra)
     assert info["kernel"] == 2 and info["precision"] == (precision or 3)
+    assert (info["window_two_groups"] > 0 and info["stages_two_groups"] >= 3) == (info["precision"] != 2)
 
 
 def test_tail_split_of_the_last_round(torch_cuda):
