@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -70,6 +71,10 @@ struct TxTables {
     DeviceBuf n0, f0m;
     DeviceBuf tab;      // the same as {bits of f0m, n0}, [plane][iz][k (kpad)] (volume tables only: das_volume_kernel)
     int kpad = 0;
+    // mirror form (das_volume_mirror_kernel), built when the planes and the angle set are mirror-symmetric
+    DeviceBuf mtab;     // [plane < n_planes / 2][iz][slot (mkpad)]
+    int mkpad = 0, n_mpairs = 0, n_msingle = 0;
+    short mk[ulm::kVolMirrorMaxAngles] = {};
 };
 
 struct Aperture {
@@ -234,6 +239,48 @@ cudaError_t build_tx_tables(const ulm_rca_plan &P, const Aperture &A, const std:
     return T.f0m.upload(f0m);
 }
 
+// Mirror form of the volume tables: possible when the planes come in pairs (p, n - 1 - p) and the angles in pairs (k, kb)
+// -- or self-mirrored -- with  U0_k(plane p, z) = U0_kb(plane n - 1 - p, z)  to 1e-5 sample (a centred grid and a
+// symmetric angle set with equal start delays; grid parameters that went through fp32 leave ~4e-6 sample on cfg 4, a
+// fraction of the fp32 ulp of the delay sum itself).  The shared table entry is the MEAN of the two delays, so each of
+// the two terms is off by half that difference.  Leaves T.mtab empty otherwise: the caller keeps das_volume_kernel.
+cudaError_t build_mirror_tables(const ulm_rca_plan &P, const Aperture &A, const std::vector<double> &refs, TxTables &T) {
+    const int np = (int)refs.size(), nk = A.n_tx, nz = A.g.n_ax;
+    if (np < 2 || (np & 1) || nk < 1 || nk > ulm::kVolMirrorMaxAngles || nz < 1) return cudaSuccess;
+    std::vector<int> mate(nk, -1);
+    const double za = A.g.z(0), zb = A.g.z(nz - 1);
+    for (int k = 0; k < nk; ++k) {
+        if (mate[k] >= 0) continue;
+        for (int k2 = k; k2 < nk; ++k2) {
+            if (mate[k2] >= 0) continue;
+            double dmax = 0;
+            for (int p = 0; p < np; ++p)
+                for (double z : {za, zb}) dmax = std::max(dmax, std::fabs(u0_of(P, A, k, refs[p], z) - u0_of(P, A, k2, refs[np - 1 - p], z)));
+            if (dmax <= 1e-5) { mate[k] = k2; mate[k2] = k; break; }
+        }
+        if (mate[k] < 0) return cudaSuccess;          // an angle without a mirror partner
+    }
+    std::vector<short> mk;
+    int n_pairs = 0, n_single = 0;
+    for (int k = 0; k < nk; ++k) if (mate[k] > k) { mk.push_back((short)k); mk.push_back((short)mate[k]); ++n_pairs; }
+    for (int k = 0; k < nk; ++k) if (mate[k] == k) { mk.push_back((short)k); ++n_single; }
+    const size_t kpad = ((size_t)mk.size() + 1) / 2 * 2;
+    std::vector<int2> tab((size_t)(np / 2) * nz * kpad, make_int2(0, 0));
+    for (int p = 0; p < np / 2; ++p)
+        for (int iz = 0; iz < nz; ++iz)
+            for (size_t sl = 0; sl < mk.size(); ++sl) {
+                const double u0 = 0.5 * (u0_of(P, A, mk[sl], refs[p], A.g.z(iz)) + u0_of(P, A, mate[mk[sl]], refs[np - 1 - p], A.g.z(iz)));
+                const double fl = std::floor(u0);
+                const float f0m = (float)(u0 - fl - 0.5);
+                int bits;
+                std::memcpy(&bits, &f0m, sizeof(bits));
+                tab[((size_t)p * nz + iz) * kpad + sl] = make_int2(bits, (int)fl - P.n_lo);
+            }
+    T.mkpad = (int)kpad; T.n_mpairs = n_pairs; T.n_msingle = n_single;
+    for (size_t sl = 0; sl < mk.size(); ++sl) T.mk[sl] = mk[sl];
+    return T.mtab.upload(tab);
+}
+
 ulm_rca_status build_demod(ulm_rca_plan &P, int demod_taps) {
     ulm::DemodConst &D = P.demod;
     if (P.input_kind == 1) {
@@ -339,6 +386,8 @@ ulm::DasParams das_params(const ulm_rca_plan &P, const Aperture &A, const TxTabl
     D.fcfs = (float)(P.fc / P.fs);
     D.n_planes = T.n_planes;
     D.rows = P.vol_rows.as<float4>(); D.tab = T.tab.as<int2>(); D.tab_kpad = T.kpad;
+    D.mtab = T.mtab.as<int2>(); D.mtab_kpad = T.mkpad; D.n_mpairs = T.n_mpairs; D.n_msingle = T.n_msingle;
+    for (int i = 0; i < ulm::kVolMirrorMaxAngles; ++i) D.mk[i] = T.mk[i];
     return D;
 }
 
@@ -389,8 +438,17 @@ void launch_unpack(const ulm_rca_plan &P, int n_frames, int f, cudaStream_t st) 
     ++P.last_launches;
 }
 
+constexpr int kVolMirrorPlanes = 2;      // planes of the lower half per thread of das_volume_mirror_kernel (+ their mirrors)
+
 void launch_volume(const ulm_rca_plan &P, const ulm::DasParams &D, cudaStream_t st) {
     if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
+    if (D.mtab && !getenv("ULM_VOL_NOMIRROR")) {      // mirror-symmetric planes and angles: two gathers per index computation
+        const dim3 grid((D.n_lat * D.n_ax + 127) / 128, (D.n_planes / 2 + kVolMirrorPlanes - 1) / kVolMirrorPlanes);
+        if (P.apod) ulm::das_volume_mirror_kernel<kVolMirrorPlanes, true><<<grid, 128, 0, st>>>(D);
+        else ulm::das_volume_mirror_kernel<kVolMirrorPlanes, false><<<grid, 128, 0, st>>>(D);
+        ++P.last_launches;
+        return;
+    }
     const dim3 grid((D.n_lat * D.n_ax + 127) / 128, (D.n_planes + kVolPlanes - 1) / kVolPlanes);
     if (P.apod) ulm::das_volume_kernel<kVolPlanes, true><<<grid, 128, 0, st>>>(D);
     else ulm::das_volume_kernel<kVolPlanes, false><<<grid, 128, 0, st>>>(D);
@@ -642,6 +700,7 @@ ulm_rca_status ulm_rca_plan_create(const ulm_rca_geometry *geo, const float *row
             std::vector<int> all(A.n_tx);
             for (int k = 0; k < A.n_tx; ++k) all[k] = k;
             CUDA_TRY(build_tx_tables(P, A, vol_refs[a], all, A.vol, true));
+            CUDA_TRY(build_mirror_tables(P, A, vol_refs[a], A.vol));
         }
     }
 

@@ -510,6 +510,8 @@ __global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constan
 }
 
 // One aperture (image) of the generic DAS kernel.
+constexpr int kVolMirrorMaxAngles = 32;
+
 struct DasParams {
     const unsigned char *iq;
     int l_row, n_rx_max, n_events;
@@ -531,6 +533,12 @@ struct DasParams {
     const float4 *rows;              // [event][rx elem (n_rx_max)][l_row] {mid.re, mid.im, d.re, d.im} of ONE frame, fp32
     const int2 *tab;                 // [plane][iz][k (tab_kpad, even)] {bits of f0m, n0}
     int tab_kpad;
+    // mirror form of the same table (das_volume_mirror_kernel; nullptr when the geometry is not mirror-symmetric):
+    // [plane < n_planes / 2][iz][slot (mtab_kpad, even)]; slots 2 i, 2 i + 1 = angles mk[2 i], mk[2 i + 1] = a pair
+    // (th, -th), i < n_mpairs; then one slot per self-mirrored angle (th = 0), mk[2 n_mpairs + i], i < n_msingle
+    const int2 *mtab;
+    int mtab_kpad, n_mpairs, n_msingle;
+    short mk[kVolMirrorMaxAngles];
 };
 
 // the interpolation weight a' = a - 0.5 of one gather: al (fp32) for full entries; ah = 16 a' rounded to fp16 for
@@ -872,6 +880,103 @@ __global__ void __launch_bounds__(128) das_volume_kernel(DasParams P) {
         float2 v = make_float2(ar[q], ai[q]);
         if (P.accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
         *dst = v;
+    }
+}
+
+// The volume DAS on MIRROR PAIRS.  On a centred grid with a symmetric angle set the transmit delay of (plane y, angle th)
+// equals that of (plane -y, angle -th): the split delay, the entry index, the interpolation weight and the phasor E(a)
+// of a term -- all that a single frame cannot share with other frames -- are computed once and serve two gathers (row
+// of event th into plane y, row of event -th into plane -y); the table entry is read once as well.  An angle th = 0 has
+// the same delay on every plane pair: one gather serves both planes.  Thread = one (lateral, depth) pixel x NPH planes
+// of the lower half and their mirrors; lanes = lateral neighbours as in das_volume_kernel.
+template <int NPH, bool APOD>
+__global__ void __launch_bounds__(128) das_volume_mirror_kernel(DasParams P) {
+    const int npix = P.n_lat * P.n_ax;
+    const int p = blockIdx.x * 128 + threadIdx.x;
+    if (p >= npix) return;
+    const int il = p % P.n_lat, iz = p / P.n_lat;
+    const int half = P.n_planes / 2, plane0 = blockIdx.y * NPH;
+    const float xs = P.xs[il], zs = P.zs[iz];
+    const float zs2 = zs * zs;
+    const float th = kTwoPi * P.fcfs, th0 = 0.5f * th;
+    float ar[2][NPH], ai[2][NPH];
+    const int2 *tq[NPH];
+#pragma unroll
+    for (int q = 0; q < NPH; ++q) {
+        ar[0][q] = ai[0][q] = ar[1][q] = ai[1][q] = 0.f;
+        tq[q] = P.mtab + ((size_t)min(plane0 + q, half - 1) * P.n_ax + iz) * P.mtab_kpad;
+        asm("" : "+l"(tq[q]));
+    }
+    const size_t ev_stride = (size_t)P.n_rx_max * P.l_row;
+    struct Idx { int idx; float al, c, s; };
+    auto index_of = [&](int tf, int tn, float H, float w) {
+        Idx r;
+        const float upm = __int_as_float(tf) + H;
+        const float tt = upm + kMagic;
+        r.al = upm - (tt - kMagic);
+        r.idx = tn + (__float_as_int(tt) - kMagicBits);
+        __sincosf(fmaf(th, r.al, th0), &r.s, &r.c);          // E(a), a = al + 0.5 in [0, 1]
+        if (APOD) { r.s *= w; r.c *= w; }
+        return r;
+    };
+    auto mac = [&](const float4 e, const Idx &x, float &accr, float &acci) {
+        const float vr = fmaf(x.al, e.z, e.x), vi = fmaf(x.al, e.w, e.y);
+        accr = fmaf(x.c, vr, accr); accr = fmaf(-x.s, vi, accr);
+        acci = fmaf(x.s, vr, acci); acci = fmaf(x.c, vi, acci);
+    };
+    const float4 *rows0 = P.rows + (size_t)P.e0 * ev_stride;
+    for (int j = 0; j < P.n_rx; ++j) {
+        const float dxs = xs - P.ejs[j];
+        const float dx2 = dxs * dxs;
+        const float den = sqrtf(dx2 + zs2) + zs;
+        const float H = den > 0.f ? __fdividef(dx2, den) : 0.f;
+        float w = 1.f;
+        if (APOD) {
+            w = P.win[j];
+            if (P.two_f > 0.f) {
+                const float lhs = __fmul_rn(fabsf(__fsub_rn(P.xm[il], P.ejm[j])), P.two_f);
+                if (!(lhs <= P.zm[iz])) w = 0.f;
+            }
+            if (w == 0.f) continue;
+        }
+        const float4 *rowj = rows0 + (size_t)j * P.l_row;
+        for (int i = 0; i < P.n_mpairs; ++i) {
+            const float4 *ra = rowj + (size_t)P.mk[2 * i] * ev_stride, *rb = rowj + (size_t)P.mk[2 * i + 1] * ev_stride;
+            asm("" : "+l"(ra), "+l"(rb));
+#pragma unroll
+            for (int q = 0; q < NPH; ++q) {
+                const int4 t = __ldg(reinterpret_cast<const int4 *>(tq[q] + 2 * i));
+                const Idx x1 = index_of(t.x, t.y, H, w);      // (plane, th) and (mirror plane, -th)
+                mac(__ldg(ra + x1.idx), x1, ar[0][q], ai[0][q]);
+                mac(__ldg(rb + x1.idx), x1, ar[1][q], ai[1][q]);
+                const Idx x2 = index_of(t.z, t.w, H, w);      // (plane, -th) and (mirror plane, th)
+                mac(__ldg(rb + x2.idx), x2, ar[0][q], ai[0][q]);
+                mac(__ldg(ra + x2.idx), x2, ar[1][q], ai[1][q]);
+            }
+        }
+        for (int i = 0; i < P.n_msingle; ++i) {
+            const float4 *ra = rowj + (size_t)P.mk[2 * P.n_mpairs + i] * ev_stride;
+#pragma unroll
+            for (int q = 0; q < NPH; ++q) {
+                const int2 t = __ldg(tq[q] + 2 * P.n_mpairs + i);
+                const Idx x = index_of(t.x, t.y, H, w);
+                const float4 e = __ldg(ra + x.idx);
+                mac(e, x, ar[0][q], ai[0][q]);
+                mac(e, x, ar[1][q], ai[1][q]);
+            }
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NPH; ++q) {
+        if (plane0 + q >= half) break;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int pl = h == 0 ? plane0 + q : P.n_planes - 1 - (plane0 + q);
+            float2 *dst = P.out + P.out_base + (long long)il * P.s_lat + (long long)pl * P.s_plane + iz;
+            float2 v = make_float2(ar[h][q], ai[h][q]);
+            if (P.accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
+            *dst = v;
+        }
     }
 }
 
