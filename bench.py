@@ -772,7 +772,8 @@ def run_volume(args):
         "gather_samples_per_s": gathers / (ms * 1e-3),
         "projection_path_ms_same_frame": ms_proj, "volume_over_projection_time": ms / ms_proj,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": 19.985152e6 + 0.501760e6, "kernel": "das_volume_kernel<4,0>"},
+                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None,
+                     "kernel": "das_volume_mirror_kernel<3,0> (das_volume_kernel<4,0> when the planes / angles are not mirror-symmetric)"},
         "gpu_launches": launches * args.steps}))
 
 

@@ -150,7 +150,8 @@ ulm_rca_status ulm_rca_beamform(const ulm_rca_plan *plan, const void *d_channel,
  * Conventional full 3-D DAS (step 4) on the grid x = grid_xz lateral, y = grid_yz lateral, z = the
  * (shared) axial grid: d_out_volume is complex fp32 [frame][x][y][z], z fastest.  Same stream and
  * ownership rules as ulm_rca_beamform.  Needs options.build_volume = 1.  Batches (max_frames) of one or two
- * frames are beamformed frame by frame from fp32 rows (das_volume_kernel), larger ones by the generic kernel.
+ * frames are beamformed frame by frame from fp32 rows (das_volume_mirror_kernel on mirror-symmetric planes and
+ * angles, else das_volume_kernel), larger ones by the generic kernel.
  */
 ulm_rca_status ulm_rca_beamform_volume(const ulm_rca_plan *plan, const void *d_channel,
                                        int32_t n_frames, void *d_out_volume, void *cuda_stream);

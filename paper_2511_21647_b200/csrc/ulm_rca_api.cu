@@ -438,11 +438,11 @@ void launch_unpack(const ulm_rca_plan &P, int n_frames, int f, cudaStream_t st) 
     ++P.last_launches;
 }
 
-constexpr int kVolMirrorPlanes = 2;      // planes of the lower half per thread of das_volume_mirror_kernel (+ their mirrors)
+constexpr int kVolMirrorPlanes = 3;      // planes of the lower half per thread of das_volume_mirror_kernel (+ their mirrors)
 
 void launch_volume(const ulm_rca_plan &P, const ulm::DasParams &D, cudaStream_t st) {
     if (D.n_tx == 0 || D.n_lat * D.n_ax == 0) return;
-    if (D.mtab && !getenv("ULM_VOL_NOMIRROR")) {      // mirror-symmetric planes and angles: two gathers per index computation
+    if (D.mtab) {      // mirror-symmetric planes and angles: two gathers per index computation
         const dim3 grid((D.n_lat * D.n_ax + 127) / 128, (D.n_planes / 2 + kVolMirrorPlanes - 1) / kVolMirrorPlanes);
         if (P.apod) ulm::das_volume_mirror_kernel<kVolMirrorPlanes, true><<<grid, 128, 0, st>>>(D);
         else ulm::das_volume_mirror_kernel<kVolMirrorPlanes, false><<<grid, 128, 0, st>>>(D);
