@@ -477,7 +477,10 @@ cudaError_t launch_demod_f(const ulm_rca_plan &P, const ulm::DemodParams &D, dim
         // fill the GPU; few rows (single-frame calls) keep one CTA per chunk
         dim3 qb = blocks;
         if ((long long)blocks.y * blocks.z >= 2048) qb.x = 1;
-        ulm::demod_quad_kernel<F, D32><<<qb, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
+        // aligned int16 pairs when every record starts 4-byte aligned and has an even length
+        const bool pair = (D.n_samples & 1) == 0 && (reinterpret_cast<unsigned long long>(D.rf) & 3ull) == 0;
+        if (pair) ulm::demod_quad_kernel<F, D32, true><<<qb, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
+        else ulm::demod_quad_kernel<F, D32, false><<<qb, 256, ulm::demod_quad_smem_bytes(F, D32), st>>>(D);
         return cudaSuccess;
     }
     if (L == 8) return P.half_band ? launch_demod_t<17, 2, false, F, D32>(D, L, blocks, st)

@@ -399,7 +399,9 @@ __device__ __forceinline__ void demod_quad_emit(const float (&A)[9], const float
     }
 }
 
-template <int F, bool D32>
+// PAIR: the raw samples are read as aligned int16 pairs (one 4-byte load for two samples; needs an even record length):
+// column c of a staging row then holds sample base - L - (n_lo & 1) + c and the filter reads one column further right.
+template <int F, bool D32, bool PAIR = false>
 __global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constant__ DemodParams P) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     constexpr int EB = entry_bytes(F, D32);
@@ -430,11 +432,26 @@ __global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constan
     const int16_t *rec = P.rf + (long long)min(fr0, P.n_frames - 1) * frame_stride +
                          ((long long)ev.x * P.channels_per_event + ch) * (long long)P.n_samples;
     const long long off_b = two ? (long long)(ev.y - ev.x) * P.channels_per_event * (long long)P.n_samples : 0;
-    const bool second = i0 + 128 < XW;
+    const bool second = !PAIR && i0 + 128 < XW;
+    const int odd = PAIR ? (P.n_lo & 1) : 0;                    // L and kDemodChunk are even: the same for every chunk
+    constexpr int NPAIRS = (XW + 2) / 2;
     int ra[2][FH], rb[2][FH];        // prefetched samples of the next chunk: [sample column][frame], first / second event
     // unconditional loads from clamped addresses (out-of-range samples and frames are zeroed when they are consumed)
     auto issue_loads = [&](int chunk) {
         const int base = P.n_lo + chunk * kDemodChunk;
+        if (PAIR) {
+            if (i0 < NPAIRS) {
+                const int n = base - L - odd + 2 * i0;           // even: the pair (n, n + 1) is 4-byte aligned, both in or both out
+                const int *src = reinterpret_cast<const int *>(rec + min(max(n, 0), P.n_samples - 2));
+#pragma unroll
+                for (int f = 0; f < FH; ++f) {
+                    ra[0][f] = __ldg(src);
+                    rb[0][f] = two ? __ldg(src + off_b / 2) : 0;
+                    if (f < f_last) src += frame_stride / 2;
+                }
+            }
+            return;
+        }
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
             if (rep == 1 && !second) break;
@@ -450,6 +467,21 @@ __global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constan
     };
     auto store_x = [&](int chunk) {
         const int base = P.n_lo + chunk * kDemodChunk;
+        if (PAIR) {
+            if (i0 < NPAIRS) {
+                const int n = base - L - odd + 2 * i0, c = 2 * i0;
+                const bool inb = n >= 0 && n < P.n_samples;
+                float *dst = s_x + (h * FH) * XS + c + 4 * (c >> 3);
+#pragma unroll
+                for (int f = 0; f < FH; ++f) {
+                    const int va = ra[0][f], vb = rb[0][f];
+                    const bool ok = inb && f <= f_last;
+                    dst[f * XS] = ok ? (float)((int)(short)(va & 0xffff) + (int)(short)(vb & 0xffff)) : 0.f;
+                    dst[f * XS + 1] = ok ? (float)((va >> 16) + (vb >> 16)) : 0.f;
+                }
+            }
+            return;
+        }
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
             if (rep == 1 && !second) break;
@@ -480,12 +512,14 @@ __global__ void __launch_bounds__(256, 4) demod_quad_kernel(const __grid_constan
         if (f < F && ((threadIdx.x & ~31) / TPG) * 8 < n_ent) {
             const int r0 = grp * 8;
             const float *x = s_x + f * XS + r0 + (r0 >> 1);         // r0 + 4 (r0 >> 3)
+            // PAIR: column u + odd; one step to the right crosses a padded group boundary after u = 7 mod 8
+            const float *x1 = x + odd, *x5 = x + 5 * odd;
             float A[9], B[9];
 #pragma unroll
             for (int q = 0; q < 9; ++q) B[q] = 0.f;
 #pragma unroll
             for (int u = 0; u < 9 + 2 * L; ++u) {
-                const float xv = x[u + 4 * (u >> 3)];
+                const float xv = PAIR ? ((u & 7) == 7 ? x5 : x1)[u + 4 * (u >> 3)] : x[u + 4 * (u >> 3)];
 #pragma unroll
                 for (int q = 0; q < 9; ++q) {
                     const int t = q - u + 2 * L;                    // tap m = t - L
