@@ -185,6 +185,8 @@ ulm_rca_status ulm_rca_plan_sizes(const ulm_rca_plan *plan, size_t *channel_byte
  *   [18] .. [21] the ring kernel's work items of TWO frame groups (24 frames x 2 pixel rows per thread; used by calls
  *        of more than 12 frames when the scratch holds compact entries; 0 = not planned): window entries per group and
  *        stage, ring stages (each holds both groups' windows), tiles per projection x-z, y-z
+ *   [22] 1 when single-frame volumes (ulm_rca_beamform_volume) run on mirror pairs: planes and angles of every
+ *        aperture are mirror-symmetric (centred grid, symmetric angle set, equal start delays), 0 otherwise
  * [4] .. [9], [11] describe the work items of one frame group (12 frames x 4 pixel rows per thread). */
 ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *values, int32_t n);
 

@@ -134,7 +134,7 @@ def _farr(v):
 
 INFO_KEYS = ["n_lo", "l_row", "iq_scratch_bytes", "kernel", "frames_per_thread", "tile_pixels", "window",
              "stages", "tiles_xz", "smem_bytes", "launches_last_call", "tiles_yz", "precision", "scratch_bytes_per_sample", "host_upload_bytes_per_frame", "events_executed",
-             "stage2_taps", "stage2_tile_cols", "window_two_groups", "stages_two_groups", "tiles_xz_two_groups", "tiles_yz_two_groups"]
+             "stage2_taps", "stage2_tile_cols", "window_two_groups", "stages_two_groups", "tiles_xz_two_groups", "tiles_yz_two_groups", "volume_mirror_pairs"]
 
 
 LOCALIZE_STATIC_MAX_FRAMES = 4096        # ULM_RCA_LOCALIZE_STATIC_MAX_FRAMES of include/ulm_rca.h

@@ -802,7 +802,8 @@ ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n
     if (!plan || !v || n < 0) return fail(ULM_RCA_EINVAL, "plan/values is NULL");
     const bool ring = plan->kernel == 2, d32 = plan->d32;
     const bool dual = ring && plan->ring.window2 > 0;
-    const int64_t vals[22] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
+    const bool vmirror = plan->build_volume && ((plan->ap[0].n_tx == 0 || plan->ap[0].vol.mtab.p) && (plan->ap[1].n_tx == 0 || plan->ap[1].vol.mtab.p));
+    const int64_t vals[23] = {plan->n_lo, plan->l_row, (int64_t)plan->iq_bytes, plan->kernel, 12,
                               ring ? ulm::kRingConsumers * ulm::kRingPx : 128, ring ? plan->ring.window : 0,
                               ring ? ulm::ring_stages(plan->ring.window, 12, d32) : 0, ring ? plan->ap[0].ring.n_tiles : 0,
                               ring ? ulm::ring_smem_bytes(plan->ring.window, 12, d32) : 0, plan->last_launches,
@@ -810,8 +811,8 @@ ulm_rca_status ulm_rca_plan_info(const ulm_rca_plan *plan, int64_t *v, int32_t n
                               (int64_t)host_upload_bytes_per_frame(*plan), plan->nv_events,
                               plan->s2.ready ? plan->s2.nt : 0, plan->s2.ready ? plan->s2.ncol : 0,
                               dual ? plan->ring.window2 : 0, dual ? ulm::ring_dual_stages(plan->ring.window2) : 0,
-                              dual ? plan->ap[0].ring2.n_tiles : 0, dual ? plan->ap[1].ring2.n_tiles : 0};
-    for (int i = 0; i < n && i < 22; ++i) v[i] = vals[i];
+                              dual ? plan->ap[0].ring2.n_tiles : 0, dual ? plan->ap[1].ring2.n_tiles : 0, vmirror ? 1 : 0};
+    for (int i = 0; i < n && i < 23; ++i) v[i] = vals[i];
     return ULM_RCA_OK;
 }
 

@@ -421,6 +421,36 @@ def test_volume_small(torch_cuda, n_frames, precision):
         assert rel_err(vol[f], v_rc + v_cr) <= TOL
 
 
+@pytest.mark.parametrize("nx,ny,sym,f_number", [(18, 14, True, 0.0), (18, 14, True, 1.4), (19, 14, True, 0.0), (18, 14, False, 1.4)])
+def test_volume_mirror_pairs(torch_cuda, nx, ny, sym, f_number):
+    """Single-frame volumes on mirror pairs (das_volume_mirror_kernel): centred grids with an even plane count, an angle
+    set symmetric about 0 (with a theta = 0 event) and equal start delays share the index / weight / phasor arithmetic
+    between (plane y, theta) and (plane -y, -theta); an odd plane count or an asymmetric angle set keeps
+    das_volume_kernel.  Plane counts off the 3-planes-per-thread grouping (9 and 7 lower-half planes)."""
+    torch = torch_cuda
+    from paper_2511_21647_b200 import Plan
+    d = synth.LAMBDA_M / 2
+    gx = centred_grid(nx, d, 33, 6e-3, d, ref=0.0)
+    gy = centred_grid(ny, 1.3 * d, 33, 6e-3, d, ref=0.0)
+    row = np.radians([-7.0, -2.5, 0.0, 2.5, 7.0]) if sym else np.radians([-7.0, 1.0, 6.0])
+    col = np.radians([-4.0, 4.0]) if sym else np.radians([-4.0, 8.0])
+    cfg = small(grid_xz=gx, grid_yz=gy, n_frames=2, f_number=f_number, row_tx_angles=tuple(row), col_tx_angles=tuple(col),
+                t0=None if sym else (0.2e-6, -0.1e-6, 0.05e-6, 0.3e-6, -0.25e-6))
+    ch = synth.random_channel(cfg, 2, seed=43, amplitude=6000)
+    kw = rounded_kwargs(cfg)
+    assert_mask_margin(kw)
+    p = oracle.OracleParams(**kw)
+    xs = kw["grid_xz"][1] + kw["grid_xz"][2] * np.arange(gx[0])
+    ys = kw["grid_yz"][1] + kw["grid_yz"][2] * np.arange(gy[0])
+    zs = kw["grid_xz"][4] + kw["grid_xz"][5] * np.arange(gx[3])
+    with Plan(**kw, build_volume=True, precision=2) as plan:
+        vol = plan.beamform_volume(torch.from_numpy(ch).cuda()).cpu().numpy()
+        assert plan.info()["volume_mirror_pairs"] == int(sym and nx % 2 == 0 and ny % 2 == 0)
+    for f in range(2):
+        v_rc, v_cr = oracle.volume(p, ch[f], xs, ys, zs)
+        assert rel_err(vol[f], v_rc + v_cr) <= NOISE_TOL_FULL
+
+
 def test_config1_full_frame(torch_cuda):
     cfg = synth.config(1)
     ch = synth.render(cfg)
