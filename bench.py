@@ -88,6 +88,16 @@ def measured_traffic(config_index: int, precision: int):
         return None
 
 
+def capture_traffic(name: str):
+    """The same figure for the dominant kernel of another workload (profiles/r02_traffic.json, section "captures")."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as fh:
+            rec = json.load(fh)["captures"][name]
+        return float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
+    except Exception:
+        return None
+
+
 DTYPE_OF_PRECISION = {1: "f32 accumulate; staged IQ: fp24 mid + fp16 difference, fp16 weight (precision=1, compact-fast)",
                       2: "f32 (staged IQ, interpolation and accumulation all fp32; precision=2)",
                       3: "f32 accumulate; staged IQ: fp24 mid + fp16 difference, two-term fp16 weight (precision=3, compact)"}
@@ -417,7 +427,7 @@ def run_stage2(args):
         "kernels_ms": {"groupsum": gs_ms, "project": pj_ms},
         "roofline": {"bound": "alu", "achieved": flop_exec / (pj_ms * 1e-3) / 1e12, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
                      "frac": flop_exec / (pj_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS, "peak_measured": fp32_probe,
-                     "frac_of_measured": flop_exec / (pj_ms * 1e-3) / 1e12 / fp32_probe, "traffic": None,
+                     "frac_of_measured": flop_exec / (pj_ms * 1e-3) / 1e12 / fp32_probe, "traffic": capture_traffic("r02_stage2"),
                      "kernel": "stage2_project_kernel<%d>" % info["stage2_taps"], "kernel_ms": pj_ms,
                      "executed_complex_macs": cmac, "flop_executed": flop_exec, "flop_of_the_definition": flop_def,
                      "frac_on_definition_count": flop_def / (pj_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
@@ -504,7 +514,7 @@ def run_clutter(args):
                    "l2_policy": "inputs (%.2f GB) larger than L2, no flush" % (d_x.numel() * 8 / 1e9), "plan": info},
         "kernels_ms": k_ms,
         "roofline": {"bound": "tensor", "achieved": flop_alg / (k_ms["gram"] * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
-                     "frac": flop_alg / (k_ms["gram"] * 1e-3) / 1e12 / peak, "traffic": None, "kernel": "clutter_gram_kernel",
+                     "frac": flop_alg / (k_ms["gram"] * 1e-3) / 1e12 / peak, "traffic": capture_traffic("r02_clutter"), "kernel": "clutter_gram_kernel",
                      "kernel_ms": k_ms["gram"], "flop_algorithmic": flop_alg, "flop_executed": flop_exec,
                      "achieved_executed": flop_exec / (k_ms["gram"] * 1e-3) / 1e12,
                      "frac_executed": flop_exec / (k_ms["gram"] * 1e-3) / 1e12 / peak, "peak_source": src},
@@ -772,7 +782,7 @@ def run_volume(args):
         "gather_samples_per_s": gathers / (ms * 1e-3),
         "projection_path_ms_same_frame": ms_proj, "volume_over_projection_time": ms / ms_proj,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None,
+                     "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": capture_traffic("r02_cfg4_volume"),
                      "kernel": "das_volume_mirror_kernel<3,0> (das_volume_kernel<4,0> when the planes / angles are not mirror-symmetric)"},
         "gpu_launches": launches * args.steps}))
 
